@@ -1,0 +1,483 @@
+"""CPU ORACLE for the ViBE per-GPU MoE-layer hot path.  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this module.  The product (paper_2606_00735_b200/) never does, and
+this module imports nothing from the product except nothing at all: inputs arrive
+as numpy arrays produced by paper_2606_00735_b200.inputs (the seeded generators).
+
+What it is: a plain, slow, obviously-correct numpy (fp64 unless stated) statement
+of what each C-ABI call computes, written from PAPER.md (ViBE, arxiv 2606.00735)
+and, where the paper is silent (it treats the fused MoE kernel as a black box,
+PAPER.md L176/L220/L420), from the readings listed in DESIGN.md ("Readings").
+No blocking, no fusion, no reordering beyond the definitions.
+
+Citations:  P:L<n> = /root/reference/PAPER.md line n;  R*/P*/F*/C*/M*/L* = DESIGN.md reading ids.
+
+Pins (tests/test_oracle_*.py, all `-m "not gpu"`): every function below is pinned to
+something other than itself -- brute force, closed forms, library routines
+(scipy.special.softmax/expit, np.argsort(kind='stable'), torch CPU fp64 matmul+silu),
+hand-worked golden fixtures in tests/golden/.  The only unpinned item is the latency
+*profile* (a measurement; nothing to pin numerically) -- its *model* (O5) is pinned.
+"""
+from __future__ import annotations
+
+import itertools
+import numpy as np
+
+SCORE_SOFTMAX = 0
+SCORE_SIGMOID = 1
+
+# ======================================================================================
+# bf16 helpers (the oracle's own copy; the CUDA path has its own)
+# ======================================================================================
+
+def bf16_bits_to_f64(b):
+    """bf16 bit pattern (uint16) -> exact value in f64."""
+    b = np.ascontiguousarray(b, dtype=np.uint16)
+    return (b.astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+
+
+def f64_to_bf16_bits(x):
+    """Round an f64 array to bf16 with round-to-nearest-even, in one rounding
+    (not via f32, which could double-round).  Inputs must be finite and within
+    bf16 normal range or zero (true for every tensor on this path; F4)."""
+    x = np.asarray(x, dtype=np.float64)
+    m, e = np.frexp(x)                     # x = m * 2^e, 0.5 <= |m| < 1
+    # bf16 has 8 significant bits: quantum = 2^(e-8); subnormal floor at 2^-133
+    q = np.ldexp(1.0, np.maximum(e - 8, -133))
+    r = np.rint(x / q) * q                 # np.rint = round-half-to-even
+    r32 = r.astype(np.float32)             # exact: r has <= 8 significant bits
+    u = r32.view(np.uint32)
+    assert np.all((u & np.uint32(0xFFFF)) == 0), "bf16 rounding produced non-bf16 value"
+    return (u >> np.uint32(16)).astype(np.uint16)
+
+
+def bf16_round_f64(x):
+    """x (f64) -> nearest bf16 value, returned as f64."""
+    return bf16_bits_to_f64(f64_to_bf16_bits(x))
+
+
+# ======================================================================================
+# O1  route top-k  +  O1.6 activation histogram      (a1, a2)
+# The paper only says "route each token to a subset of experts" and
+# profiles "expert activation" into W in R^{LxE}.  Readings R1-R8.
+# ======================================================================================
+
+_F = np.float32
+_LOG2E = _F(1.4426950408889634)
+_LN2_HI = _F(0.693359375)            # 355/512, 9 significant bits: n*LN2_HI exact for |n|<2^15
+_LN2_LO = _F(-2.12194440e-4)         # ln2 - LN2_HI
+_VSIG_COEF = [_F(1.0 / 5040.0), _F(1.0 / 720.0), _F(1.0 / 120.0), _F(1.0 / 24.0),
+              _F(1.0 / 6.0), _F(0.5), _F(1.0), _F(1.0)]      # Taylor e^r, degree 7, high -> low
+
+
+def vsig_f32(x):
+    """Reproducible f32 sigmoid used ONLY as the selection key (reading R2).
+
+    Defined as this exact sequence of individually, correctly rounded IEEE-754
+    binary32 operations (no fused multiply-add anywhere), so that a CPU and a GPU
+    evaluating it agree bit for bit:
+        x  = min(max(x,-80),80);  a = -x
+        n  = rint(a*LOG2E)                       (round half to even)
+        r  = (a - n*LN2_HI) - n*LN2_LO           (Cody-Waite; 3 roundings)
+        p  = (((((((c7*r + c6)*r + c5)*r + c4)*r + c3)*r + c2)*r + c1)*r + c0
+             each * and each + rounded separately; c_j = f32(1/j!)
+        e  = p * 2^n                             (exact scaling; |n| <= 116 keeps it normal)
+        vsig = 1 / (1 + e)                       (one add, one IEEE division)
+    numpy evaluates every ufunc on float32 arrays as a separate correctly rounded
+    binary32 operation, which is exactly this definition.
+    """
+    x = np.asarray(x, dtype=_F)
+    x = np.minimum(np.maximum(x, _F(-80.0)), _F(80.0))
+    a = -x
+    n = np.rint(a * _LOG2E)
+    r = a - n * _LN2_HI
+    r = r - n * _LN2_LO
+    p = np.full_like(r, _VSIG_COEF[0])
+    for c in _VSIG_COEF[1:]:
+        p = p * r
+        p = p + c
+    e = np.ldexp(p, n.astype(np.int32))
+    assert e.dtype == _F
+    one = _F(1.0)
+    return one / (one + e)
+
+
+def route_topk(logits, num_experts, top_k, score_fn=SCORE_SOFTMAX, renormalize=1,
+               routed_scale=1.0, n_group=0, topk_group=0, select_bias=None):
+    """O1 steps 1-6.  logits f32 [T,E] -> (topk_ids i32 [T,k], topk_w f32 [T,k], counts i32 [E]).
+
+    1. x[e] = logits[t,e]
+    2. key: softmax -> x (select on the raw logits, softmax is monotone; R2);
+            sigmoid -> vsig(x) + select_bias (one f32 add; bias is selection-only; R1,R7)
+    3. group limiting (R6): contiguous groups of E/n_group; group score = largest key +
+       second largest key (one f32 add); keep the topk_group best groups (ties -> lower
+       group index); key = -inf elsewhere
+    4. k rounds of arg-max, ties -> lowest expert index (R3); ids in pick order
+    5. weights in f64, rounded once to f32: softmax over ALL E experts (R1) or the true
+       sigmoid 1/(1+e^-x) (bias excluded); optional renormalisation over the k picked
+       (R4: no epsilon); times routed_scale (R5)
+    6. counts[e] = number of assignments with id e, over GLOBAL experts (R8; one row of
+       the activation matrix W of P:L178)
+    """
+    x = np.ascontiguousarray(logits, dtype=np.float32)
+    T, E = x.shape
+    k = int(top_k)
+    assert E == num_experts and 1 <= k <= E
+    # step 2
+    if score_fn == SCORE_SOFTMAX:
+        key = x.copy()
+    else:
+        s32 = vsig_f32(x)
+        key = s32 if select_bias is None else (s32 + np.asarray(select_bias, dtype=_F)[None, :])
+        assert key.dtype == _F
+    key = key + _F(0.0)                      # -0.0 -> +0.0 (they compare equal anyway)
+    # step 3
+    if n_group and n_group > 1:
+        assert E % n_group == 0 and 1 <= topk_group <= n_group and topk_group * (E // n_group) >= k
+        gs = E // n_group
+        kg = key.reshape(T, n_group, gs)
+        srt = np.sort(kg, axis=2)
+        if gs >= 2:
+            gscore = srt[:, :, -1] + srt[:, :, -2]          # f32 add: larger + second
+        else:
+            gscore = srt[:, :, -1]
+        assert gscore.dtype == _F
+        keep = np.zeros((T, n_group), dtype=bool)
+        g = gscore.copy()
+        for _ in range(topk_group):
+            best = np.argmax(g, axis=1)                      # first occurrence = lowest group index
+            keep[np.arange(T), best] = True
+            g[np.arange(T), best] = -np.inf
+        key = np.where(np.repeat(keep, gs, axis=1), key, _F(-np.inf)).astype(_F)
+    # step 4
+    ids = np.empty((T, k), dtype=np.int32)
+    kk = key.copy()
+    rows = np.arange(T)
+    for j in range(k):
+        best = np.argmax(kk, axis=1)                         # first occurrence = lowest index
+        ids[:, j] = best
+        kk[rows, best] = -np.inf
+    # step 5
+    xd = x.astype(np.float64)
+    if score_fn == SCORE_SOFTMAX:
+        ex = np.exp(xd - xd.max(axis=1, keepdims=True))
+        p = ex / ex.sum(axis=1, keepdims=True)
+    else:
+        p = 1.0 / (1.0 + np.exp(-xd))
+    w = np.take_along_axis(p, ids.astype(np.int64), axis=1)
+    if renormalize:
+        w = w / w.sum(axis=1, keepdims=True)
+    w = w * float(routed_scale)
+    # step 6
+    counts = np.zeros(E, dtype=np.int32)
+    for e in ids.ravel():
+        counts[e] += 1
+    return ids, w.astype(np.float32), counts
+
+
+# ======================================================================================
+# O2  permute  (a3): stable counting sort of assignments by local expert slot.
+# "token dispatch remains local" on one GPU; readings P1-P4.
+# ======================================================================================
+
+def permute(X_bits, topk_ids, expert_map, E_loc, align=1):
+    """X bf16 bits [T,d]; topk_ids [T,k]; expert_map[E] -> slot or -1 (None = identity).
+    Returns offsets[E_loc+1], row_to_assign[R_cap], assign_to_row[A], Xp bits [R_cap,d], R
+    where R_cap = offsets[E_loc] and R = number of real rows."""
+    T, k = topk_ids.shape
+    A = T * k
+    flat = topk_ids.reshape(-1)
+    E = int(flat.max()) + 1 if expert_map is None else len(expert_map)
+    emap = np.arange(E, dtype=np.int32) if expert_map is None else np.asarray(expert_map, dtype=np.int32)
+    cnt = np.zeros(E_loc, dtype=np.int64)
+    for i in range(A):
+        s = emap[flat[i]]
+        if s >= 0:
+            cnt[s] += 1
+    offsets = np.zeros(E_loc + 1, dtype=np.int32)
+    for s in range(E_loc):
+        offsets[s + 1] = offsets[s] + ((cnt[s] + align - 1) // align) * align
+    R_cap = int(offsets[E_loc])
+    row_to_assign = np.full(R_cap, -1, dtype=np.int32)
+    assign_to_row = np.full(A, -1, dtype=np.int32)
+    Xp = np.zeros((R_cap, X_bits.shape[1]), dtype=np.uint16)
+    fill = np.zeros(E_loc, dtype=np.int64)
+    for i in range(A):                       # walk assignments in flat order => stable
+        s = emap[flat[i]]
+        if s < 0:
+            continue
+        r = int(offsets[s] + fill[s])
+        fill[s] += 1
+        row_to_assign[r] = i
+        assign_to_row[i] = r
+        Xp[r, :] = X_bits[i // k, :]
+    return offsets, row_to_assign, assign_to_row, Xp, int(cnt.sum())
+
+
+# ======================================================================================
+# O3  grouped SwiGLU FFN (a4): the "fused MoE kernel" ViBE profiles;
+# the dominant cost (49 % of prefill).  Readings F1-F4, C2.
+# ======================================================================================
+
+def swiglu_ffn_rows(x_bits, W1_bits, W3_bits, W2_bits, round_h=True, round_y=False):
+    """One expert on a block of rows.  x bf16 bits [n,d]; W1,W3 [d,f]; W2 [f,d].
+       g = x W1 ; u = x W3 ; h = bf16_rne( g/(1+exp(-g)) * u ) ; y = h W2     (all sums in f64)
+    round_h: H is an MMA operand by contract (F2) -> rounded to bf16.
+    round_y: additionally round Y to bf16 (the 'mirrored' reference; C2 uses round_y=False)."""
+    x = bf16_bits_to_f64(x_bits)
+    g = x @ bf16_bits_to_f64(W1_bits)
+    u = x @ bf16_bits_to_f64(W3_bits)
+    h = (g / (1.0 + np.exp(-g))) * u
+    if round_h:
+        h = bf16_round_f64(h)
+    y = h @ bf16_bits_to_f64(W2_bits)
+    if round_y:
+        y = bf16_round_f64(y)
+    return y, h
+
+
+def grouped_ffn(Xp_bits, offsets, row_to_assign, W1_bits, W3_bits, W2_bits,
+                round_h=True, round_y=False, rows=None):
+    """Y f64 [R_cap,d] (and H f64 [R_cap,f]); padding rows (row_to_assign<0) stay zero.
+    `rows`: optional iterable of row indices to compute (others left NaN) -- used for
+    sampled parity at full size."""
+    E_loc = len(offsets) - 1
+    R_cap, d = Xp_bits.shape
+    f = W1_bits.shape[2]
+    Y = np.zeros((R_cap, d), dtype=np.float64)
+    H = np.zeros((R_cap, f), dtype=np.float64)
+    if rows is not None:
+        Y[:] = np.nan
+        H[:] = np.nan
+        rows = np.asarray(sorted(set(int(r) for r in rows)), dtype=np.int64)
+    for s in range(E_loc):
+        lo, hi = int(offsets[s]), int(offsets[s + 1])
+        sel = np.arange(lo, hi, dtype=np.int64)
+        if rows is not None:
+            sel = rows[(rows >= lo) & (rows < hi)]
+        sel = sel[row_to_assign[sel] >= 0] if len(sel) else sel
+        if len(sel) == 0:
+            continue
+        y, h = swiglu_ffn_rows(Xp_bits[sel], W1_bits[s], W3_bits[s], W2_bits[s], round_h, round_y)
+        Y[sel] = y
+        H[sel] = h
+    if rows is not None:
+        pad = np.nonzero(row_to_assign < 0)[0]
+        Y[pad] = 0.0
+        H[pad] = 0.0
+    return Y, H
+
+
+def ffn_naive_triple_loop(x_bits, W1_bits, W3_bits, W2_bits):
+    """Pure-Python triple loops for tiny shapes (pin for swiglu_ffn_rows); math.fsum-free,
+    plain left-to-right f64 accumulation."""
+    import math
+    x = bf16_bits_to_f64(x_bits).tolist()
+    W1 = bf16_bits_to_f64(W1_bits).tolist()
+    W3 = bf16_bits_to_f64(W3_bits).tolist()
+    W2 = bf16_bits_to_f64(W2_bits).tolist()
+    n, d, f = len(x), len(W1), len(W1[0])
+    Y = [[0.0] * d for _ in range(n)]
+    for r in range(n):
+        h = [0.0] * f
+        for j in range(f):
+            g = 0.0
+            u = 0.0
+            for c in range(d):
+                g += x[r][c] * W1[c][j]
+                u += x[r][c] * W3[c][j]
+            h[j] = (g / (1.0 + math.exp(-g))) * u
+        hb = bf16_round_f64(np.array(h)).tolist()
+        for m in range(d):
+            acc = 0.0
+            for j in range(f):
+                acc += hb[j] * W2[j][m]
+            Y[r][m] = acc
+    return np.array(Y)
+
+
+# ======================================================================================
+# O4  weighted un-permute / combine (a5).  Reading C1.
+# ======================================================================================
+
+def combine(Y, assign_to_row, topk_w, T, k, round_out=False):
+    """out[t,:] = sum_j (f64)w[t,j] * Y[assign_to_row[t*k+j],:] over resident j, slot order."""
+    d = Y.shape[1]
+    out = np.zeros((T, d), dtype=np.float64)
+    w = np.asarray(topk_w, dtype=np.float32).astype(np.float64).reshape(T, k)
+    a2r = np.asarray(assign_to_row).reshape(T, k)
+    for t in range(T):
+        for j in range(k):
+            r = a2r[t, j]
+            if r >= 0:
+                out[t, :] += w[t, j] * Y[r, :]
+    if round_out:
+        out = bf16_round_f64(out)
+    return out
+
+
+def moe_layer_direct(X_bits, topk_ids, topk_w, expert_map, W1_bits, W3_bits, W2_bits, tokens=None):
+    """Independent statement of the whole layer with NO permutation:
+       out[t] = sum_j w[t,j] * FFN_{slot(id[t,j])}(x_t)   (non-resident experts contribute 0).
+    Used to pin permute+ffn+combine together, and as the sampled full-size reference."""
+    T, k = topk_ids.shape
+    d = X_bits.shape[1]
+    toks = range(T) if tokens is None else tokens
+    out = {}
+    for t in toks:
+        acc = np.zeros(d, dtype=np.float64)
+        for j in range(k):
+            s = topk_ids[t, j] if expert_map is None else expert_map[topk_ids[t, j]]
+            if s < 0:
+                continue
+            y, _ = swiglu_ffn_rows(X_bits[t:t + 1], W1_bits[s], W3_bits[s], W2_bits[s])
+            acc += float(np.float32(topk_w[t, j])) * y[0]
+        out[t] = acc
+    if tokens is None:
+        return np.stack([out[t] for t in range(T)])
+    return out
+
+
+# ======================================================================================
+# O5  latency model  f(n)  from profiled points  (a6 -> a7).  P:L176 "produces a function
+# f_g(n) that maps token load n to expected kernel latency"; form unspecified -> M1.
+# ======================================================================================
+
+class LatencyModel:
+    """Monotone piecewise-linear per-expert latency l(n) [us] with l(0)=0, linear
+    extrapolation with the last segment's slope (M1).  E_prof = experts resident when
+    profiled in uniform mode (M2), so the whole-kernel latency is F(n) = E_prof*l(n/E_prof)."""
+
+    def __init__(self, tokens, latency_us, E_prof=1):
+        t = np.asarray(tokens, dtype=np.float64)
+        l = np.asarray(latency_us, dtype=np.float64)
+        assert t.ndim == 1 and t.shape == l.shape and len(t) >= 1 and np.all(np.diff(t) > 0) and t[0] > 0
+        self.tokens = np.concatenate([[0.0], t])
+        self.lat = np.concatenate([[0.0], np.maximum.accumulate(l)])   # enforce non-decreasing
+        self.E_prof = int(E_prof)
+
+    def per_expert(self, n):
+        n = float(n)
+        t, l = self.tokens, self.lat
+        if n <= 0.0:
+            return 0.0
+        if n >= t[-1]:
+            slope = (l[-1] - l[-2]) / (t[-1] - t[-2])
+            return float(l[-1] + slope * (n - t[-1]))
+        i = int(np.searchsorted(t, n, side="right")) - 1
+        return float(l[i] + (l[i + 1] - l[i]) * (n - t[i]) / (t[i + 1] - t[i]))
+
+    def whole_kernel(self, n_total):
+        return self.E_prof * self.per_expert(float(n_total) / self.E_prof)
+
+
+# ======================================================================================
+# O6  placement evaluator (a7):  T = max_g f_g(n_g),  n_g = sum_{e in S_g} w_e
+# with f_g(n) = f(n)/sigma_g (M5).  model kind A: scalar f(n_g) (paper); kind B: per-expert sum (L4).
+# ======================================================================================
+
+MODEL_A = 0
+MODEL_B = 1
+
+
+def placement_eval(assign, load, G, scale, model, model_kind=MODEL_B):
+    """Returns (score, per_bin[G])."""
+    assign = np.asarray(assign)
+    load = np.asarray(load, dtype=np.float64)
+    per_bin = np.zeros(G, dtype=np.float64)
+    for g in range(G):
+        members = [e for e in range(len(load)) if assign[e] == g]
+        if model_kind == MODEL_A:
+            n_g = 0.0
+            for e in members:
+                n_g += load[e]
+            L = model.whole_kernel(n_g)
+        else:
+            L = 0.0
+            for e in members:
+                L += model.per_expert(load[e])
+        per_bin[g] = L / float(scale[g])
+    return float(per_bin.max()), per_bin
+
+
+# ======================================================================================
+# O7  greedy placement (a8):  Algorithm 1 Phase 2 (prose P:L186-L196)
+#     N = sum_e w_e ; s_g = 1/f_g(N/E) ; tau_g = N s_g / sum_h s_h ;
+#     experts in descending w_e ; assign e to argmax_g (tau_g - n_g) ; n_g += w_e
+# Readings L1 (cap), L2 (ties), L3 (token-balanced = sigma==1), M5/M6.
+# ======================================================================================
+
+def placement_greedy(load, G, scale, model, cap=0):
+    load = np.asarray(load, dtype=np.float64)
+    E = len(load)
+    N = 0.0
+    for e in range(E):
+        N += load[e]
+    n_ref = N / E
+    fref = model.whole_kernel(n_ref) if model is not None else 1.0
+    s = np.array([1.0 / (fref / float(scale[g])) if fref > 0 else float(scale[g]) for g in range(G)])
+    ssum = 0.0
+    for g in range(G):
+        ssum += s[g]
+    tau = np.array([N * s[g] / ssum for g in range(G)])
+    order = sorted(range(E), key=lambda e: (-load[e], e))        # stable: ties -> lower e
+    n = np.zeros(G, dtype=np.float64)
+    cnt = np.zeros(G, dtype=np.int64)
+    assign = np.full(E, -1, dtype=np.int32)
+    for e in order:
+        best, best_gap = -1, 0.0
+        for g in range(G):
+            if cap > 0 and cnt[g] >= cap:
+                continue
+            gap = tau[g] - n[g]
+            if best < 0 or gap > best_gap:                      # strict > : ties -> lower g
+                best, best_gap = g, gap
+        assert best >= 0, "cap*G < E"
+        assign[e] = best
+        n[best] += load[e]
+        cnt[best] += 1
+    return assign
+
+
+def placement_token_balanced(load, G, cap=0):
+    """'EPLB implicitly assumes f_g(n)=n': the same greedy with all sigma equal."""
+    return placement_greedy(load, G, np.ones(G), None, cap)
+
+
+def placement_contiguous(E, G):
+    """vLLM's default: expert e -> GPU floor(e*G/E)."""
+    return np.array([(e * G) // E for e in range(E)], dtype=np.int32)
+
+
+# ======================================================================================
+# O8  brute force over all G^E labelled binnings (tests only; NP-hard in general)
+# ======================================================================================
+
+def placement_brute_force(load, G, scale, model, model_kind=MODEL_B, cap=0):
+    E = len(load)
+    best_score, best_assign = np.inf, None
+    for a in itertools.product(range(G), repeat=E):
+        if cap > 0 and max(a.count(g) for g in range(G)) > cap:
+            continue
+        sc, _ = placement_eval(a, load, G, scale, model, model_kind)
+        if sc < best_score:
+            best_score, best_assign = sc, np.array(a, dtype=np.int32)
+    return best_score, best_assign
+
+
+# ======================================================================================
+# parity metrics (F3): max|err| / RMS(ref)  and  mean|err| / mean|ref|
+# ======================================================================================
+
+def ffn_error_metrics(got, ref):
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    err = np.abs(got - ref)
+    rms = float(np.sqrt(np.mean(ref * ref)))
+    mean_abs_ref = float(np.mean(np.abs(ref)))
+    return {
+        "max_abs_err_over_rms": float(err.max() / rms) if rms > 0 else float(err.max()),
+        "mean_rel_err": float(err.mean() / mean_abs_ref) if mean_abs_ref > 0 else float(err.mean()),
+        "rms_ref": rms,
+    }
