@@ -1,0 +1,261 @@
+/* vibe.h -- C ABI of libvibe.so: the B200-native (sm_100a) per-GPU MoE-layer hot path
+ * behind ViBE's variability-aware expert placement (arxiv 2606.00735).
+ *
+ * Citations: P:L<n> = PAPER.md line n (ViBE paper).  Reading ids (R1.., P1.., F1..,
+ * M1.., L1..) are listed in DESIGN.md "Readings of the paper".  The paper treats the
+ * per-GPU MoE layer ("the fused MoE kernel") as a black box that it
+ * profiles as latency-vs-token-load f_g(n) and counts expert activations for
+ * (activation matrix W).  This library IS that black box, rebuilt for one B200:
+ *
+ *   vibe_route_topk   -> vibe_permute -> vibe_grouped_ffn -> vibe_combine       (one stream,
+ *   no host synchronisation between calls), plus vibe_profile_expert_latency which measures
+ *   f(n), and the host-side placement evaluator / greedy solver that consume it
+ *   (Algorithm 1 Phase 2 P:L446-L453).
+ *
+ * Conventions
+ *   - Plain C, no torch / C++ types.  Every pointer is a DEVICE pointer unless the
+ *     parameter comment says "host".  bf16 tensors are passed as `const void*` to raw
+ *     16-bit storage; all tensors are dense row-major.
+ *   - The caller owns every buffer, including workspaces (size them with
+ *     vibe_workspace_bytes / vibe_rows_cap).  The library allocates no device memory per
+ *     call; it keeps process-lifetime caches only (TMA tensor maps keyed by pointer+shape).
+ *   - All device work is enqueued asynchronously on `stream` (a cudaStream_t passed as
+ *     void*; NULL = legacy default stream).  No call synchronises with the host except
+ *     vibe_profile_expert_latency and vibe_moe_layer_forward_host (they return host data).
+ *   - Data-dependent sizes (rows per expert) are never read back: kernels take extents
+ *     from the device-side `offsets` array.
+ *   - Errors: every function returns a vibe_status; argument errors are detected before
+ *     any launch; text of the last error on this thread: vibe_last_error().
+ *   - There is no CPU fallback and no other back-end.  Without a CUDA device every compute
+ *     entry point returns VIBE_ERR_CUDA.
+ *   - Inputs must be finite.  NaN/Inf behaviour is unspecified.
+ */
+#ifndef VIBE_H_
+#define VIBE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define VIBE_API
+#else
+#define VIBE_API __attribute__((visibility("default")))
+#endif
+
+typedef enum {
+  VIBE_OK = 0,
+  VIBE_ERR_INVALID_ARG = 1, /* null pointer, bad size, inconsistent config          */
+  VIBE_ERR_UNSUPPORTED = 2, /* valid request outside what the kernels implement      */
+  VIBE_ERR_WORKSPACE = 3,   /* workspace pointer null / too small / misaligned       */
+  VIBE_ERR_CUDA = 4         /* CUDA runtime / driver error (text in vibe_last_error) */
+} vibe_status;
+
+typedef enum { VIBE_SCORE_SOFTMAX = 0, VIBE_SCORE_SIGMOID = 1 } vibe_score_fn;
+
+/* Routing configuration (readings R1-R7).  Plain data, host memory. */
+typedef struct {
+  int32_t num_experts;      /* E: global experts, 1..512                                  */
+  int32_t top_k;            /* k: 1..min(E,32)                                            */
+  int32_t score_fn;         /* vibe_score_fn                                              */
+  int32_t renormalize;      /* 1: divide the k gate weights by their sum (no epsilon, R4) */
+  float routed_scale;       /* multiplies the final weights (R5); 1.0f in all configs     */
+  int32_t n_group;          /* 0 or 1: no group limiting; else E % n_group == 0 (R6)      */
+  int32_t topk_group;       /* groups kept; topk_group * (E/n_group) >= k                 */
+  const float* select_bias; /* DEVICE [E] or NULL: added to the score for SELECTION only  */
+} vibe_route_cfg;
+
+/* ------------------------------------------------------------------------------------
+ * a1 + a2.  Top-k routing with fused expert-activation histogram.
+ * "route each token to a subset of experts"; counts = one row of the
+ * activation matrix W in R^{LxE}, over GLOBAL experts (R8).
+ *
+ * Per token t (readings R1-R3, R6):
+ *   key[e]  = logits[t,e]                               (softmax: select on raw logits)
+ *           = vsig(logits[t,e]) + select_bias[e]        (sigmoid; vsig = the fixed sequence
+ *             of correctly rounded binary32 operations given in DESIGN.md R2, so ids are
+ *             reproducible bit for bit)
+ *   group limiting: E/n_group contiguous experts per group, group score = largest +
+ *             second largest key (one f32 add), keep the topk_group best groups
+ *             (ties -> lower group), other keys = -inf
+ *   topk_ids[t,0..k) = k rounds of arg-max, ties -> LOWEST expert index, in pick order
+ *   topk_w[t,j]      = softmax over all E of logits (or the true sigmoid, bias excluded) at
+ *             the picked experts, evaluated in fp64, optionally renormalised over the k
+ *             picks, times routed_scale, rounded once to f32
+ *   counts[e]        = number of (t,j) with topk_ids[t,j] == e   (overwritten, not accumulated)
+ *
+ * logits [T,E] f32 (16-byte aligned), topk_ids [T,k] i32, topk_w [T,k] f32, counts [E] i32.
+ * T >= 0 (T == 0 just zeroes counts).  T*k < 2^31.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_route_topk(const vibe_route_cfg* cfg /*host*/, const float* logits, int32_t T,
+                                     int32_t* topk_ids, float* topk_w, int32_t* counts, void* stream);
+
+/* ------------------------------------------------------------------------------------
+ * a3.  Permute: stable counting sort of the A = T*k assignments (flat index i = t*k+j) by
+ * local expert slot, and gather of the token rows into expert-contiguous order.
+ * "token dispatch remains local"; readings P1-P4.
+ *
+ *   slot(i)   = expert_map[topk_ids[i]]  (-1 = expert not resident on this GPU)
+ *   offsets[0] = 0; offsets[s+1] = offsets[s] + roundup(#{i: slot(i)=s}, align)
+ *   rows of slot s are its assignments in ascending i (stable); then padding rows
+ *   row_to_assign[r] = i (or -1 for padding); assign_to_row[i] = r (or -1 if not resident)
+ *   Xp[r,:] = X[i / k, :] (bit copy); padding rows are zero
+ * Rows >= offsets[E_loc] are not written.
+ *
+ * X [T,d] bf16; expert_map [E] i32 or NULL (identity, requires E_loc == E);
+ * d % 8 == 0 (16-byte rows); align >= 1.
+ * Outputs: Xp [R_cap,d] bf16, offsets [E_loc+1] i32, row_to_assign [R_cap] i32,
+ * assign_to_row [A] i32, with R_cap >= vibe_rows_cap(T,k,E_loc,align).
+ * counts: optional (may be NULL) -- the histogram produced by vibe_route_topk; advisory.
+ * ws: vibe_workspace_bytes(VIBE_WS_PERMUTE, ...) bytes, 16-byte aligned.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_permute(const void* X, const int32_t* topk_ids, const int32_t* counts,
+                                  const int32_t* expert_map, int32_t T, int32_t d, int32_t k, int32_t E,
+                                  int32_t E_loc, int32_t align, void* Xp, int32_t* offsets,
+                                  int32_t* row_to_assign, int32_t* assign_to_row, void* ws, size_t ws_bytes,
+                                  void* stream);
+
+/* ------------------------------------------------------------------------------------
+ * a4.  Grouped SwiGLU expert FFN over the resident experts -- the kernel whose
+ * latency-vs-token-load ViBE profiles and the dominant cost of MoE serving
+ * (49 % of prefill time).  Readings F1-F4.
+ *
+ *   for slot s, rows r in [offsets[s], offsets[s+1]):
+ *     H[r,:] = bf16( silu(Xp[r,:] . W1[s]) * (Xp[r,:] . W3[s]) )      (fp32 accumulate)
+ *     Y[r,:] = bf16( H[r,:] . W2[s] )                                  (fp32 accumulate)
+ *
+ * Xp [R_cap,d] bf16; offsets [E_loc+1] i32 (device; offsets[E_loc] <= R_cap);
+ * W1, W3 [E_loc,d,f] bf16 (gate, up); W2 [E_loc,f,d] bf16 (down); all row-major, consumed
+ * in place (no repacking).  H_ws [R_cap,f] bf16 scratch; Y [R_cap,d] bf16.
+ * Shape limits of the tcgen05 kernels: d % 64 == 0, f % 64 == 0, all base pointers
+ * 16-byte aligned (TMA), R_cap >= 1.  Rows >= offsets[E_loc] of H_ws / Y are not written.
+ * ws: vibe_workspace_bytes(VIBE_WS_FFN, ...) bytes (may be 0 -> ws may be NULL).
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_grouped_ffn(const void* Xp, const int32_t* offsets, int32_t E_loc, int32_t R_cap,
+                                      int32_t d, int32_t f, const void* W1, const void* W3, const void* W2,
+                                      void* H_ws, void* Y, void* ws, size_t ws_bytes, void* stream);
+
+/* ------------------------------------------------------------------------------------
+ * a5.  Weighted un-permute / combine (reading C1):
+ *   out[t,:] = bf16( sum_{j<k, assign_to_row[t*k+j] >= 0} topk_w[t,j] * Y[assign_to_row[t*k+j],:] )
+ * fp32 accumulation in slot order j = 0..k-1 (deterministic); tokens without a resident
+ * expert get zeros.  Y [R_cap,d] bf16, out [T,d] bf16, d % 8 == 0.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_combine(const void* Y, const int32_t* assign_to_row, const float* topk_w, int32_t T,
+                                  int32_t k, int32_t d, void* out, void* stream);
+
+/* ------------------------------------------------------------------------------------
+ * a6.  Per-expert latency profile: measured vibe_grouped_ffn time versus tokens per
+ * expert, at warmed steady state -- "Each GPU is warmed to steady-state operating
+ * conditions and profiled independently using the fused MoE kernel across a range of
+ * token counts.  This produces a function f_g(n)" (protocol P:L335, L420).
+ * Readings M1-M4.
+ *
+ *   mode 0 (uniform): every one of the E_loc experts receives n = tokens_per_expert[p]
+ *           rows; latency_us[p] = median kernel time / E_loc   (per-expert cost l(n))
+ *   mode 1 (solo):    expert 0 receives n rows, the others none; latency_us[p] = median time
+ * Times are CUDA-event times of `iters` back-to-back calls (each call timed separately)
+ * after `warmup` untimed calls per point.  Activations are an arbitrary finite pattern
+ * written by the library into ws (latency does not depend on values).
+ * This call SYNCHRONISES the stream.  tokens_per_expert, latency_us, samples_us: HOST.
+ * samples_us: optional host [n_points*iters] per-iteration times (NULL to skip).
+ * ws: vibe_workspace_bytes(VIBE_WS_PROFILE, T = max tokens_per_expert, ...) bytes.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int32_t f, const void* W1,
+                                                 const void* W3, const void* W2,
+                                                 const int32_t* tokens_per_expert /*host*/, int32_t n_points,
+                                                 int32_t mode, int32_t warmup, int32_t iters,
+                                                 float* latency_us /*host*/, float* samples_us /*host|NULL*/,
+                                                 void* ws, size_t ws_bytes, void* stream);
+
+/* ------------------------------------------------------------------------------------
+ * The whole layer (a1..a5) as one call: enqueues route -> permute -> grouped FFN ->
+ * combine on `stream` using one caller-provided device arena.
+ * arena: vibe_workspace_bytes(VIBE_WS_LAYER, ...) bytes, 256-byte aligned.
+ * Outputs: out [T,d] bf16, counts [E] i32 (device).  Optional device outputs topk_ids /
+ * topk_w may be NULL (then they live in the arena).
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg /*host*/, const float* logits,
+                                            const void* X, const int32_t* expert_map, int32_t T, int32_t d,
+                                            int32_t f, int32_t E_loc, const void* W1, const void* W3,
+                                            const void* W2, void* out, int32_t* counts, int32_t* topk_ids,
+                                            float* topk_w, void* arena, size_t arena_bytes, void* stream);
+
+/* Same, end to end from HOST buffers: copies logits_h and X_h (pinned or pageable host
+ * memory) to the device, runs the layer, copies out_h and counts_h back, and waits for
+ * the stream.  Weights, select_bias and expert_map stay device-resident (model state).
+ * arena additionally holds the device copies: vibe_workspace_bytes(VIBE_WS_LAYER_HOST, ...). */
+VIBE_API vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg /*host*/,
+                                                 const float* logits_h /*host*/, const void* X_h /*host*/,
+                                                 const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
+                                                 int32_t E_loc, const void* W1, const void* W3, const void* W2,
+                                                 void* out_h /*host*/, int32_t* counts_h /*host*/, void* arena,
+                                                 size_t arena_bytes, void* stream);
+
+/* Workspace sizing.  `which` selects the consumer. */
+enum {
+  VIBE_WS_PERMUTE = 0,
+  VIBE_WS_FFN = 1,
+  VIBE_WS_PROFILE = 2, /* T = max tokens per expert of the sweep */
+  VIBE_WS_LAYER = 3,
+  VIBE_WS_LAYER_HOST = 4
+};
+VIBE_API size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int32_t E, int32_t E_loc, int32_t d,
+                                     int32_t f, int32_t align);
+/* Upper bound on offsets[E_loc]: min(T*k, T*E_loc) + E_loc*(align-1). */
+VIBE_API int64_t vibe_rows_cap(int32_t T, int32_t k, int32_t E_loc, int32_t align);
+
+VIBE_API const char* vibe_status_string(vibe_status s);
+VIBE_API const char* vibe_last_error(void); /* thread-local, never NULL */
+VIBE_API int32_t vibe_version(void);
+/* Number of kernel launches this library has issued on this thread since load
+ * (memsets and copies not counted): lets a caller report how many of ITS kernels ran. */
+VIBE_API int64_t vibe_launch_count(void);
+
+/* ====================================================================================
+ * Host-side placement (fp64, no device work).  P:L182-L196, Algorithm 1 Phase 2.
+ * ==================================================================================== */
+
+/* Latency model (reading M1): monotone piecewise-linear per-expert latency l(n) through
+ * (0,0) and the profiled points (running max applied), linear extrapolation with the last
+ * segment's slope.  E_prof: experts resident when profiled in uniform mode, so the
+ * whole-kernel latency with n tokens in total is F(n) = E_prof * l(n / E_prof).
+ * tokens must be strictly increasing and > 0.  NULL model pointer means f(n) = n. */
+typedef struct {
+  int32_t n_points;
+  const double* tokens;     /* host [n_points] */
+  const double* latency_us; /* host [n_points] */
+  int32_t E_prof;
+} vibe_latency_model;
+
+enum { VIBE_MODEL_A = 0, /* paper-faithful scalar model  L_g = F(sum_e load_e) */
+       VIBE_MODEL_B = 1  /* per-expert profile           L_g = sum_e l(load_e)   (L4)     */ };
+
+/* a7.  score(S) = max_g L_g / scale[g]   -- "T = max_g f_g(n_g)", n_g = sum_{e in S_g} w_e
+ * with f_g = f / sigma_g (M5).  assign [E] in [0,G); load [E] tokens;
+ * scale [G] in (0,1]; per_bin [G] or NULL receives L_g / scale[g].
+ * Returns the score, or a negative value on invalid arguments (see vibe_last_error). */
+VIBE_API double vibe_placement_eval(const int32_t* assign, const double* load, int32_t E, int32_t G,
+                                    const double* scale, const vibe_latency_model* m, int32_t model_kind,
+                                    double* per_bin);
+
+/* a8.  ViBE's latency-aware greedy (Algorithm 1 Phase 2):
+ *   N = sum_e load_e; s_g = 1/f_g(N/E); tau_g = N s_g / sum_h s_h; experts in descending
+ *   load (ties -> lower e); each to argmax_g (tau_g - n_g) (ties -> lower g) among bins
+ *   with fewer than `cap` experts (cap = 0: unlimited; P:L260 uses cap = E/G). */
+VIBE_API vibe_status vibe_placement_greedy(const double* load, int32_t E, int32_t G, const double* scale,
+                                           const vibe_latency_model* m, int32_t cap, int32_t* assign);
+/* Token-balanced baseline: "EPLB implicitly assumes f_g(n) = n" = the same greedy
+ * with all scales equal (L3). */
+VIBE_API vibe_status vibe_placement_token_balanced(const double* load, int32_t E, int32_t G, int32_t cap,
+                                                   int32_t* assign);
+/* vLLM's contiguous default: e -> floor(e*G/E). */
+VIBE_API vibe_status vibe_placement_contiguous(int32_t E, int32_t G, int32_t* assign);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VIBE_H_ */

@@ -317,26 +317,34 @@ def combine(Y, assign_to_row, topk_w, T, k, round_out=False):
     return out
 
 
-def moe_layer_direct(X_bits, topk_ids, topk_w, expert_map, W1_bits, W3_bits, W2_bits, tokens=None):
+def moe_layer_direct(X_bits, topk_ids, topk_w, expert_map, W1_bits, W3_bits, W2_bits, tokens=None,
+                     return_abs=False):
     """Independent statement of the whole layer with NO permutation:
        out[t] = sum_j w[t,j] * FFN_{slot(id[t,j])}(x_t)   (non-resident experts contribute 0).
-    Used to pin permute+ffn+combine together, and as the sampled full-size reference."""
+    Used to pin permute+ffn+combine together, and as the sampled full-size reference.
+    return_abs: also return sum_j w[t,j]*|FFN(x_t)| per element, the quantity that bounds the
+    error contributed by storing Y in bf16."""
     T, k = topk_ids.shape
     d = X_bits.shape[1]
     toks = range(T) if tokens is None else tokens
-    out = {}
+    out, out_abs = {}, {}
     for t in toks:
         acc = np.zeros(d, dtype=np.float64)
+        acc_abs = np.zeros(d, dtype=np.float64)
         for j in range(k):
             s = topk_ids[t, j] if expert_map is None else expert_map[topk_ids[t, j]]
             if s < 0:
                 continue
             y, _ = swiglu_ffn_rows(X_bits[t:t + 1], W1_bits[s], W3_bits[s], W2_bits[s])
-            acc += float(np.float32(topk_w[t, j])) * y[0]
+            wj = float(np.float32(topk_w[t, j]))
+            acc += wj * y[0]
+            acc_abs += wj * np.abs(y[0])
         out[t] = acc
+        out_abs[t] = acc_abs
     if tokens is None:
-        return np.stack([out[t] for t in range(T)])
-    return out
+        out = np.stack([out[t] for t in range(T)])
+        out_abs = np.stack([out_abs[t] for t in range(T)])
+    return (out, out_abs) if return_abs else out
 
 
 # ======================================================================================

@@ -1,0 +1,370 @@
+"""Thin ctypes binding over libvibe.so (include/vibe.h) -- argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; PyTorch is used here
+for device memory and streams only.  Names mirror the C ABI:
+
+    route_topk, permute, grouped_ffn, combine, profile_expert_latency,
+    moe_layer_forward, moe_layer_forward_host,
+    placement_eval, placement_greedy, placement_token_balanced, placement_contiguous
+
+There is NO fallback: if libvibe.so is missing or a call fails, a VibeError is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libvibe.so")
+
+VIBE_OK = 0
+SCORE_SOFTMAX = 0
+SCORE_SIGMOID = 1
+WS_PERMUTE, WS_FFN, WS_PROFILE, WS_LAYER, WS_LAYER_HOST = 0, 1, 2, 3, 4
+MODEL_A, MODEL_B = 0, 1
+
+# every symbol include/vibe.h declares (tests check that the .so exports exactly these)
+EXPORTED_SYMBOLS = (
+    "vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_profile_expert_latency",
+    "vibe_moe_layer_forward", "vibe_moe_layer_forward_host", "vibe_workspace_bytes", "vibe_rows_cap",
+    "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
+    "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
+)
+
+
+class VibeError(RuntimeError):
+    pass
+
+
+class _RouteCfg(C.Structure):
+    _fields_ = [("num_experts", C.c_int32), ("top_k", C.c_int32), ("score_fn", C.c_int32),
+                ("renormalize", C.c_int32), ("routed_scale", C.c_float), ("n_group", C.c_int32),
+                ("topk_group", C.c_int32), ("select_bias", C.c_void_p)]
+
+
+class _LatencyModel(C.Structure):
+    _fields_ = [("n_points", C.c_int32), ("tokens", C.POINTER(C.c_double)),
+                ("latency_us", C.POINTER(C.c_double)), ("E_prof", C.c_int32)]
+
+
+@dataclasses.dataclass
+class RouteConfig:
+    num_experts: int
+    top_k: int
+    score_fn: int = SCORE_SOFTMAX
+    renormalize: int = 1
+    routed_scale: float = 1.0
+    n_group: int = 0
+    topk_group: int = 0
+    select_bias: Optional[torch.Tensor] = None      # device f32 [E]
+
+    def _c(self) -> _RouteCfg:
+        b = self.select_bias
+        if b is not None:
+            _check(b, torch.float32, "select_bias")
+        return _RouteCfg(self.num_experts, self.top_k, self.score_fn, self.renormalize, self.routed_scale,
+                         self.n_group, self.topk_group, b.data_ptr() if b is not None else None)
+
+
+@dataclasses.dataclass
+class LatencyModel:
+    tokens: Sequence[float]
+    latency_us: Sequence[float]
+    E_prof: int = 1
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """Load libvibe.so (built in-tree by `python -m paper_2606_00735_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise VibeError(f"{LIB_PATH} not found: build it with `python -m paper_2606_00735_b200.build` "
+                        "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, sz = C.c_void_p, C.c_int32, C.c_size_t
+    lib.vibe_route_topk.argtypes = [C.POINTER(_RouteCfg), vp, i32, vp, vp, vp, vp]
+    lib.vibe_permute.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_grouped_ffn.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_combine.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    lib.vibe_profile_expert_latency.argtypes = [i32, i32, i32, vp, vp, vp, C.POINTER(i32), i32, i32, i32, i32,
+                                                C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
+    lib.vibe_moe_layer_forward.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
+                                           vp, vp, vp, sz, vp]
+    lib.vibe_moe_layer_forward_host.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
+                                                vp, vp, vp, sz, vp]
+    lib.vibe_workspace_bytes.argtypes = [i32] * 8
+    lib.vibe_workspace_bytes.restype = sz
+    lib.vibe_rows_cap.argtypes = [i32] * 4
+    lib.vibe_rows_cap.restype = C.c_int64
+    lib.vibe_status_string.argtypes = [C.c_int]
+    lib.vibe_status_string.restype = C.c_char_p
+    lib.vibe_last_error.restype = C.c_char_p
+    lib.vibe_version.restype = i32
+    lib.vibe_launch_count.restype = C.c_int64
+    dp = C.POINTER(C.c_double)
+    lib.vibe_placement_eval.argtypes = [C.POINTER(i32), dp, i32, i32, dp, C.POINTER(_LatencyModel), i32, dp]
+    lib.vibe_placement_eval.restype = C.c_double
+    lib.vibe_placement_greedy.argtypes = [dp, i32, i32, dp, C.POINTER(_LatencyModel), i32, C.POINTER(i32)]
+    lib.vibe_placement_token_balanced.argtypes = [dp, i32, i32, i32, C.POINTER(i32)]
+    lib.vibe_placement_contiguous.argtypes = [i32, i32, C.POINTER(i32)]
+    for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine",
+                 "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
+                 "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous"):
+        getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _ok(status: int, what: str) -> None:
+    if status != VIBE_OK:
+        lib = load()
+        raise VibeError(f"{what}: {lib.vibe_status_string(status).decode()}: {lib.vibe_last_error().decode()}")
+
+
+def _check(t: torch.Tensor, dtype, name: str) -> None:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise VibeError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if t.dtype != dtype:
+        raise VibeError(f"{name} must be {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise VibeError(f"{name} must be contiguous")
+
+
+def _stream(stream) -> int:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return s.cuda_stream
+
+
+def launch_count() -> int:
+    return int(load().vibe_launch_count())
+
+
+def workspace_bytes(which: int, T: int, k: int, E: int, E_loc: int, d: int, f: int, align: int = 1) -> int:
+    return int(load().vibe_workspace_bytes(which, T, k, E, E_loc, d, f, align))
+
+
+def rows_cap(T: int, k: int, E_loc: int, align: int = 1) -> int:
+    return int(load().vibe_rows_cap(T, k, E_loc, align))
+
+
+# ------------------------------------------------------------------------------------ a1+a2
+def route_topk(logits: torch.Tensor, cfg: RouteConfig, out=None, stream=None):
+    """-> (topk_ids i32 [T,k], topk_w f32 [T,k], counts i32 [E])"""
+    lib = load()
+    _check(logits, torch.float32, "logits")
+    T, E = logits.shape
+    if E != cfg.num_experts:
+        raise VibeError("logits.shape[1] != cfg.num_experts")
+    dev = logits.device
+    if out is None:
+        ids = torch.empty((T, cfg.top_k), dtype=torch.int32, device=dev)
+        w = torch.empty((T, cfg.top_k), dtype=torch.float32, device=dev)
+        counts = torch.empty((E,), dtype=torch.int32, device=dev)
+    else:
+        ids, w, counts = out
+    c = cfg._c()
+    _ok(lib.vibe_route_topk(C.byref(c), logits.data_ptr(), T, ids.data_ptr(), w.data_ptr(), counts.data_ptr(),
+                            _stream(stream)), "vibe_route_topk")
+    return ids, w, counts
+
+
+# ------------------------------------------------------------------------------------ a3
+def permute(X: torch.Tensor, topk_ids: torch.Tensor, counts: Optional[torch.Tensor],
+            expert_map: Optional[torch.Tensor], E: int, E_loc: int, align: int = 1, out=None, ws=None, stream=None):
+    """-> (Xp bf16 [R_cap,d], offsets i32 [E_loc+1], row_to_assign i32 [R_cap], assign_to_row i32 [T*k])"""
+    lib = load()
+    _check(X, torch.bfloat16, "X")
+    _check(topk_ids, torch.int32, "topk_ids")
+    T, d = X.shape
+    k = topk_ids.shape[1]
+    dev = X.device
+    Rcap = max(1, rows_cap(T, k, E_loc, align))
+    if out is None:
+        Xp = torch.empty((Rcap, d), dtype=torch.bfloat16, device=dev)
+        offsets = torch.empty((E_loc + 1,), dtype=torch.int32, device=dev)
+        r2a = torch.empty((Rcap,), dtype=torch.int32, device=dev)
+        a2r = torch.empty((T * k,), dtype=torch.int32, device=dev)
+    else:
+        Xp, offsets, r2a, a2r = out
+    need = workspace_bytes(WS_PERMUTE, T, k, E, E_loc, d, 0, align)
+    if ws is None:
+        ws = torch.empty((max(need, 16),), dtype=torch.uint8, device=dev)
+    _ok(lib.vibe_permute(X.data_ptr(), topk_ids.data_ptr(), counts.data_ptr() if counts is not None else None,
+                         expert_map.data_ptr() if expert_map is not None else None, T, d, k, E, E_loc, align,
+                         Xp.data_ptr(), offsets.data_ptr(), r2a.data_ptr(), a2r.data_ptr(), ws.data_ptr(),
+                         ws.numel(), _stream(stream)), "vibe_permute")
+    return Xp, offsets, r2a, a2r
+
+
+# ------------------------------------------------------------------------------------ a4
+def grouped_ffn(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: torch.Tensor, W2: torch.Tensor,
+                H: Optional[torch.Tensor] = None, Y: Optional[torch.Tensor] = None, stream=None):
+    """-> Y bf16 [R_cap,d]  (H bf16 [R_cap,f] scratch is returned too)"""
+    lib = load()
+    for t, n in ((Xp, "Xp"), (W1, "W1"), (W3, "W3"), (W2, "W2")):
+        _check(t, torch.bfloat16, n)
+    _check(offsets, torch.int32, "offsets")
+    Rcap, d = Xp.shape
+    E_loc, d1, f = W1.shape
+    if d1 != d or tuple(W3.shape) != (E_loc, d, f) or tuple(W2.shape) != (E_loc, f, d):
+        raise VibeError("weight shapes must be W1,W3 [E_loc,d,f], W2 [E_loc,f,d]")
+    if offsets.numel() != E_loc + 1:
+        raise VibeError("offsets must have E_loc+1 entries")
+    if H is None:
+        H = torch.empty((Rcap, f), dtype=torch.bfloat16, device=Xp.device)
+    if Y is None:
+        Y = torch.empty((Rcap, d), dtype=torch.bfloat16, device=Xp.device)
+    _ok(lib.vibe_grouped_ffn(Xp.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1.data_ptr(), W3.data_ptr(),
+                             W2.data_ptr(), H.data_ptr(), Y.data_ptr(), None, 0, _stream(stream)), "vibe_grouped_ffn")
+    return Y, H
+
+
+# ------------------------------------------------------------------------------------ a5
+def combine(Y: torch.Tensor, assign_to_row: torch.Tensor, topk_w: torch.Tensor, T: int, k: int,
+            out: Optional[torch.Tensor] = None, stream=None):
+    lib = load()
+    _check(Y, torch.bfloat16, "Y")
+    _check(assign_to_row, torch.int32, "assign_to_row")
+    _check(topk_w, torch.float32, "topk_w")
+    d = Y.shape[1]
+    if out is None:
+        out = torch.empty((T, d), dtype=torch.bfloat16, device=Y.device)
+    _ok(lib.vibe_combine(Y.data_ptr(), assign_to_row.data_ptr(), topk_w.data_ptr(), T, k, d, out.data_ptr(),
+                         _stream(stream)), "vibe_combine")
+    return out
+
+
+# ------------------------------------------------------------------------------------ a6
+DEFAULT_SWEEP = (1, 2, 3, 4, 6, 8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 1536, 2048,
+                 3072, 4096)
+
+
+def profile_expert_latency(W1: torch.Tensor, W3: torch.Tensor, W2: torch.Tensor,
+                           tokens_per_expert: Sequence[int] = DEFAULT_SWEEP, mode: int = 0, warmup: int = 10,
+                           iters: int = 100, return_samples: bool = False, ws=None, stream=None):
+    """Measured grouped-FFN latency [us] per sweep point (median); mode 0 = per-expert cost with all
+    experts loaded uniformly, mode 1 = one loaded expert."""
+    lib = load()
+    for t, n in ((W1, "W1"), (W3, "W3"), (W2, "W2")):
+        _check(t, torch.bfloat16, n)
+    E_loc, d, f = W1.shape
+    toks = (C.c_int32 * len(tokens_per_expert))(*[int(x) for x in tokens_per_expert])
+    npts = len(tokens_per_expert)
+    lat = (C.c_float * npts)()
+    samples = (C.c_float * (npts * iters))() if return_samples else None
+    need = workspace_bytes(WS_PROFILE, max(tokens_per_expert), 1, E_loc, E_loc, d, f, 1)
+    if ws is None:
+        ws = torch.empty((need,), dtype=torch.uint8, device=W1.device)
+    _ok(lib.vibe_profile_expert_latency(E_loc, d, f, W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), toks, npts, mode,
+                                        warmup, iters, lat, samples, ws.data_ptr(), ws.numel(), _stream(stream)),
+        "vibe_profile_expert_latency")
+    lat_np = np.array(lat[:], dtype=np.float64)
+    if return_samples:
+        return lat_np, np.array(samples[:], dtype=np.float64).reshape(npts, iters)
+    return lat_np
+
+
+# ------------------------------------------------------------------------------------ layer
+def moe_layer_forward(cfg: RouteConfig, logits, X, expert_map, W1, W3, W2, out=None, counts=None, topk_ids=None,
+                      topk_w=None, arena=None, stream=None):
+    lib = load()
+    _check(logits, torch.float32, "logits")
+    _check(X, torch.bfloat16, "X")
+    T, d = X.shape
+    E_loc, _, f = W1.shape
+    dev = X.device
+    if out is None:
+        out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+    if counts is None:
+        counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
+    need = workspace_bytes(WS_LAYER, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
+    if arena is None:
+        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+    c = cfg._c()
+    _ok(lib.vibe_moe_layer_forward(C.byref(c), logits.data_ptr(), X.data_ptr(),
+                                   expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
+                                   W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), out.data_ptr(), counts.data_ptr(),
+                                   topk_ids.data_ptr() if topk_ids is not None else None,
+                                   topk_w.data_ptr() if topk_w is not None else None, arena.data_ptr(),
+                                   arena.numel(), _stream(stream)), "vibe_moe_layer_forward")
+    return out, counts
+
+
+def moe_layer_forward_host(cfg: RouteConfig, logits_h: torch.Tensor, X_h: torch.Tensor, expert_map, W1, W3, W2,
+                           out_h: torch.Tensor, counts_h: torch.Tensor, arena: torch.Tensor, stream=None):
+    """End to end from (pinned) HOST tensors; returns when out_h / counts_h are filled."""
+    lib = load()
+    T, d = X_h.shape
+    E_loc, _, f = W1.shape
+    assert not logits_h.is_cuda and not X_h.is_cuda and not out_h.is_cuda and not counts_h.is_cuda
+    c = cfg._c()
+    _ok(lib.vibe_moe_layer_forward_host(C.byref(c), logits_h.data_ptr(), X_h.data_ptr(),
+                                        expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
+                                        W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), out_h.data_ptr(),
+                                        counts_h.data_ptr(), arena.data_ptr(), arena.numel(), _stream(stream)),
+        "vibe_moe_layer_forward_host")
+    return out_h, counts_h
+
+
+# ------------------------------------------------------------------------------------ placement (host)
+def _dp(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _model(m: Optional[LatencyModel]):
+    if m is None:
+        return None, None
+    t, tp = _dp(m.tokens)
+    l, lp = _dp(m.latency_us)
+    return C.byref(_LatencyModel(len(t), tp, lp, int(m.E_prof))), (t, l)
+
+
+def placement_eval(assign, load_, G: int, scale, model: Optional[LatencyModel], model_kind: int = MODEL_B):
+    lib = load()
+    a = np.ascontiguousarray(assign, dtype=np.int32)
+    ld, ldp = _dp(load_)
+    sc, scp = _dp(scale)
+    per = np.zeros(G, dtype=np.float64)
+    mref, keep = _model(model)
+    v = lib.vibe_placement_eval(a.ctypes.data_as(C.POINTER(C.c_int32)), ldp, len(ld), G, scp, mref, model_kind,
+                                per.ctypes.data_as(C.POINTER(C.c_double)))
+    if v < 0:
+        raise VibeError("vibe_placement_eval: " + lib.vibe_last_error().decode())
+    return float(v), per
+
+
+def placement_greedy(load_, G: int, scale, model: Optional[LatencyModel], cap: int = 0):
+    lib = load()
+    ld, ldp = _dp(load_)
+    sc, scp = _dp(scale)
+    out = np.empty(len(ld), dtype=np.int32)
+    mref, keep = _model(model)
+    _ok(lib.vibe_placement_greedy(ldp, len(ld), G, scp, mref, cap, out.ctypes.data_as(C.POINTER(C.c_int32))),
+        "vibe_placement_greedy")
+    return out
+
+
+def placement_token_balanced(load_, G: int, cap: int = 0):
+    lib = load()
+    ld, ldp = _dp(load_)
+    out = np.empty(len(ld), dtype=np.int32)
+    _ok(lib.vibe_placement_token_balanced(ldp, len(ld), G, cap, out.ctypes.data_as(C.POINTER(C.c_int32))),
+        "vibe_placement_token_balanced")
+    return out
+
+
+def placement_contiguous(E: int, G: int):
+    lib = load()
+    out = np.empty(E, dtype=np.int32)
+    _ok(lib.vibe_placement_contiguous(E, G, out.ctypes.data_as(C.POINTER(C.c_int32))), "vibe_placement_contiguous")
+    return out

@@ -1,0 +1,78 @@
+// common.cuh -- shared plumbing of libvibe.so (host error state, launch accounting, small
+// device helpers).  CUDA path only: nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdarg.h>
+
+#include "../../include/vibe.h"
+
+namespace vibe {
+
+// ---- host-side error state (thread-local) -------------------------------------------
+void set_error(const char* fmt, ...);
+void clear_error();
+void count_launch(int n = 1);
+int num_sms();
+
+#define VIBE_REQUIRE(cond, status, ...)         \
+  do {                                          \
+    if (!(cond)) {                              \
+      ::vibe::set_error(__VA_ARGS__);           \
+      return (status);                          \
+    }                                           \
+  } while (0)
+
+#define VIBE_CUDA(call)                                                                   \
+  do {                                                                                    \
+    cudaError_t e__ = (call);                                                             \
+    if (e__ != cudaSuccess) {                                                             \
+      ::vibe::set_error("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, \
+                        __LINE__);                                                        \
+      return VIBE_ERR_CUDA;                                                               \
+    }                                                                                     \
+  } while (0)
+
+// after a <<<>>> launch
+#define VIBE_LAUNCH_CHECK(name)                                                             \
+  do {                                                                                      \
+    cudaError_t e__ = cudaGetLastError();                                                   \
+    if (e__ != cudaSuccess) {                                                               \
+      ::vibe::set_error("launch of %s failed: %s", name, cudaGetErrorString(e__));          \
+      return VIBE_ERR_CUDA;                                                                 \
+    }                                                                                       \
+    ::vibe::count_launch();                                                                 \
+  } while (0)
+
+// ---- internal cross-file declarations -------------------------------------------------
+struct LayerArena {
+  size_t ids, w, offsets, r2a, a2r, Xp, H, Y, perm_ws, total;
+  int64_t R_cap;
+};
+LayerArena layer_arena(int T, int k, int E_loc, int d, int f);
+size_t permute_ws_bytes(int T, int k, int E_loc);
+vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
+                             const void* W1, const void* W3, const void* W2, void* H_ws, void* Y, cudaStream_t st);
+vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
+                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y);
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- device helpers ---------------------------------------------------------------------
+__device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_na_v4(void* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+               "r"(v.w)
+               : "memory");
+}
+
+}  // namespace vibe

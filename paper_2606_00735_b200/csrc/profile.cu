@@ -1,0 +1,102 @@
+// profile.cu -- a6: per-expert latency profile f(n) of the grouped FFN (vibe_profile_expert_latency).
+// "Each GPU is warmed to steady-state operating conditions and profiled independently using
+// the fused MoE kernel across a range of token counts.  This produces a function f_g(n)"
+// (Algorithm 1 Phase 1, L439-L443; protocol L335).  DESIGN.md M1-M4.
+#include <algorithm>
+#include <vector>
+
+#include "common.cuh"
+
+namespace vibe {
+namespace {
+// arbitrary finite activations in (-1,1): latency does not depend on the values
+__global__ void fill_pattern_kernel(__nv_bfloat16* p, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    uint32_t h = (uint32_t)i * 2654435761u;
+    h ^= h >> 15;
+    h *= 2246822519u;
+    h ^= h >> 13;
+    p[i] = __float2bfloat16_rn(((int)(h & 0xffff) - 32768) * (1.0f / 32768.0f));
+  }
+}
+}  // namespace
+}  // namespace vibe
+
+extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int32_t f, const void* W1,
+                                                   const void* W3, const void* W2,
+                                                   const int32_t* tokens_per_expert, int32_t n_points, int32_t mode,
+                                                   int32_t warmup, int32_t iters, float* latency_us,
+                                                   float* samples_us, void* ws, size_t ws_bytes, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(tokens_per_expert && latency_us && n_points >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency: need tokens_per_expert, latency_us, n_points >= 1");
+  VIBE_REQUIRE(mode == 0 || mode == 1, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency: mode must be 0 or 1");
+  VIBE_REQUIRE(warmup >= 0 && iters >= 1 && iters <= 100000, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency: need warmup >= 0, 1 <= iters <= 100000");
+  int n_max = 0;
+  for (int p = 0; p < n_points; ++p) {
+    VIBE_REQUIRE(tokens_per_expert[p] >= 0, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency: negative token count");
+    n_max = std::max(n_max, tokens_per_expert[p]);
+  }
+  VIBE_REQUIRE((int64_t)E_loc * std::max(n_max, 1) < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency: E_loc * max tokens >= 2^31");
+  const int R_cap = E_loc * std::max(n_max, 1);
+  const size_t need = vibe_workspace_bytes(VIBE_WS_PROFILE, n_max, 1, E_loc, E_loc, d, f, 1);
+  VIBE_REQUIRE(ws != nullptr && ws_bytes >= need && (reinterpret_cast<uintptr_t>(ws) & 255u) == 0, VIBE_ERR_WORKSPACE,
+               "vibe_profile_expert_latency: workspace needs %zu bytes, 256-byte aligned (got %zu)", need, ws_bytes);
+  char* base = reinterpret_cast<char*>(ws);
+  void* Xp = base;
+  void* Y = base + round_up((size_t)R_cap * d * 2, 256);
+  void* H = base + 2 * round_up((size_t)R_cap * d * 2, 256);
+  int32_t* offsets = reinterpret_cast<int32_t*>(base + 2 * round_up((size_t)R_cap * d * 2, 256) +
+                                                round_up((size_t)R_cap * f * 2, 256));
+  vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y);
+  if (s != VIBE_OK) return s;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  fill_pattern_kernel<<<num_sms() * 4, 256, 0, st>>>(reinterpret_cast<__nv_bfloat16*>(Xp), (size_t)R_cap * d);
+  VIBE_LAUNCH_CHECK("fill_pattern_kernel");
+
+  std::vector<cudaEvent_t> ev(2 * (size_t)iters);
+  for (auto& e : ev) VIBE_CUDA(cudaEventCreate(&e));
+  std::vector<int32_t> off(E_loc + 1);
+  std::vector<float> t(iters);
+  vibe_status rc = VIBE_OK;
+  for (int p = 0; p < n_points && rc == VIBE_OK; ++p) {
+    const int n = tokens_per_expert[p];
+    off[0] = 0;
+    for (int e = 0; e < E_loc; ++e) off[e + 1] = off[e] + ((mode == 0 || e == 0) ? n : 0);
+    cudaError_t ce = cudaMemcpyAsync(offsets, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) {
+      set_error("vibe_profile_expert_latency: offsets upload failed: %s", cudaGetErrorString(ce));
+      rc = VIBE_ERR_CUDA;
+      break;
+    }
+    for (int i = 0; i < warmup && rc == VIBE_OK; ++i)
+      rc = grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st);
+    for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
+      cudaEventRecord(ev[2 * i], st);
+      rc = grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st);
+      cudaEventRecord(ev[2 * i + 1], st);
+    }
+    if (rc != VIBE_OK) break;
+    ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) {
+      set_error("vibe_profile_expert_latency: kernel failed: %s", cudaGetErrorString(ce));
+      rc = VIBE_ERR_CUDA;
+      break;
+    }
+    for (int i = 0; i < iters; ++i) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]);
+      t[i] = ms * 1000.0f;
+      if (samples_us) samples_us[(size_t)p * iters + i] = t[i];
+    }
+    std::sort(t.begin(), t.end());
+    const float med = (iters & 1) ? t[iters / 2] : 0.5f * (t[iters / 2 - 1] + t[iters / 2]);
+    latency_us[p] = (mode == 0) ? med / (float)E_loc : med;
+  }
+  for (auto& e : ev) cudaEventDestroy(e);
+  return rc;
+}

@@ -1,0 +1,358 @@
+// route.cu -- a1 + a2: top-k routing with fused expert-activation histogram (vibe_route_topk).
+//
+// One token per group of LANES lanes (LANES = 8 for small E, else a full warp); every lane
+// keeps VPL consecutive experts' keys in registers (vectorised, coalesced 16-byte loads).
+// Selection is k rounds of {local max, redux.sync max over the group, ballot, lowest lane
+// wins} on order-preserving u32 images of the f32 keys, which gives the "ties -> lowest
+// expert index" rule for free (lane-major element order).  The histogram is privatised in
+// shared memory per block and merged with one global atomic per non-empty bin.
+// Gate weights are evaluated in fp64 for the k picked experts only.
+//
+// Semantics: include/vibe.h (vibe_route_topk), readings R1-R8.
+#include "common.cuh"
+
+namespace vibe {
+namespace {
+
+struct RouteParams {
+  const float* logits;
+  const float* bias;
+  int32_t* ids;
+  float* w;
+  int32_t* counts;
+  int T, E, k;
+  int renorm;
+  float scale;
+  int n_group, topk_group;
+  int fast_groups;  // 1: a lane's VPL experts lie in one group and lanes/group is a power of two
+};
+
+// ---- reproducible f32 sigmoid for the selection key (R2) ----------------------
+// Exactly this sequence of separately rounded binary32 operations; no FMA contraction
+// (explicit _rn intrinsics).  Constants are given by bit pattern.
+__device__ __forceinline__ float vsig(float x) {
+  const float LOG2E = __uint_as_float(0x3fb8aa3bu);   // 1.44269502
+  const float LN2_HI = __uint_as_float(0x3f318000u);  // 0.693359375
+  const float LN2_LO = __uint_as_float(0xb95e8083u);  // -2.12194442e-4
+  x = fminf(fmaxf(x, -80.0f), 80.0f);
+  const float a = -x;
+  const float n = rintf(__fmul_rn(a, LOG2E));
+  float r = __fsub_rn(a, __fmul_rn(n, LN2_HI));
+  r = __fsub_rn(r, __fmul_rn(n, LN2_LO));
+  float p = __uint_as_float(0x39500d01u);                               // 1/5040
+  p = __fadd_rn(__fmul_rn(p, r), __uint_as_float(0x3ab60b61u));        // 1/720
+  p = __fadd_rn(__fmul_rn(p, r), __uint_as_float(0x3c088889u));        // 1/120
+  p = __fadd_rn(__fmul_rn(p, r), __uint_as_float(0x3d2aaaabu));        // 1/24
+  p = __fadd_rn(__fmul_rn(p, r), __uint_as_float(0x3e2aaaabu));        // 1/6
+  p = __fadd_rn(__fmul_rn(p, r), 0.5f);
+  p = __fadd_rn(__fmul_rn(p, r), 1.0f);
+  p = __fadd_rn(__fmul_rn(p, r), 1.0f);
+  // exact scaling by 2^n: p in (0.70, 1.42) and |n| <= 116 keep the result normal
+  const float e = __int_as_float(__float_as_int(p) + (__float2int_rn(n) << 23));
+  return __fdiv_rn(1.0f, __fadd_rn(1.0f, e));
+}
+
+// order-preserving map f32 -> u32 (after -0 -> +0 so that -0 == +0 as in a float compare)
+__device__ __forceinline__ uint32_t ordered_u32(float x) {
+  const uint32_t b = __float_as_uint(__fadd_rn(x, 0.0f));
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+template <int LANES>
+__device__ __forceinline__ uint32_t group_max_u32(unsigned gmask, uint32_t v) {
+  return __reduce_max_sync(gmask, v);
+}
+template <int LANES>
+__device__ __forceinline__ double group_sum_f64(unsigned gmask, double v) {
+#pragma unroll
+  for (int o = LANES / 2; o >= 1; o >>= 1) v += __shfl_xor_sync(gmask, v, o);
+  return v;
+}
+
+constexpr uint32_t kTaken = 0u;  // below ordered_u32(-inf) = 0x007fffff
+
+template <int LANES, int VPL, bool SIGMOID>
+__global__ void __launch_bounds__(256) route_topk_kernel(const RouteParams p) {
+  extern __shared__ int s_mem[];
+  int* s_hist = s_mem;                                        // [E]
+  float* s_gscore = reinterpret_cast<float*>(s_mem + p.E);    // [groups_per_block][n_group] (generic path)
+  for (int i = threadIdx.x; i < p.E; i += blockDim.x) s_hist[i] = 0;
+  __syncthreads();
+
+  const int lane = threadIdx.x & 31;
+  const int sub = lane % LANES;
+  const unsigned gmask = (LANES == 32) ? 0xffffffffu : (((1u << LANES) - 1u) << (lane - sub));
+  constexpr int kGroupsPerBlock = 256 / LANES;
+  const int gidx = threadIdx.x / LANES;
+  const int e0 = sub * VPL;
+  const int E = p.E, k = p.k;
+  const float NEG_INF = __int_as_float(0xff800000);
+  const bool vec_ok = (VPL % 4 == 0) && (E % 4 == 0);
+
+  float bias[VPL];
+#pragma unroll
+  for (int v = 0; v < VPL; ++v) bias[v] = (SIGMOID && p.bias != nullptr && e0 + v < E) ? p.bias[e0 + v] : 0.0f;
+
+  for (int t = blockIdx.x * kGroupsPerBlock + gidx; t < p.T; t += gridDim.x * kGroupsPerBlock) {
+    // ---- load this lane's VPL logits ----
+    float x[VPL];
+    const float* row = p.logits + (size_t)t * E;
+    if (vec_ok) {
+#pragma unroll
+      for (int q = 0; q < VPL / 4; ++q) {
+        if (e0 + 4 * q < E) {
+          const uint4 u = ld_nc_v4(row + e0 + 4 * q);
+          x[4 * q + 0] = __uint_as_float(u.x);
+          x[4 * q + 1] = __uint_as_float(u.y);
+          x[4 * q + 2] = __uint_as_float(u.z);
+          x[4 * q + 3] = __uint_as_float(u.w);
+        } else {
+          x[4 * q + 0] = x[4 * q + 1] = x[4 * q + 2] = x[4 * q + 3] = NEG_INF;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < VPL; ++v) x[v] = (e0 + v < E) ? __ldg(row + e0 + v) : NEG_INF;
+    }
+    // ---- selection keys ----
+    float key[VPL];
+    uint32_t uk[VPL];
+#pragma unroll
+    for (int v = 0; v < VPL; ++v) {
+      if (SIGMOID) {
+        key[v] = (e0 + v < E) ? __fadd_rn(vsig(x[v]), bias[v]) : NEG_INF;
+      } else {
+        key[v] = x[v];
+      }
+      uk[v] = ordered_u32(key[v]);
+    }
+    // ---- group-limited routing (R6) ----
+    if (p.n_group > 1) {
+      const int gs = E / p.n_group;
+      if (p.fast_groups) {
+        const int lpg = gs / VPL;  // lanes per group (power of two)
+        float m1 = NEG_INF, m2 = NEG_INF;
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) {
+          const float c = key[v];
+          if (c > m1) { m2 = m1; m1 = c; } else if (c > m2) { m2 = c; }
+        }
+        for (int o = 1; o < lpg; o <<= 1) {
+          const float q1 = __shfl_xor_sync(gmask, m1, o);
+          const float q2 = __shfl_xor_sync(gmask, m2, o);
+          const float lo = fminf(m1, q1);
+          m1 = fmaxf(m1, q1);
+          m2 = fmaxf(lo, fmaxf(m2, q2));
+        }
+        const int g = e0 / gs;
+        float score = (gs >= 2) ? __fadd_rn(m1, m2) : m1;
+        if (e0 >= E) score = NEG_INF;
+        int rank = 0;
+        for (int g2 = 0; g2 < p.n_group; ++g2) {
+          const float s2 = __shfl_sync(gmask, score, (lane - sub) + g2 * lpg);
+          rank += (s2 > score || (s2 == score && g2 < g)) ? 1 : 0;
+        }
+        if (rank >= p.topk_group || e0 >= E) {
+#pragma unroll
+          for (int v = 0; v < VPL; ++v) uk[v] = ordered_u32(NEG_INF);
+        }
+      } else {
+        // generic: one pass per group, scores parked in shared memory
+        float* gsc = s_gscore + gidx * p.n_group;
+        for (int g2 = 0; g2 < p.n_group; ++g2) {
+          float m1 = NEG_INF, m2 = NEG_INF;
+#pragma unroll
+          for (int v = 0; v < VPL; ++v) {
+            const int e = e0 + v;
+            const float c = (e < E && e / gs == g2) ? key[v] : NEG_INF;
+            if (c > m1) { m2 = m1; m1 = c; } else if (c > m2) { m2 = c; }
+          }
+#pragma unroll
+          for (int o = 1; o < LANES; o <<= 1) {
+            const float q1 = __shfl_xor_sync(gmask, m1, o);
+            const float q2 = __shfl_xor_sync(gmask, m2, o);
+            const float lo = fminf(m1, q1);
+            m1 = fmaxf(m1, q1);
+            m2 = fmaxf(lo, fmaxf(m2, q2));
+          }
+          if (sub == 0) gsc[g2] = (gs >= 2) ? __fadd_rn(m1, m2) : m1;
+        }
+        __syncwarp(gmask);
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) {
+          const int e = e0 + v;
+          if (e < E) {
+            const int g = e / gs;
+            const float score = gsc[g];
+            int rank = 0;
+            for (int g2 = 0; g2 < p.n_group; ++g2) {
+              const float s2 = gsc[g2];
+              rank += (s2 > score || (s2 == score && g2 < g)) ? 1 : 0;
+            }
+            if (rank >= p.topk_group) uk[v] = ordered_u32(NEG_INF);
+          }
+        }
+        __syncwarp(gmask);
+      }
+    }
+    // ---- k rounds of arg-max, ties -> lowest index (R3) ----
+    int my_id = 0;
+    float my_x = 0.0f;
+    for (int j = 0; j < k; ++j) {
+      uint32_t lm = uk[0];
+#pragma unroll
+      for (int v = 1; v < VPL; ++v) lm = max(lm, uk[v]);
+      const uint32_t gm = group_max_u32<LANES>(gmask, lm);
+      const unsigned b = __ballot_sync(gmask, lm == gm) & gmask;
+      const int win = __ffs(b) - 1;
+      int id_local = 0;
+      float xv = 0.0f;
+      if (lane == win) {
+        bool found = false;
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) {
+          if (!found && uk[v] == gm) {
+            id_local = e0 + v;
+            xv = x[v];
+            uk[v] = kTaken;
+            found = true;
+          }
+        }
+      }
+      const int id = __shfl_sync(gmask, id_local, win);
+      const float xs = __shfl_sync(gmask, xv, win);
+      if (sub == j) { my_id = id; my_x = xs; }
+    }
+    // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
+    double wj = 0.0;
+    if (SIGMOID) {
+      const double sj = (sub < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
+      wj = sj;
+      if (p.renorm) wj = sj / group_sum_f64<LANES>(gmask, sj);
+    } else {
+      float lmx = x[0];
+#pragma unroll
+      for (int v = 1; v < VPL; ++v) lmx = fmaxf(lmx, x[v]);
+      const float mx = __uint_as_float([](uint32_t o) { return (o & 0x80000000u) ? (o & 0x7fffffffu) : ~o; }(
+          group_max_u32<LANES>(gmask, ordered_u32(lmx))));
+      const double ej = (sub < k) ? exp((double)my_x - (double)mx) : 0.0;
+      double denom;
+      if (p.renorm) {
+        denom = group_sum_f64<LANES>(gmask, ej);
+      } else {
+        double part = 0.0;
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) part += (e0 + v < E) ? (double)expf(x[v] - mx) : 0.0;
+        denom = group_sum_f64<LANES>(gmask, part);
+      }
+      wj = ej / denom;
+    }
+    wj *= (double)p.scale;
+    if (sub < k) {
+      p.ids[(size_t)t * k + sub] = my_id;
+      p.w[(size_t)t * k + sub] = __double2float_rn(wj);
+      atomicAdd(&s_hist[my_id], 1);
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
+    const int c = s_hist[i];
+    if (c) atomicAdd(&p.counts[i], c);
+  }
+}
+
+template <int LANES, int VPL>
+vibe_status launch_route(const RouteParams& p, bool sigmoid, cudaStream_t st) {
+  constexpr int gpb = 256 / LANES;
+  int blocks = (p.T + gpb - 1) / gpb;
+  const int cap = num_sms() * 8;
+  if (blocks > cap) blocks = cap;
+  size_t smem = (size_t)p.E * sizeof(int);
+  if (p.n_group > 1 && !p.fast_groups) smem += (size_t)gpb * p.n_group * sizeof(float);
+  if (sigmoid)
+    route_topk_kernel<LANES, VPL, true><<<blocks, 256, smem, st>>>(p);
+  else
+    route_topk_kernel<LANES, VPL, false><<<blocks, 256, smem, st>>>(p);
+  VIBE_LAUNCH_CHECK("route_topk_kernel");
+  return VIBE_OK;
+}
+
+}  // namespace
+}  // namespace vibe
+
+extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* logits, int32_t T, int32_t* topk_ids,
+                                       float* topk_w, int32_t* counts, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(cfg != nullptr, VIBE_ERR_INVALID_ARG, "vibe_route_topk: cfg is NULL");
+  const int E = cfg->num_experts, k = cfg->top_k;
+  VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_route_topk: need 1 <= k <= E (E=%d k=%d)", E, k);
+  VIBE_REQUIRE(T >= 0, VIBE_ERR_INVALID_ARG, "vibe_route_topk: T < 0");
+  VIBE_REQUIRE((int64_t)T * k < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG, "vibe_route_topk: T*k >= 2^31");
+  VIBE_REQUIRE(cfg->score_fn == VIBE_SCORE_SOFTMAX || cfg->score_fn == VIBE_SCORE_SIGMOID, VIBE_ERR_INVALID_ARG,
+               "vibe_route_topk: unknown score_fn %d", cfg->score_fn);
+  VIBE_REQUIRE(counts != nullptr, VIBE_ERR_INVALID_ARG, "vibe_route_topk: counts is NULL");
+  VIBE_REQUIRE(T == 0 || (logits && topk_ids && topk_w), VIBE_ERR_INVALID_ARG, "vibe_route_topk: NULL tensor");
+  VIBE_REQUIRE(T == 0 || aligned16(logits), VIBE_ERR_INVALID_ARG, "vibe_route_topk: logits must be 16-byte aligned");
+  const int ng = cfg->n_group > 1 ? cfg->n_group : 0;
+  if (ng) {
+    VIBE_REQUIRE(E % ng == 0, VIBE_ERR_INVALID_ARG, "vibe_route_topk: E %% n_group != 0");
+    VIBE_REQUIRE(cfg->topk_group >= 1 && cfg->topk_group <= ng, VIBE_ERR_INVALID_ARG,
+                 "vibe_route_topk: need 1 <= topk_group <= n_group");
+    VIBE_REQUIRE((int64_t)cfg->topk_group * (E / ng) >= k, VIBE_ERR_INVALID_ARG,
+                 "vibe_route_topk: topk_group * (E/n_group) < k");
+  }
+  VIBE_REQUIRE(E <= 512, VIBE_ERR_UNSUPPORTED, "vibe_route_topk: E > 512 not implemented");
+  VIBE_REQUIRE(k <= 32, VIBE_ERR_UNSUPPORTED, "vibe_route_topk: k > 32 not implemented");
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  VIBE_CUDA(cudaMemsetAsync(counts, 0, (size_t)E * sizeof(int32_t), st));
+  if (T == 0) return VIBE_OK;
+
+  RouteParams p;
+  p.logits = logits;
+  p.bias = cfg->select_bias;
+  p.ids = topk_ids;
+  p.w = topk_w;
+  p.counts = counts;
+  p.T = T;
+  p.E = E;
+  p.k = k;
+  p.renorm = cfg->renormalize ? 1 : 0;
+  p.scale = cfg->routed_scale;
+  p.n_group = ng;
+  p.topk_group = cfg->topk_group;
+  const bool sig = cfg->score_fn == VIBE_SCORE_SIGMOID;
+
+  int lanes, vpl;
+  if (E <= 64 && k <= 8) {
+    lanes = 8;
+    vpl = E <= 8 ? 1 : E <= 16 ? 2 : E <= 32 ? 4 : 8;
+  } else {
+    lanes = 32;
+    vpl = E <= 32 ? 1 : E <= 64 ? 2 : E <= 128 ? 4 : E <= 256 ? 8 : 16;
+  }
+  p.fast_groups = 0;
+  if (ng) {
+    const int gs = E / ng;
+    if (gs % vpl == 0) {
+      const int lpg = gs / vpl;
+      if ((lpg & (lpg - 1)) == 0 && lpg <= lanes) p.fast_groups = 1;
+    }
+    VIBE_REQUIRE(p.fast_groups || ng <= 64, VIBE_ERR_UNSUPPORTED,
+                 "vibe_route_topk: n_group > 64 with irregular group size not implemented");
+  }
+#define VIBE_ROUTE_CASE(L, V) \
+  if (lanes == L && vpl == V) return launch_route<L, V>(p, sig, st);
+  VIBE_ROUTE_CASE(8, 1)
+  VIBE_ROUTE_CASE(8, 2)
+  VIBE_ROUTE_CASE(8, 4)
+  VIBE_ROUTE_CASE(8, 8)
+  VIBE_ROUTE_CASE(32, 1)
+  VIBE_ROUTE_CASE(32, 2)
+  VIBE_ROUTE_CASE(32, 4)
+  VIBE_ROUTE_CASE(32, 8)
+  VIBE_ROUTE_CASE(32, 16)
+#undef VIBE_ROUTE_CASE
+  set_error("vibe_route_topk: no kernel for E=%d k=%d", E, k);
+  return VIBE_ERR_UNSUPPORTED;
+}
