@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the per-GPU MoE-layer hot path (route -> permute -> grouped
+SwiGLU FFN -> combine) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C1]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is ONE pass of the whole hot path over one batch of synthetic input (BASELINE.json
+configs[1], the Mixtral-8x7B-shaped layer, unless --config says otherwise).  `value` is
+whole-job tokens/s with inputs resident in HBM; `e2e` is the same metric through the C-ABI
+call that takes HOST buffers (H2D of logits+X and D2H of out+counts inside the timed region).
+N > 1: independent replicas, one per GPU, no data-path collective.
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "moe_layer_tokens_per_s"
+UNIT = "tokens/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                    "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"]))}, "measured"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def load_ncu_traffic(config_name: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "ffn_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(config_name)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self._stop_evt = threading.Event()
+        self.max_mhz = None
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                self.reason_bits |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power.append(self.nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        out = {"sm_mhz": int(statistics.median(self.samples)) if self.samples else None,
+               "sm_max_mhz": self.max_mhz,
+               "reasons": [n for b, n in sorted(self.REASONS.items()) if self.reason_bits & b],
+               "samples": len(self.samples)}
+        if self.power:
+            out["power_w_max"] = round(max(self.power), 1)
+        return out
+
+
+def oracle_sample_step(O, I, cfg, L, S):
+    """The whole hot path in the oracle on the first S tokens of a batch."""
+    lg, X = L["logits"][:S], L["X"][:S]
+    ids, w, counts = O.route_topk(lg, select_bias=L["select_bias"], **I.route_kwargs(cfg))
+    em = L["expert_map"] if cfg.E_loc < cfg.E else None
+    off, r2a, a2r, Xp, R = O.permute(X, ids, em, cfg.E_loc, 1)
+    Y, _ = O.grouped_ffn(Xp, off, r2a, L["W1"], L["W3"], L["W2"])
+    out = O.combine(Y, a2r, w, S, cfg.k, round_out=True)
+    return out, int((np.diff(off) > 0).sum())
+
+
+def run_reference(args, group):
+    """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
+    if not group.is_main:
+        return
+    from oracle import vibe_oracle as O
+    from paper_2606_00735_b200 import inputs as I
+    cfg = I.CONFIGS[args.config]
+    L = I.make_layer(cfg, args.seed)
+    cores = len(os.sched_getaffinity(0))
+    # bounded sample: per step the oracle converts every touched expert's bf16 weights to f64
+    # (~3*d*f elements each); choose the largest S whose estimated cost fits the step budget
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    t0 = time.perf_counter()
+    O.bf16_bits_to_f64(L["W1"][0])
+    per_expert = 3.3 * (time.perf_counter() - t0) + 6.0 * cfg.d * cfg.f * 8 / 20e9
+    S = 1
+    for cand in (2, 4, 8, 16, 32, 64, 128, 256):
+        touched = min(cfg.E_loc, cand * cfg.k)
+        if cand <= cfg.T and touched * per_expert <= budget:
+            S = cand
+    for _ in range(args.warmup):
+        oracle_sample_step(O, I, cfg, L, S)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_sample_step(O, I, cfg, L, S)
+    dt = time.perf_counter() - t0
+    value = S * args.steps / dt
+    sample = f"first {S} of {cfg.T} tokens per step through oracle route+permute+grouped_ffn+combine (fp64 numpy)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "T": cfg.T, "d": cfg.d, "f": cfg.f, "E": cfg.E, "k": cfg.k,
+                   "E_loc": cfg.E_loc, "sample_tokens_per_step": S},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--sets", type=int, default=4, help="rotating input buffer sets")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    from paper_2606_00735_b200 import dist as D
+    if args.impl == "reference":
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        if world > 1 and int(os.environ.get("RANK", "0")) != 0:
+            return                      # other ranks exit 0 without work
+        run_reference(args, D.Group(0, 1, 0, None))
+        return
+
+    import torch
+    from paper_2606_00735_b200 import binding as B
+    from paper_2606_00735_b200 import inputs as I
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product has no CPU fallback (use --impl reference "
+                         "for the oracle)")
+    group = D.init_from_env()
+    torch.cuda.set_device(group.local_rank)
+    dev = torch.device("cuda", group.local_rank)
+    B.load()
+    cfg = I.CONFIGS[args.config]
+    peaks, peak_kind = load_peaks()
+
+    # ---------------------------------------------------------------- inputs (seeded, numpy)
+    def pin_bf16(shape):
+        return torch.empty(shape, dtype=torch.bfloat16).pin_memory()
+
+    Wh = [pin_bf16((cfg.E_loc, cfg.d, cfg.f)), pin_bf16((cfg.E_loc, cfg.d, cfg.f)), pin_bf16((cfg.E_loc, cfg.f, cfg.d))]
+    I.make_weights(cfg.E_loc, cfg.d, cfg.f, args.seed,
+                   out=[w.view(torch.int16).numpy().view(np.uint16) for w in Wh])
+    W1, W3, W2 = (w.to(dev, non_blocking=True) for w in Wh)
+    emap_np = I.make_expert_map(cfg, "contiguous", args.seed)
+    emap = torch.from_numpy(emap_np).to(dev) if cfg.E_loc < cfg.E else None
+    bias_np = I.make_select_bias(cfg.E, args.seed) if cfg.has_select_bias else None
+    bias = torch.from_numpy(bias_np).to(dev) if bias_np is not None else None
+    rc = B.RouteConfig(select_bias=bias, **I.route_kwargs(cfg))
+    sets_h, sets_d = [], []
+    for i in range(args.sets):
+        lg = torch.from_numpy(I.make_logits(cfg.T, cfg.E, cfg.zipf_s, args.seed + i, cfg.alpha)).pin_memory()
+        Xb = torch.from_numpy(I.make_X(cfg.T, cfg.d, args.seed + i).view(np.int16)).view(torch.bfloat16).pin_memory()
+        sets_h.append((lg, Xb))
+        sets_d.append((lg.to(dev), Xb.to(dev)))
+    T, k, E, E_loc, d, f = cfg.T, cfg.k, cfg.E, cfg.E_loc, cfg.d, cfg.f
+    A = T * k
+    Rcap = max(1, B.rows_cap(T, k, E_loc, 1))
+    ids = torch.empty((T, k), dtype=torch.int32, device=dev)
+    gw = torch.empty((T, k), dtype=torch.float32, device=dev)
+    counts = torch.empty((E,), dtype=torch.int32, device=dev)
+    Xp = torch.empty((Rcap, d), dtype=torch.bfloat16, device=dev)
+    H = torch.empty((Rcap, f), dtype=torch.bfloat16, device=dev)
+    Y = torch.empty((Rcap, d), dtype=torch.bfloat16, device=dev)
+    off = torch.empty((E_loc + 1,), dtype=torch.int32, device=dev)
+    r2a = torch.empty((Rcap,), dtype=torch.int32, device=dev)
+    a2r = torch.empty((A,), dtype=torch.int32, device=dev)
+    out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+    pws = torch.empty((max(16, B.workspace_bytes(B.WS_PERMUTE, T, k, E, E_loc, d, f)),), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(i, ev=None):
+        lg, Xd = sets_d[i % args.sets]
+        if ev:
+            ev[0].record(stream)
+        B.route_topk(lg, rc, out=(ids, gw, counts), stream=stream)
+        if ev:
+            ev[1].record(stream)
+        B.permute(Xd, ids, counts, emap, E, E_loc, 1, out=(Xp, off, r2a, a2r), ws=pws, stream=stream)
+        if ev:
+            ev[2].record(stream)
+        B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y, stream=stream)
+        if ev:
+            ev[3].record(stream)
+        B.combine(Y, a2r, gw, T, k, out=out, stream=stream)
+        if ev:
+            ev[4].record(stream)
+
+    # ---------------------------------------------------------------- device-resident timing
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(group.local_rank)
+    group.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    n0 = B.launch_count()
+    t_start.record(stream)
+    for i in range(args.steps):
+        step(i, evs[i])
+    t_end.record(stream)
+    torch.cuda.synchronize()
+    launches = B.launch_count() - n0
+    clocks = sampler.stop()
+    group.barrier()
+    my_ms = t_start.elapsed_time(t_end)
+    value, max_ms = D.aggregate_throughput(group, float(T) * args.steps, my_ms)
+    stage_ms = [sum(e[j].elapsed_time(e[j + 1]) for e in evs) / args.steps for j in range(4)]
+
+    # real rows / resident tokens of the routed batch (for algorithmic bytes and flops)
+    R_real = int(off[-1].item())
+    res_tok = int((a2r.view(T, k) >= 0).any(dim=1).sum().item())
+
+    # ---------------------------------------------------------------- end to end from host buffers
+    arena = torch.empty((B.workspace_bytes(B.WS_LAYER_HOST, T, k, E, E_loc, d, f),), dtype=torch.uint8, device=dev)
+    out_h = torch.empty((T, d), dtype=torch.bfloat16).pin_memory()
+    cnt_h = torch.empty((E,), dtype=torch.int32).pin_memory()
+    for i in range(3):
+        B.moe_layer_forward_host(rc, *sets_h[i % args.sets], emap, W1, W3, W2, out_h, cnt_h, arena, stream=stream)
+    group.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(args.steps):
+        B.moe_layer_forward_host(rc, *sets_h[i % args.sets], emap, W1, W3, W2, out_h, cnt_h, arena, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    group.barrier()
+    e2e_value, _ = D.aggregate_throughput(group, float(T) * args.steps, e0.elapsed_time(e1))
+    h2d = T * E * 4 + T * d * 2
+    d2h = T * d * 2 + E * 4
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel
+    ffn_s = stage_ms[2] * 1e-3
+    flops = 6.0 * R_real * d * f
+    achieved_tf = flops / ffn_s / 1e12
+    sustained = peaks["bf16_tflops_sustained"]
+    roofline = {"kernel": "ffn_gemm_kernel (2 launches per step: gate_up+SwiGLU, down)", "bound": "tensor",
+                "achieved": round(achieved_tf, 2), "peak": sustained, "unit": "TFLOP/s",
+                "frac": round(achieved_tf / sustained, 4), "traffic": load_ncu_traffic(cfg.name),
+                "peak_kind": f"{peak_kind} sustained cuBLAS bf16 (kernel timed inside a long step)",
+                "frac_of_burst": round(achieved_tf / peaks["bf16_tflops"], 4),
+                "flops_per_step": flops, "ms_per_step": round(stage_ms[2], 4)}
+    hbm = peaks["hbm_gbs"]
+    bytes_route = 4.0 * T * E + 8.0 * T * k + 4.0 * E
+    bytes_perm = 2.0 * res_tok * d + 2.0 * R_real * d + 12.0 * A
+    bytes_comb = 2.0 * R_real * d + 2.0 * T * d + 8.0 * A
+    stages = {}
+    for name, ms, by in (("route", stage_ms[0], bytes_route), ("permute", stage_ms[1], bytes_perm),
+                         ("combine", stage_ms[3], bytes_comb)):
+        gbs = by / (ms * 1e-3) / 1e9
+        stages[name] = {"ms": round(ms, 4), "GB/s": round(gbs, 1), "frac_hbm": round(gbs / hbm, 4)}
+    stages["grouped_ffn"] = {"ms": round(stage_ms[2], 4), "TFLOP/s": round(achieved_tf, 2)}
+
+    # ---------------------------------------------------------------- CPU baseline (oracle, rank 0, N = 1)
+    cpu_baseline = None
+    if group.is_main and group.world == 1 and not args.no_cpu_baseline:
+        from oracle import vibe_oracle as O
+        S = min(T, 128)
+        L = {"logits": sets_h[0][0].numpy(), "X": sets_h[0][1].view(torch.int16).numpy().view(np.uint16),
+             "select_bias": bias_np, "expert_map": emap_np,
+             "W1": Wh[0].view(torch.int16).numpy().view(np.uint16),
+             "W3": Wh[1].view(torch.int16).numpy().view(np.uint16),
+             "W2": Wh[2].view(torch.int16).numpy().view(np.uint16)}
+        t0 = time.perf_counter()
+        ref_out, touched = oracle_sample_step(O, I, cfg, L, S)
+        dt = time.perf_counter() - t0
+        cpu_baseline = {"value": S / dt, "unit": UNIT, "cores": len(os.sched_getaffinity(0)), "kind": "oracle",
+                        "sample": f"first {S} of {T} tokens of batch 0 through the fp64 numpy oracle "
+                                  f"(route+permute+grouped_ffn+combine, {touched} experts touched), {dt:.1f} s"}
+
+    if group.is_main:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": group.world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": cfg.name, "T": T, "d": d, "f": f, "E": E, "k": k, "E_loc": E_loc,
+                       "routing": f"zipf_s={cfg.zipf_s} alpha={cfg.alpha}", "real_rows": R_real,
+                       "parallelism": "replicas" if group.world > 1 else "single-gpu",
+                       "l2": f"inputs rotate over {args.sets} buffer sets; "
+                             f"{(3 * E_loc * d * f * 2) / 1e9:.2f} GB of weights stream through the 126 MB L2 every step"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+            "stages": stages,
+            "ffn_tflops": round(achieved_tf, 2),
+        }
+        print(json.dumps(line), flush=True)
+    group.close()
+
+
+if __name__ == "__main__":
+    main()
