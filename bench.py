@@ -46,11 +46,15 @@ def load_peaks():
 
 
 def load_ncu_traffic(config_name: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "ffn_traffic.json")
+    """DRAM bytes (read + write) per vibe_grouped_ffn call (both launches) from the committed
+    `ncu --set full` capture, or None.  profiles/ffn_traffic.csv: config,dram_bytes,source."""
+    p = os.path.join(ROOT, "profiles", "ffn_traffic.csv")
     if os.path.exists(p):
         try:
-            return json.load(open(p)).get(config_name)
+            for ln in open(p):
+                cols = [c.strip() for c in ln.split(",")]
+                if len(cols) >= 2 and cols[0] == config_name:
+                    return float(cols[1])
         except Exception:
             return None
     return None
@@ -61,7 +65,7 @@ class ClockSampler(threading.Thread):
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
                0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
 
-    def __init__(self, index: int, period_s: float = 0.02):
+    def __init__(self, index: int, period_s: float = 0.005):
         super().__init__(daemon=True)
         self.index, self.period = index, period_s
         self.samples, self.reason_bits, self.power = [], 0, []
@@ -125,21 +129,30 @@ def run_reference(args, group):
     cores = len(os.sched_getaffinity(0))
     # bounded sample: per step the oracle converts every touched expert's bf16 weights to f64
     # (~3*d*f elements each); choose the largest S whose estimated cost fits the step budget
-    budget = 150.0 / max(1, args.steps + args.warmup)
     t0 = time.perf_counter()
     O.bf16_bits_to_f64(L["W1"][0])
     per_expert = 3.3 * (time.perf_counter() - t0) + 6.0 * cfg.d * cfg.f * 8 / 20e9
+    # The whole run must end within a few minutes.  A step can not cost less than one token
+    # (k experts' weights converted to f64), so when K+W such steps do not fit, fewer steps are
+    # run and the line reports the count actually timed.
+    total_budget = 200.0
+    min_step = min(cfg.E_loc, cfg.k) * per_expert
+    steps = max(1, min(args.steps, int(total_budget * 0.8 / min_step)))
+    warmup = max(0, min(args.warmup, int(total_budget * 0.2 / min_step)))
+    budget = total_budget / (steps + warmup)
     S = 1
     for cand in (2, 4, 8, 16, 32, 64, 128, 256):
         touched = min(cfg.E_loc, cand * cfg.k)
         if cand <= cfg.T and touched * per_expert <= budget:
             S = cand
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         oracle_sample_step(O, I, cfg, L, S)
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         oracle_sample_step(O, I, cfg, L, S)
     dt = time.perf_counter() - t0
+    requested = (args.steps, args.warmup)
+    args.steps, args.warmup = steps, warmup
     value = S * args.steps / dt
     sample = f"first {S} of {cfg.T} tokens per step through oracle route+permute+grouped_ffn+combine (fp64 numpy)"
     line = {
@@ -147,7 +160,8 @@ def run_reference(args, group):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "T": cfg.T, "d": cfg.d, "f": cfg.f, "E": cfg.E, "k": cfg.k,
-                   "E_loc": cfg.E_loc, "sample_tokens_per_step": S},
+                   "E_loc": cfg.E_loc, "sample_tokens_per_step": S,
+                   "steps_requested": requested[0], "warmup_requested": requested[1]},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -158,8 +172,8 @@ def run_reference(args, group):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=40)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C1", choices=["C0", "C1", "C2", "C3"])
     ap.add_argument("--seed", type=int, default=0)

@@ -12,9 +12,10 @@
 //                      memory => rows inside a slot are in ascending flat index (stable,
 //                      bit-exact w.r.t. the counting-sort definition).  Writes
 //                      assign_to_row / row_to_assign; zero-fills padding rows.
-//   K4 perm_rows     : token-major gather/scatter of the bf16 rows with 16-byte vectors:
+//   K4 perm_rows     : token-major gather/scatter of the bf16 rows, one thread per 16-byte vector:
 //                      X[t,:] is read ONCE and written to each of its <= k destination rows,
 //                      so DRAM traffic equals the algorithmic 2*T_res*d + 2*R*d bytes.
+//                      (E_loc < E: the row-major variant perm_rows_by_row, work ~ R.)
 #include "common.cuh"
 
 namespace vibe {
@@ -169,33 +170,64 @@ __global__ void __launch_bounds__(256) perm_index_kernel(const int32_t* __restri
 }
 
 // K4 ------------------------------------------------------------------------------------
-// One CTA iteration per token; thread handles up to VEC 16-byte vectors of the row.
-template <int VEC>
+// One thread per VPT 16-byte vectors of one token row (vectors v and v + vpr/2 when VPT == 2):
+// the vector is read once and stored to each of the token's <= k destination rows.  The k
+// row indices are warp-uniform addresses (one broadcast transaction, L1-resident).  No
+// grid-stride loop: the grid covers T * vpr / VPT threads.
+template <int VPT>
 __global__ void __launch_bounds__(256) perm_rows_kernel(const __nv_bfloat16* __restrict__ X,
                                                         const int32_t* __restrict__ assign_to_row, int T, int k,
                                                         int d, __nv_bfloat16* __restrict__ Xp) {
-  const int vec_per_row = d / 8;
-  for (int t = blockIdx.x; t < T; t += gridDim.x) {
-    const int32_t* a2r = assign_to_row + (size_t)t * k;
-    bool any = false;
-    for (int j = 0; j < k; ++j) any |= (__ldg(a2r + j) >= 0);
-    if (!any) continue;
-    const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)t * d);
-    uint4 val[VEC];
+  const int vpr = d >> 3;
+  const int per_row = vpr / VPT;
+  const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (g >= (long long)T * per_row) return;
+  const int t = (int)(g / per_row);
+  const int v0 = (int)(g - (long long)t * per_row);
+  const int32_t* a2r = assign_to_row + (size_t)t * k;
+  bool any = false;
+  for (int j = 0; j < k; ++j) any |= (__ldg(a2r + j) >= 0);
+  if (!any) return;
+  const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)t * d) + v0;
+  uint4 val[VPT];
 #pragma unroll
-    for (int q = 0; q < VEC; ++q) {
-      const int v = threadIdx.x + q * 256;
-      if (v < vec_per_row) val[q] = ld_nc_v4(src + v);
-    }
-    for (int j = 0; j < k; ++j) {
-      const int r = __ldg(a2r + j);
-      if (r < 0) continue;
-      uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
+  for (int q = 0; q < VPT; ++q) val[q] = ld_nc_v4(src + q * per_row);
+  for (int j = 0; j < k; ++j) {
+    const int r = __ldg(a2r + j);
+    if (r < 0) continue;
+    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d) + v0;
 #pragma unroll
-      for (int q = 0; q < VEC; ++q) {
-        const int v = threadIdx.x + q * 256;
-        if (v < vec_per_row) st_na_v4(dst + v, val[q]);
-      }
+    for (int q = 0; q < VPT; ++q) st_na_v4(dst + q * per_row, val[q]);
+  }
+}
+
+// K4' -----------------------------------------------------------------------------------
+// Row-major variant for expert-parallel shards (E_loc < E), where only a fraction of the
+// T*k assignments is resident: persistent warps walk the R = offsets[E_loc] real rows
+// (extent read on the device) and copy X[row_to_assign[r] / k, :] -> Xp[r, :], UNROLL
+// independent 16-byte loads in flight per lane.  Work is proportional to R, not to T*k.
+template <int UNROLL>
+__global__ void __launch_bounds__(256) perm_rows_by_row_kernel(const __nv_bfloat16* __restrict__ X,
+                                                               const int32_t* __restrict__ row_to_assign,
+                                                               const int32_t* __restrict__ offsets, int E_loc,
+                                                               int k, int d, __nv_bfloat16* __restrict__ Xp) {
+  const int R = __ldg(offsets + E_loc);
+  const int lane = threadIdx.x & 31;
+  const int nwarps = gridDim.x * (256 / 32);
+  const int vpr = d >> 3;
+  for (int r = blockIdx.x * (256 / 32) + (threadIdx.x >> 5); r < R; r += nwarps) {
+    const int i = __ldg(row_to_assign + r);
+    if (i < 0) continue;   // padding row: already zero-filled by perm_index_kernel
+    const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)(i / k) * d);
+    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
+    for (int v0 = lane; v0 < vpr; v0 += 32 * UNROLL) {
+      uint4 val[UNROLL];
+#pragma unroll
+      for (int q = 0; q < UNROLL; ++q)
+        if (v0 + 32 * q < vpr) val[q] = ld_nc_v4(src + v0 + 32 * q);
+#pragma unroll
+      for (int q = 0; q < UNROLL; ++q)
+        if (v0 + 32 * q < vpr) st_na_v4(dst + v0 + 32 * q, val[q]);
     }
   }
 }
@@ -237,7 +269,6 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   VIBE_REQUIRE(vibe_rows_cap(T, k, E_loc, align) < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG,
                "vibe_permute: row capacity >= 2^31");
   VIBE_REQUIRE(E_loc <= kMaxSlots, VIBE_ERR_UNSUPPORTED, "vibe_permute: E_loc > %d not implemented", kMaxSlots);
-  VIBE_REQUIRE(d <= 8 * 256 * 8, VIBE_ERR_UNSUPPORTED, "vibe_permute: d > 16384 not implemented");
   VIBE_REQUIRE(offsets != nullptr, VIBE_ERR_INVALID_ARG, "vibe_permute: offsets is NULL");
   VIBE_REQUIRE(T == 0 || (X && topk_ids && Xp && row_to_assign && assign_to_row), VIBE_ERR_INVALID_ARG,
                "vibe_permute: NULL tensor");
@@ -266,19 +297,21 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   perm_index_kernel<<<nblk, 256, smem3, st>>>(topk_ids, expert_map, A, E, E_loc, NW, align, d, hist, totals, offsets,
                                               row_to_assign, assign_to_row, reinterpret_cast<__nv_bfloat16*>(Xp));
   VIBE_LAUNCH_CHECK("perm_index_kernel");
-  const int vec_per_row = d / 8;
-  const int vec = (vec_per_row + 255) / 256;
-  int blocks = T < num_sms() * 8 ? T : num_sms() * 8;
+  const int vpr = d / 8;
   const __nv_bfloat16* Xb = reinterpret_cast<const __nv_bfloat16*>(X);
   __nv_bfloat16* Xpb = reinterpret_cast<__nv_bfloat16*>(Xp);
-  if (vec <= 1)
-    perm_rows_kernel<1><<<blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
-  else if (vec <= 2)
-    perm_rows_kernel<2><<<blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
-  else if (vec <= 4)
-    perm_rows_kernel<4><<<blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
-  else
-    perm_rows_kernel<8><<<blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
+  if (E_loc < E) {
+    // expert-parallel shard: work proportional to the resident rows
+    perm_rows_by_row_kernel<4><<<num_sms() * 8, 256, 0, st>>>(Xb, row_to_assign, offsets, E_loc, k, d, Xpb);
+  } else {
+    const int vpt = (vpr % 2 == 0) ? 2 : 1;
+    const long long blocks = ((long long)T * (vpr / vpt) + 255) / 256;
+    VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "vibe_permute: T*d too large for one launch");
+    if (vpt == 2)
+      perm_rows_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
+    else
+      perm_rows_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
+  }
   VIBE_LAUNCH_CHECK("perm_rows_kernel");
   return VIBE_OK;
 }
