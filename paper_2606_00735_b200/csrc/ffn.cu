@@ -1,24 +1,38 @@
 // ffn.cu -- a4: grouped SwiGLU expert FFN (vibe_grouped_ffn) on 5th-gen tensor cores.
 //
-// Two launches of one persistent, warp-specialised tcgen05 kernel (one CTA per SM):
-//   GEMM-1  H[r, n0:n0+128]  = silu(Xp[r,:] W1[s][:, n0:..]) * (Xp[r,:] W3[s][:, n0:..])   K = d
-//           one UMMA of N = 256 per K-step: columns 0..127 gate, 128..255 up; SwiGLU is
-//           applied in the epilogue straight out of TMEM (H never exists in fp32 in HBM).
-//   GEMM-2  Y[r, n0:n0+256]  = H[r,:] W2[s][:, n0:..]                                     K = f
+// Two launches of one persistent, warp-specialised tcgen05 kernel; the grid is 74 CTA PAIRS
+// (clusters of 2, one CTA per SM) and every MMA is a cta_group::2 instruction of M = 256.
+//
+// "Swap-AB": the WEIGHTS are the UMMA A operand (M side = output features, always full
+// tiles) and the TOKENS are the B operand (N side).  The ragged dimension -- rows per expert --
+// therefore lands on UMMA N, which is a runtime field of the instruction descriptor with a
+// granularity of 16: an expert with n rows costs roundup(n,16) columns of MMA work, not
+// roundup(n,128) rows, and the last tile of every expert is exactly as wide as it needs to be.
+//
+//   GEMM-1  H^T[n, r] = silu(W1[s]^T Xp^T) * (W3[s]^T Xp^T)      K = d
+//           pair tile = 128 features x <=256 tokens.  Each CTA's A tile is two 64-feature
+//           TMA atoms: its 64 gate features (W1) in TMEM lanes 0..63 and the SAME 64 features
+//           of W3 in lanes 64..127, so ONE MMA stream produces gate and up; the epilogue
+//           warps of the two lane halves swap 32-column blocks through shared memory and
+//           apply SwiGLU out of TMEM (H never exists in fp32 in HBM).
+//   GEMM-2  Y^T[n, r] = W2[s]^T H^T                               K = f
+//           pair tile = 256 features x <=256 tokens.
 // Operands:
-//   A (activations, K-major)   : ONE 2-D TMA map over all permuted rows; the row coordinate
-//                                is offsets[s] + 128*m_blk, taken from the device-side
-//                                offsets -> no per-expert descriptors, no host sync.
-//   B (weights [E_loc,K,N], N contiguous = "MN-major") : ONE 3-D TMA map (N, K, E_loc),
-//                                consumed IN PLACE through MN-major UMMA descriptors --
-//                                no weight repacking.
-// Rows of a 128-row tile that spill past the end of the expert's segment are computed and
-// masked at the store; rows past R_cap are zero-filled by TMA.
-// Pipeline: warp 0 = TMA producer, warp 1 = UMMA issuer (+ TMEM owner), warps 2..5 = epilogue.
-// 4 smem stages x 48 KB (A 128x64, B 256x64), 2 TMEM accumulator stages x 256 columns so the
+//   A (weights [E_loc,K,N], N contiguous = "MN-major"): ONE 3-D TMA map (N, K, E_loc), 64x64
+//       boxes, consumed IN PLACE through MN-major UMMA descriptors -- no weight repacking.
+//   B (activations [R_cap,K], K-major): ONE 2-D TMA map over all permuted rows; the row
+//       coordinate comes from the device-side offsets -> no per-expert descriptors, no host
+//       sync.  Each CTA of the pair loads HALF of the token tile (cta_group::2 takes N/2
+//       columns of B from each CTA), so per-SM shared-memory fill is 32 KB per 64-deep K step.
+// Token columns past the end of the expert's segment are computed on whatever the box holds
+// and masked at the store (columns are independent, nothing leaks); rows past R_cap are
+// zero-filled by TMA.
+// Pipeline: warp 0 = TMA producer (both CTAs), warp 1 = UMMA issuer (leader CTA) + TMEM owner,
+// warps 2..5 = epilogue.  6 smem stages x 32 KB, 2 TMEM accumulator stages x 256 columns so the
 // epilogue of tile i overlaps the MMAs of tile i+1.
-// Tile order: expert-major, then n-block, then m-block fastest, so CTAs that run at the
-// same time share the same weight tile through L2 and each weight byte leaves HBM once.
+// Tile order: expert-major, then feature block, then token tile fastest, so pairs that run at
+// the same time share a weight tile through L2 (both operands evict_last) and each weight byte
+// leaves HBM once.
 //
 // Semantics: include/vibe.h (vibe_grouped_ffn); F1-F4.
 #include <mutex>
@@ -32,40 +46,41 @@
 namespace vibe {
 namespace {
 
-constexpr int BM = 128;                 // rows per tile (UMMA M)
 constexpr int BK = 64;                  // K per smem stage (one 128-byte swizzle atom of bf16)
-constexpr int UMMA_N = 256;             // accumulator columns per tile
+constexpr int TN = 256;                 // tokens per tile = max UMMA N
 constexpr int UMMA_K = 16;
-constexpr int STAGES = 4;
-constexpr int A_BYTES = BM * BK * 2;            // 16 KB
-constexpr int B_ATOM_BYTES = 64 * BK * 2;       // 8 KB : 64 N-columns x 64 K-rows
-constexpr int B_BYTES = 4 * B_ATOM_BYTES;       // 32 KB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 48 KB
+constexpr int STAGES = 6;
+constexpr int ATOM_BYTES = 64 * BK * 2;         // 8 KB : 64 features x 64 K (MN-major, SW128)
+constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumulator lanes
+constexpr int B_BYTES = (TN / 2) * BK * 2;      // 16 KB: this CTA's half of the token tile
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
+constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
 constexpr int NUM_THREADS = 192;
-constexpr int MAX_SLOTS = 1024;
+constexpr int MAX_SLOTS = 512;
 constexpr int TMEM_COLS = 512;
 
 struct SmemTail {
-  uint64_t full[STAGES];
-  uint64_t empty[STAGES];
-  uint64_t tfull[2];
-  uint64_t tempty[2];
+  uint64_t full[STAGES];          // leader CTA: both CTAs' TMA bytes of a stage have landed
+  uint64_t empty[STAGES];         // each CTA: the MMAs reading the stage have retired
+  uint64_t tfull[2];              // each CTA: accumulator stage complete
+  uint64_t tempty[2];             // leader CTA: all 8 epilogue warps of the pair drained it
   uint32_t tmem_base;
-  int32_t total_m_tiles;
+  int32_t total_t_tiles;
   int32_t off[MAX_SLOTS + 1];     // segment starts (rows)
-  int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of m-tiles per slot
+  int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
 };
-constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + sizeof(SmemTail);
+constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + sizeof(SmemTail);
+static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB dynamic shared memory of sm_100");
 
 struct TileCursor {
   int e = 0;
-  // Decode tile id -> (slot e, m_blk, n_blk).  Tiles ids are monotone per CTA, so e only advances.
-  __device__ __forceinline__ void decode(const SmemTail* t, int tile, int NB, int& m_blk, int& n_blk) {
+  // tile id -> (slot e, feature block, token tile).  Tile ids are monotone per CTA, so e only advances.
+  __device__ __forceinline__ void decode(const SmemTail* t, int tile, int NB, int& f_blk, int& t_blk) {
     while (tile >= t->cum[e + 1] * NB) ++e;
     const int local = tile - t->cum[e] * NB;
-    const int mt = t->cum[e + 1] - t->cum[e];
-    n_blk = local / mt;
-    m_blk = local - n_blk * mt;
+    const int tt = t->cum[e + 1] - t->cum[e];
+    f_blk = local / tt;
+    t_blk = local - f_blk * tt;
   }
 };
 
@@ -73,39 +88,61 @@ __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<const uint32_t*>(&h);
 }
+__device__ __forceinline__ float swiglu(float g, float u) { return __fdividef(g, 1.0f + __expf(-g)) * u; }
+
+// Store a 32-lane x 32-column block held one lane (= feature) per thread, v[i] = column
+// (= token) i, into row-major out[token][feature].  Lanes pair up so that every store is a
+// bf16x2 of two adjacent features: even lanes store the even columns, odd lanes the odd ones.
+__device__ __forceinline__ void store_block_T(const float (&v)[32], __nv_bfloat16* __restrict__ out, size_t ld,
+                                              int row0, int n_rows, int feat, bool feat_ok, int lane) {
+  const bool odd = lane & 1;
+  __nv_bfloat16* base = out + (size_t)row0 * ld + (feat - (odd ? 1 : 0));
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    const float send = odd ? v[i] : v[i + 1];
+    const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
+    const int tok = i + (odd ? 1 : 0);
+    const uint32_t pk = odd ? pack2_bf16(recv, v[i + 1]) : pack2_bf16(v[i], recv);
+    if (feat_ok && tok < n_rows) *reinterpret_cast<uint32_t*>(base + (size_t)tok * ld) = pk;
+  }
+}
 
 template <bool kGateUp>
-__global__ void __launch_bounds__(NUM_THREADS, 1)
-ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
-                const __grid_constant__ CUtensorMap tmB1, const int32_t* __restrict__ offsets, int E_loc,
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
+                const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
                 int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out) {
-  constexpr int BN_OUT = kGateUp ? 128 : 256;  // output columns per tile
+  constexpr int FB = kGateUp ? 128 : 256;   // output features per pair tile
+  constexpr int FC = FB / 2;                // ... per CTA
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  SmemTail* tail = reinterpret_cast<SmemTail*>(smem + (size_t)STAGES * STAGE_BYTES);
+  float* xchg = reinterpret_cast<float*>(smem + (size_t)STAGES * STAGE_BYTES);
+  SmemTail* tail = reinterpret_cast<SmemTail*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int NB = (n_total + BN_OUT - 1) / BN_OUT;
+  const uint32_t rank = ptx::cluster_ctarank();      // 0 = leader (issues the MMAs)
+  const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
+  const int NB = (n_total + FB - 1) / FB;
   const int KB = k_total / BK;
 
   // ------------------------------------------------------------------ setup
   if (warp == 0 && lane == 0) {
-    ptx::prefetch_tensormap(&tmA);
-    ptx::prefetch_tensormap(&tmB0);
-    if (kGateUp) ptx::prefetch_tensormap(&tmB1);
+    ptx::prefetch_tensormap(&tmAct);
+    ptx::prefetch_tensormap(&tmW0);
+    if (kGateUp) ptx::prefetch_tensormap(&tmW1);
     for (int s = 0; s < STAGES; ++s) {
       ptx::mbar_init(ptx::smem_u32(&tail->full[s]), 1);
       ptx::mbar_init(ptx::smem_u32(&tail->empty[s]), 1);
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(ptx::smem_u32(&tail->tfull[a]), 1);
-      ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 4);
+      ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 8);
     }
     ptx::fence_barrier_init();
   } else if (warp == 1) {
-    ptx::tmem_alloc(ptx::smem_u32(&tail->tmem_base), TMEM_COLS);
-    ptx::tmem_relinquish();
+    ptx::tmem_alloc_2sm(ptx::smem_u32(&tail->tmem_base), TMEM_COLS);
+    ptx::tmem_relinquish_2sm();
   } else if (warp == 2) {
-    // segment starts + exclusive scan of m-tiles per slot (warp-shuffle scan, 32 slots a step)
+    // segment starts + exclusive scan of token tiles per slot (warp-shuffle scan, 32 slots a step)
     int carry = 0;
     for (int base = 0; base < E_loc; base += 32) {
       const int e = base + lane;
@@ -115,78 +152,92 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         hi = offsets[e + 1];
         tail->off[e] = lo;
       }
-      const int mt = (hi - lo + BM - 1) / BM;
-      int inc = mt;
+      const int nt = (hi - lo + TN - 1) / TN;
+      int inc = nt;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const int n = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += n;
       }
-      if (e < E_loc) tail->cum[e] = carry + inc - mt;
+      if (e < E_loc) tail->cum[e] = carry + inc - nt;
       carry += __shfl_sync(0xffffffffu, inc, 31);
     }
     if (lane == 0) {
       tail->cum[E_loc] = carry;
       tail->off[E_loc] = offsets[E_loc];
-      tail->total_m_tiles = carry;
+      tail->total_t_tiles = carry;
     }
   }
   ptx::tc_fence_before();
   __syncthreads();
+  ptx::cluster_sync_all();      // the peer's barriers are initialised before anything signals them
   ptx::tc_fence_after();
 
   const uint32_t tmem_base = tail->tmem_base;
-  const int total_tiles = tail->total_m_tiles * NB;
+  const int total_tiles = tail->total_t_tiles * NB;
 
   if (warp == 0) {
-    // ================================================================ TMA producer
+    // ================================================================ TMA producer (both CTAs)
     if (lane == 0) {
-      const uint64_t pol_a = ptx::policy_evict_last();    // activations are re-read by every n-block
-      const uint64_t pol_b = ptx::policy_evict_first();   // each weight byte is needed once (per wave)
+      // Both operands are re-read through L2: an activation tile by every feature block of its
+      // expert, a weight tile by the pairs working on the other token tiles of the same expert.
+      // Those pairs are NOT in lock-step (tile costs differ with the ragged N), so a weight line
+      // must survive a few microseconds: evict_first on the weights doubled the DRAM reads
+      // (measured, profiles/), evict_last keeps them at the algorithmic bytes.
+      const uint64_t pol_act = ptx::policy_evict_last();
+      const uint64_t pol_w = ptx::policy_evict_last();
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        int m_blk, n_blk;
-        cur.decode(tail, tile, NB, m_blk, n_blk);
+      for (int tile = pair; tile < total_tiles; tile += num_pairs) {
+        int f_blk, t_blk;
+        cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
-        const int row0 = tail->off[e] + m_blk * BM;
-        const int n0 = n_blk * BN_OUT;
+        const int row0 = tail->off[e] + t_blk * TN;
+        const int n_rows = min(TN, tail->off[e + 1] - row0);
+        const int half = ((n_rows + 15) >> 4) << 3;          // UMMA N / 2: this CTA's share of the columns
+        const int row_b = row0 + (int)rank * half;
+        const int n0 = f_blk * FB + (int)rank * FC;
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
-          const uint32_t full = ptx::smem_u32(&tail->full[stage]);
-          ptx::mbar_arrive_expect_tx(full, STAGE_BYTES);
+          const uint32_t full_local = ptx::smem_u32(&tail->full[stage]);
+          if (rank == 0) ptx::mbar_arrive_expect_tx(full_local, 2 * STAGE_BYTES);
+          const uint32_t full = ptx::mapa_u32(full_local, 0);   // the leader's barrier
           const uint32_t a_s = ptx::smem_u32(smem + (size_t)stage * STAGE_BYTES);
           const uint32_t b_s = a_s + A_BYTES;
           const int k0 = kb * BK;
-          ptx::tma_load_2d(a_s, &tmA, full, k0, row0, pol_a);
           if (kGateUp) {
-            ptx::tma_load_3d(b_s + 0 * B_ATOM_BYTES, &tmB0, full, n0, k0, e, pol_b);
-            ptx::tma_load_3d(b_s + 1 * B_ATOM_BYTES, &tmB0, full, n0 + 64, k0, e, pol_b);
-            ptx::tma_load_3d(b_s + 2 * B_ATOM_BYTES, &tmB1, full, n0, k0, e, pol_b);
-            ptx::tma_load_3d(b_s + 3 * B_ATOM_BYTES, &tmB1, full, n0 + 64, k0, e, pol_b);
+            ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);                 // gate -> lanes 0..63
+            ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, n0, k0, e, pol_w);    // up   -> lanes 64..127
           } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              ptx::tma_load_3d(b_s + j * B_ATOM_BYTES, &tmB0, full, n0 + 64 * j, k0, e, pol_b);
+            ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);
+            ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, n0 + 64, k0, e, pol_w);
           }
+          ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
-    // ================================================================ UMMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc = ptx::make_idesc_bf16_f32(BM, UMMA_N, /*a_mn=*/false, /*b_mn=*/true);
+    // ================================================================ UMMA issuer (leader CTA)
+    if (rank == 0 && lane == 0) {
+      constexpr uint32_t idesc0 = ptx::make_idesc_bf16_f32(256, 0, /*a_mn=*/true, /*b_mn=*/false);
+      TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
+      for (int tile = pair; tile < total_tiles; tile += num_pairs, ++it) {
+        int f_blk, t_blk;
+        cur.decode(tail, tile, NB, f_blk, t_blk);
+        const int e = cur.e;
+        const int n_rows = min(TN, tail->off[e + 1] - (tail->off[e] + t_blk * TN));
+        const uint32_t n_mma = (uint32_t)((n_rows + 15) >> 4) << 4;
+        const uint32_t idesc = idesc0 | ((n_mma >> 3) << 17);
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&tail->tempty[acc]), acc_phase ^ 1u);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)acc * UMMA_N;
+        const uint32_t d_tmem = tmem_base + (uint32_t)acc * TN;
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->full[stage]), phase);
           ptx::tc_fence_after();
@@ -194,91 +245,89 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           const uint32_t b_s = a_s + A_BYTES;
 #pragma unroll
           for (int k = 0; k < BK / UMMA_K; ++k) {
-            // A: K-major SW128 -> advance 16 elements = 32 bytes inside the 128-byte row
-            const uint64_t da = ptx::make_smem_desc_sw128(a_s + k * (UMMA_K * 2), 16, 1024);
-            // B: MN-major SW128 -> 16 K-rows = 2 swizzle atoms of 1024 B; next 64 N-columns at LBO
-            const uint64_t db = ptx::make_smem_desc_sw128(b_s + k * (UMMA_K * 128), B_ATOM_BYTES, 1024);
-            ptx::umma_bf16(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
+            // A: MN-major SW128 -> 16 K-rows = 2 swizzle atoms of 1024 B; next 64 features at LBO
+            const uint64_t da = ptx::make_smem_desc_sw128(a_s + k * (UMMA_K * 128), ATOM_BYTES, 1024);
+            // B: K-major SW128 -> advance 16 elements = 32 bytes inside the 128-byte row
+            const uint64_t db = ptx::make_smem_desc_sw128(b_s + k * (UMMA_K * 2), 16, 1024);
+            ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
           }
-          ptx::umma_commit(ptx::smem_u32(&tail->empty[stage]));   // frees the smem stage when MMAs retire
+          ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
-        ptx::umma_commit(ptx::smem_u32(&tail->tfull[acc]));       // accumulator ready for the epilogue
+        ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->tfull[acc]), 3);       // accumulator ready in both CTAs
       }
     }
   } else {
-    // ================================================================ epilogue (warps 2..5)
+    // ================================================================ epilogue (warps 2..5, both CTAs)
     const int q = warp & 3;  // TMEM lane quarter this warp may access
     TileCursor cur;
     int it = 0;
-    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
-      int m_blk, n_blk;
-      cur.decode(tail, tile, NB, m_blk, n_blk);
+    for (int tile = pair; tile < total_tiles; tile += num_pairs, ++it) {
+      int f_blk, t_blk;
+      cur.decode(tail, tile, NB, f_blk, t_blk);
       const int e = cur.e;
-      const int seg_end = tail->off[e + 1];
-      const int grow = tail->off[e] + m_blk * BM + q * 32 + lane;
-      const bool row_ok = grow < seg_end;
-      const int n0 = n_blk * BN_OUT;
+      const int row0 = tail->off[e] + t_blk * TN;
+      const int n_rows = min(TN, tail->off[e + 1] - row0);
       const int acc = it & 1;
       const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * UMMA_N;
-      __nv_bfloat16* orow = out + (size_t)grow * ld_out + n0;
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
       if (kGateUp) {
-#pragma unroll 1
-        for (int c = 0; c < 4; ++c) {
-          uint32_t g[32], u[32];
-          ptx::tmem_ld_32x32(taddr + c * 32, g);
-          ptx::tmem_ld_32x32(taddr + 128 + c * 32, u);
+        // lanes 0..63 gate (q = 0,1), lanes 64..127 up (q = 2,3) of the same 64 features.
+        // Per 64 columns: the gate warp finishes columns 0..31 (needs the partner's up block),
+        // the up warp finishes columns 32..63 (needs the partner's gate block).
+        const bool is_up = q >= 2;
+        const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
+        const bool feat_ok = feat < n_total;
+        float* mine = xchg + ((q & 1) * 2 + (is_up ? 1 : 0)) * 1024;      // block I publish  [col][lane]
+        float* theirs = xchg + ((q & 1) * 2 + (is_up ? 0 : 1)) * 1024;    // block my partner publishes
+        const uint32_t bar_id = 1 + (q & 1);
+        for (int c0 = 0; c0 < n_rows; c0 += 64) {
+          uint32_t a[32], b[32];
+          ptx::tmem_ld_32x32(taddr + c0, a);
+          ptx::tmem_ld_32x32(taddr + c0 + 32, b);
           ptx::tmem_ld_wait();
-          uint32_t h[16];
+          // publish the block the partner finishes: gate warp -> its gate of cols 32..63; up warp -> its up of cols 0..31
 #pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const float g0 = __uint_as_float(g[2 * i]), g1 = __uint_as_float(g[2 * i + 1]);
-            const float u0 = __uint_as_float(u[2 * i]), u1 = __uint_as_float(u[2 * i + 1]);
-            const float h0 = __fdividef(g0, 1.0f + __expf(-g0)) * u0;
-            const float h1 = __fdividef(g1, 1.0f + __expf(-g1)) * u1;
-            h[i] = pack2_bf16(h0, h1);
-          }
-          if (row_ok && n0 + c * 32 < n_total) {
-            uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
+          for (int i = 0; i < 32; ++i) mine[i * 32 + lane] = __uint_as_float(is_up ? a[i] : b[i]);
+          ptx::named_bar_sync(bar_id, 64);
+          float h[32];
 #pragma unroll
-            for (int v = 0; v < 4; ++v) dst[v] = make_uint4(h[4 * v], h[4 * v + 1], h[4 * v + 2], h[4 * v + 3]);
+          for (int i = 0; i < 32; ++i) {
+            const float o = theirs[i * 32 + lane];
+            h[i] = is_up ? swiglu(o, __uint_as_float(b[i])) : swiglu(__uint_as_float(a[i]), o);
           }
+          ptx::named_bar_sync(bar_id, 64);     // both blocks consumed before the next publish
+          const int cbase = c0 + (is_up ? 32 : 0);
+          store_block_T(h, out, (size_t)ld_out, row0 + cbase, n_rows - cbase, feat, feat_ok, lane);
         }
       } else {
-#pragma unroll 1
-        for (int c = 0; c < 8; ++c) {
+        const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
+        const bool feat_ok = feat < n_total;
+        for (int c0 = 0; c0 < n_rows; c0 += 32) {
           uint32_t a[32];
-          ptx::tmem_ld_32x32(taddr + c * 32, a);
+          ptx::tmem_ld_32x32(taddr + c0, a);
           ptx::tmem_ld_wait();
-          if (row_ok && n0 + c * 32 < n_total) {
-            uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
+          float v[32];
 #pragma unroll
-            for (int v = 0; v < 4; ++v) {
-              uint4 o;
-              o.x = pack2_bf16(__uint_as_float(a[8 * v + 0]), __uint_as_float(a[8 * v + 1]));
-              o.y = pack2_bf16(__uint_as_float(a[8 * v + 2]), __uint_as_float(a[8 * v + 3]));
-              o.z = pack2_bf16(__uint_as_float(a[8 * v + 4]), __uint_as_float(a[8 * v + 5]));
-              o.w = pack2_bf16(__uint_as_float(a[8 * v + 6]), __uint_as_float(a[8 * v + 7]));
-              dst[v] = o;
-            }
-          }
+          for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]);
+          store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
         }
       }
       ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(ptx::smem_u32(&tail->tempty[acc]));
+      if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa_u32(ptx::smem_u32(&tail->tempty[acc]), 0));
     }
   }
 
   // ------------------------------------------------------------------ teardown
   ptx::tc_fence_before();
   __syncthreads();
+  ptx::cluster_sync_all();      // neither CTA frees TMEM / exits while the peer still uses the pair
   if (warp == 1) {
     ptx::tc_fence_after();
-    ptx::tmem_dealloc(tmem_base, TMEM_COLS);
+    ptx::tmem_dealloc_2sm(tmem_base, TMEM_COLS);
   }
 }
 
@@ -367,8 +416,8 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
                              cudaStream_t st) {
   CUtensorMap tmX, tmH, tmW1, tmW3, tmW2;
   vibe_status s;
-  if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, BM, &tmX)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, BM, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W1, f, d, E_loc, 64, BK, &tmW1)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W3, f, d, E_loc, 64, BK, &tmW3)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W2, d, f, E_loc, 64, BK, &tmW2)) != VIBE_OK) return s;
@@ -383,7 +432,7 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   });
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
-  const int grid = num_sms();
+  const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
   ffn_gemm_kernel<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
                                                                reinterpret_cast<__nv_bfloat16*>(H_ws), f);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");

@@ -240,16 +240,43 @@ def test_ffn_c0_tiny():
 
 
 @pytest.mark.parametrize("T,E,k,d,f,align", [
-    (700, 4, 2, 256, 384, 1),      # several 128-row tiles per expert + ragged tails
+    (700, 4, 2, 256, 384, 1),      # several token tiles per expert + ragged tails
     (700, 4, 2, 256, 384, 128),    # tile-aligned segments (zero padding rows)
     (300, 8, 2, 320, 320, 1),      # partial N tiles in both GEMMs (f%128=64, d%256=64)
     (50, 16, 4, 64, 64, 1),        # smallest legal d,f; segments far below one tile
-    (1024, 2, 1, 512, 1024, 1),    # long K loop wraps the 4-stage ring many times
+    (1024, 2, 1, 512, 1024, 1),    # long K loop wraps the smem stage ring many times
     (129, 1, 1, 128, 128, 1),      # one expert, 128+1 rows
 ])
 def test_ffn_tiles_and_tails(T, E, k, d, f, align):
     cfg = I.LayerConfig("case", T=T, d=d, f=f, E=E, k=k, E_loc=E, zipf_s=1.0)
     check_ffn(cfg, T + d, align)
+
+
+@pytest.mark.parametrize("rows,d,f", [
+    ([1, 15, 16, 17, 0, 31, 33, 255], 128, 256),          # every N granule edge of the swap-AB tile (N = roundup(n,16))
+    ([256, 257, 511, 513, 0, 0, 2, 768], 256, 128),       # full token tiles + 1-row / 255-row tails, empty slots
+    ([3] * 70 + [0] * 30 + [40] * 28, 64, 192),           # 128 slots: the slot scan spans several 32-lane steps
+])
+def test_ffn_ragged_token_tiles(rows, d, f):
+    """Segment lengths chosen around the UMMA-N granule (16), the CTA-pair split (N/2) and the
+    256-token tile edge; every slot has its own weights so a wrong tile->slot decode shows."""
+    E = len(rows)
+    off = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    R = int(off[-1])
+    Xp = I.make_X(R, d, 77)
+    W1, W3, W2 = I.make_weights(E, d, f, 78)
+    r2a = np.arange(R, dtype=np.int32)
+    Xp_d = torch.full((R + 300, d), float("nan"), dtype=torch.bfloat16, device="cuda")   # poison past the end
+    Xp_d[:R] = dev_bf16(Xp)
+    Y, H = B.grouped_ffn(Xp_d, dev(off), dev_bf16(W1), dev_bf16(W3), dev_bf16(W2))
+    torch.cuda.synchronize()
+    Y_ref, H_ref = O.grouped_ffn(Xp, off, r2a, W1, W3, W2, round_h=True, round_y=False)
+    Yg = O.bf16_bits_to_f64(host_bits(Y)[:R])
+    Hg = O.bf16_bits_to_f64(host_bits(H)[:R])
+    mh = O.ffn_error_metrics(Hg, H_ref)
+    my = O.ffn_error_metrics(Yg, Y_ref)
+    assert np.all(np.abs(Hg - H_ref) <= 2.0 ** -7 * np.abs(H_ref) + 1e-3 * mh["rms_ref"]), ("H", mh)
+    assert my["max_abs_err_over_rms"] <= FFN_MAX and my["mean_rel_err"] <= FFN_MEAN, ("Y", my)
 
 
 def test_ffn_partial_residency_empty_experts_and_many_tiles():
