@@ -11,7 +11,7 @@ and, where the paper is silent (it treats the fused MoE kernel as a black box,
 PAPER.md L176/L220/L420), from the readings listed in DESIGN.md ("Readings").
 No blocking, no fusion, no reordering beyond the definitions.
 
-Citations:  P:L<n> = /root/reference/PAPER.md line n;  R*/P*/F*/C*/M*/L* = DESIGN.md reading ids.
+Citations:  P:L<n> = /root/reference/PAPER.md line n;  R*/P*/F*/C*/M*/L* = DESIGN.md reading ids (D* = the f1 recalibration readings).
 
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): every function below is pinned to
 something other than itself -- brute force, closed forms, library routines
@@ -472,6 +472,121 @@ def placement_brute_force(load, G, scale, model, model_kind=MODEL_B, cap=0):
         if sc < best_score:
             best_score, best_assign = sc, np.array(a, dtype=np.int32)
     return best_score, best_assign
+
+
+# ======================================================================================
+# O9  drift detector (f1):  d = 1 - (w . w_ref) / (|w| |w_ref|)
+#     "Every H forward passes (default H=10) ... cosine distance between the current
+#     100-sample window average w and the reference ... When any layer's d exceeds a
+#     threshold delta_cos (default 0.05) ... triggers the incremental solver";
+#     Alg. 1 Phase 3: snapshot := current w at a rearrangement, then
+#     "Cooldown for H forward passes".  Readings D1, D3.
+# ======================================================================================
+
+def cosine_distance(w, w_ref):
+    w = np.asarray(w, dtype=np.float64)
+    r = np.asarray(w_ref, dtype=np.float64)
+    dot = 0.0
+    nw = 0.0
+    nr = 0.0
+    for e in range(len(w)):
+        dot += w[e] * r[e]
+        nw += w[e] * w[e]
+        nr += r[e] * r[e]
+    if nw == 0.0 or nr == 0.0:
+        return 0.0                                    # D1: a zero vector carries no direction
+    return 1.0 - dot / (np.sqrt(nw) * np.sqrt(nr))
+
+
+class DriftMonitor:
+    """Alg. 1 Phase 3 bookkeeping for L layers x E experts (D3): a sliding window of the last
+    `window` per-pass load vectors; every H-th pass, if a reference exists and no cooldown is
+    running, d_l = cosine_distance(window mean_l, reference_l); trigger iff max_l d_l > delta."""
+
+    def __init__(self, L, E, window=100, H=10, delta=0.05):
+        self.L, self.E, self.window, self.H, self.delta = L, E, window, H, delta
+        self.samples = []          # most recent `window` pushes, each [L,E]
+        self.ref = None
+        self.passes = 0
+        self.cooldown = 0
+
+    def window_mean(self):
+        acc = np.zeros((self.L, self.E), dtype=np.float64)
+        for s in self.samples:
+            acc += s
+        return acc / max(1, len(self.samples))
+
+    def set_reference(self, W):
+        self.ref = np.array(W, dtype=np.float64).reshape(self.L, self.E)
+
+    def rearranged(self):
+        """'w_ref <- w for all l; Cooldown for H forward passes' (P:L460-L462)."""
+        self.ref = self.window_mean()
+        self.cooldown = self.H
+
+    def push(self, loads):
+        """One forward pass.  Returns (triggered, d[L] or None when no check ran)."""
+        self.samples.append(np.array(loads, dtype=np.float64).reshape(self.L, self.E))
+        if len(self.samples) > self.window:
+            self.samples.pop(0)
+        self.passes += 1
+        if self.cooldown > 0:
+            self.cooldown -= 1
+            return False, None
+        if self.ref is None or self.passes % self.H != 0:
+            return False, None
+        w = self.window_mean()
+        d = np.array([cosine_distance(w[l], self.ref[l]) for l in range(self.L)])
+        return bool(d.max() > self.delta), d
+
+
+# ======================================================================================
+# O10  incremental placement update (f1): Algorithm 2 (P:L465-L472; prose P:L210-L214, L426-L428)
+#     repeat: g+ = slowest GPU, g- = fastest GPU; best swap (e_i in g+, e_j in g-) "maximizing
+#     latency reduction"; swap; until max_g f_g(n_g) <= (1+eps) * mean_g f_g(n_g) "or no
+#     latency reduction".  Reading D2: the reduction of a swap is max(L_g+, L_g-) before minus
+#     after; ties -> lowest (e_i, e_j); argmax/argmin ties -> lower g.
+# ======================================================================================
+
+def bin_latencies(assign, load, G, scale, model, model_kind):
+    return placement_eval(assign, load, G, scale, model, model_kind)[1]
+
+
+def placement_swap_refine(assign, load, G, scale, model, model_kind=MODEL_B, eps=0.03, max_swaps=1 << 30):
+    """Returns (assign', swaps) with swaps = [(e_i, e_j), ...] in the order applied."""
+    assign = np.array(assign, dtype=np.int32)
+    load = np.asarray(load, dtype=np.float64)
+    swaps = []
+    while len(swaps) < max_swaps:
+        Lg = bin_latencies(assign, load, G, scale, model, model_kind)
+        mean = 0.0
+        for g in range(G):
+            mean += Lg[g]
+        mean /= G
+        g_hi = int(np.argmax(Lg))          # first maximum: ties -> lower g
+        g_lo = int(np.argmin(Lg))
+        if Lg[g_hi] <= (1.0 + eps) * mean or g_hi == g_lo:
+            break
+        before = max(Lg[g_hi], Lg[g_lo])
+        best, best_red = None, 0.0
+        for ei in range(len(load)):
+            if assign[ei] != g_hi:
+                continue
+            for ej in range(len(load)):
+                if assign[ej] != g_lo:
+                    continue
+                trial = assign.copy()
+                trial[ei], trial[ej] = g_lo, g_hi
+                Lt = bin_latencies(trial, load, G, scale, model, model_kind)
+                red = before - max(Lt[g_hi], Lt[g_lo])
+                if red > best_red:                     # strict: ties -> first (lowest e_i, then e_j)
+                    best, best_red = (ei, ej), red
+        if best is None:
+            break                                      # "no latency reduction"
+        ei, ej = best
+        assign[ei], assign[ej] = g_lo, g_hi
+        swaps.append(best)
+    return assign, swaps
 
 
 # ======================================================================================
