@@ -255,6 +255,51 @@ VIBE_API vibe_status vibe_placement_token_balanced(const double* load, int32_t E
 /* vLLM's contiguous default: e -> floor(e*G/E). */
 VIBE_API vibe_status vibe_placement_contiguous(int32_t E, int32_t G, int32_t* assign);
 
+/* ====================================================================================
+ * f1.  Online recalibration (host, fp64): drift detector and incremental placement update.
+ * ==================================================================================== */
+
+/* d = 1 - (w . w_ref) / (|w| |w_ref|)  -- the cosine distance between the current window
+ * average and the reference load vector of one layer.  A zero vector gives 0
+ * (reading D1).  Returns a negative value on invalid arguments. */
+VIBE_API double vibe_drift_cosine(const double* w, const double* w_ref, int32_t E);
+
+/* Algorithm 1 phase 3 bookkeeping (reading D3) for L layers x E
+ * experts: a sliding window of the last `window` per-pass load vectors (paper: 100); every
+ * H-th pass (paper: 10), if a reference exists and no cooldown is running, the per-layer
+ * distances between the window mean and the reference are computed; recalibration is
+ * triggered when any exceeds delta (paper: 0.05).  The library owns the monitor object
+ * (create / destroy); all arrays are HOST, row-major [L,E]. */
+typedef struct vibe_drift_monitor vibe_drift_monitor;
+VIBE_API vibe_drift_monitor* vibe_drift_monitor_create(int32_t L, int32_t E, int32_t window, int32_t H,
+                                                       double delta); /* NULL on error */
+VIBE_API void vibe_drift_monitor_destroy(vibe_drift_monitor* m);
+/* "Snapshot w_ref <- current load vectors": explicit reference, e.g. the profiling W. */
+VIBE_API vibe_status vibe_drift_monitor_set_reference(vibe_drift_monitor* m, const double* W);
+/* One forward pass.  Returns 1 if recalibration is triggered on this pass, 0 if not, -1 on
+ * error.  *checked (optional) = 1 when distances were computed on this pass, and then
+ * d_out[L] (optional) holds them. */
+VIBE_API int32_t vibe_drift_monitor_push(vibe_drift_monitor* m, const double* loads, double* d_out,
+                                         int32_t* checked);
+/* After a rearrangement: "w_ref <- w for all l; cooldown for H forward passes". */
+VIBE_API vibe_status vibe_drift_monitor_rearranged(vibe_drift_monitor* m);
+VIBE_API vibe_status vibe_drift_monitor_window_mean(const vibe_drift_monitor* m, double* W);
+
+/* Algorithm 2 (prose P:L210-L214, L426-L428), one layer, in place on assign[E]:
+ *   repeat  g+ = slowest bin, g- = fastest bin (ties -> lower g);
+ *           stop if max_g L_g <= (1+eps) * mean_g L_g;
+ *           over all (e_i in g+, e_j in g-) take the swap with the largest reduction of
+ *           max(L_g+, L_g-) (reading D2; ties -> lowest (e_i, e_j)); stop if none reduces it;
+ *           apply the swap;
+ *   until max_swaps swaps were applied.
+ * L_g as in vibe_placement_eval (model kind A or B, scale = sigma_g).  Per-bin expert counts
+ * are preserved.  n_swaps (optional) receives the number applied; swaps (optional, capacity
+ * 2*max_swaps) the pairs (e_i, e_j) in order. */
+VIBE_API vibe_status vibe_placement_swap_refine(int32_t* assign, const double* load, int32_t E, int32_t G,
+                                                const double* scale, const vibe_latency_model* m,
+                                                int32_t model_kind, double eps, int32_t max_swaps,
+                                                int32_t* n_swaps, int32_t* swaps);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,7 +5,8 @@ for device memory and streams only.  Names mirror the C ABI:
 
     route_topk, permute, grouped_ffn, combine, profile_expert_latency,
     moe_layer_forward, moe_layer_forward_host,
-    placement_eval, placement_greedy, placement_token_balanced, placement_contiguous
+    placement_eval, placement_greedy, placement_token_balanced, placement_contiguous,
+    drift_cosine, DriftMonitor, placement_swap_refine
 
 There is NO fallback: if libvibe.so is missing or a call fails, a VibeError is raised.
 """
@@ -34,6 +35,9 @@ EXPORTED_SYMBOLS = (
     "vibe_moe_layer_forward", "vibe_moe_layer_forward_host", "vibe_workspace_bytes", "vibe_rows_cap",
     "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
+    "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
+    "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
+    "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
 )
 
 
@@ -116,9 +120,24 @@ def load() -> C.CDLL:
     lib.vibe_placement_greedy.argtypes = [dp, i32, i32, dp, C.POINTER(_LatencyModel), i32, C.POINTER(i32)]
     lib.vibe_placement_token_balanced.argtypes = [dp, i32, i32, i32, C.POINTER(i32)]
     lib.vibe_placement_contiguous.argtypes = [i32, i32, C.POINTER(i32)]
+    lib.vibe_drift_cosine.argtypes = [dp, dp, i32]
+    lib.vibe_drift_cosine.restype = C.c_double
+    lib.vibe_drift_monitor_create.argtypes = [i32, i32, i32, i32, C.c_double]
+    lib.vibe_drift_monitor_create.restype = vp
+    lib.vibe_drift_monitor_destroy.argtypes = [vp]
+    lib.vibe_drift_monitor_destroy.restype = None
+    lib.vibe_drift_monitor_set_reference.argtypes = [vp, dp]
+    lib.vibe_drift_monitor_push.argtypes = [vp, dp, dp, C.POINTER(i32)]
+    lib.vibe_drift_monitor_push.restype = i32
+    lib.vibe_drift_monitor_rearranged.argtypes = [vp]
+    lib.vibe_drift_monitor_window_mean.argtypes = [vp, dp]
+    lib.vibe_placement_swap_refine.argtypes = [C.POINTER(i32), dp, i32, i32, dp, C.POINTER(_LatencyModel), i32,
+                                               C.c_double, i32, C.POINTER(i32), C.POINTER(i32)]
     for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine",
                  "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
-                 "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous"):
+                 "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
+                 "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
+                 "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -368,3 +387,74 @@ def placement_contiguous(E: int, G: int):
     out = np.empty(E, dtype=np.int32)
     _ok(lib.vibe_placement_contiguous(E, G, out.ctypes.data_as(C.POINTER(C.c_int32))), "vibe_placement_contiguous")
     return out
+
+
+# ------------------------------------------------------------------------------------ f1: recalibration (host)
+def drift_cosine(w, w_ref) -> float:
+    lib = load()
+    a, ap = _dp(w)
+    b, bp = _dp(w_ref)
+    if len(a) != len(b):
+        raise VibeError("drift_cosine: length mismatch")
+    v = lib.vibe_drift_cosine(ap, bp, len(a))
+    if v < -0.5:
+        raise VibeError("vibe_drift_cosine: " + lib.vibe_last_error().decode())
+    return float(v)
+
+
+class DriftMonitor:
+    """Handle on a library-owned vibe_drift_monitor (Alg. 1 phase 3)."""
+
+    def __init__(self, L: int, E: int, window: int = 100, H: int = 10, delta: float = 0.05):
+        self._lib = load()
+        self.L, self.E = L, E
+        self._h = self._lib.vibe_drift_monitor_create(L, E, window, H, delta)
+        if not self._h:
+            raise VibeError("vibe_drift_monitor_create: " + self._lib.vibe_last_error().decode())
+
+    def close(self):
+        if self._h:
+            self._lib.vibe_drift_monitor_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def set_reference(self, W):
+        a, ap = _dp(np.asarray(W, dtype=np.float64).reshape(self.L * self.E))
+        _ok(self._lib.vibe_drift_monitor_set_reference(self._h, ap), "vibe_drift_monitor_set_reference")
+
+    def push(self, loads):
+        """-> (triggered, d[L] or None when no check ran on this pass)"""
+        a, ap = _dp(np.asarray(loads, dtype=np.float64).reshape(self.L * self.E))
+        d = np.zeros(self.L, dtype=np.float64)
+        chk = C.c_int32(0)
+        r = self._lib.vibe_drift_monitor_push(self._h, ap, d.ctypes.data_as(C.POINTER(C.c_double)), C.byref(chk))
+        if r < 0:
+            raise VibeError("vibe_drift_monitor_push: " + self._lib.vibe_last_error().decode())
+        return bool(r), (d if chk.value else None)
+
+    def rearranged(self):
+        _ok(self._lib.vibe_drift_monitor_rearranged(self._h), "vibe_drift_monitor_rearranged")
+
+    def window_mean(self):
+        W = np.zeros(self.L * self.E, dtype=np.float64)
+        _ok(self._lib.vibe_drift_monitor_window_mean(self._h, W.ctypes.data_as(C.POINTER(C.c_double))),
+            "vibe_drift_monitor_window_mean")
+        return W.reshape(self.L, self.E)
+
+
+def placement_swap_refine(assign, load_, G: int, scale, model: Optional[LatencyModel], model_kind: int = MODEL_B,
+                          eps: float = 0.03, max_swaps: int = 1 << 20):
+    """Algorithm 2 on one layer -> (assign', [(e_i, e_j), ...])"""
+    lib = load()
+    a = np.array(assign, dtype=np.int32)
+    ld, ldp = _dp(load_)
+    sc, scp = _dp(scale)
+    mref, keep = _model(model)
+    cap = int(min(max_swaps, 1 << 20))
+    n = C.c_int32(0)
+    sw = np.zeros(2 * max(cap, 1), dtype=np.int32)
+    _ok(lib.vibe_placement_swap_refine(a.ctypes.data_as(C.POINTER(C.c_int32)), ldp, len(ld), G, scp, mref, model_kind,
+                                       eps, cap, C.byref(n), sw.ctypes.data_as(C.POINTER(C.c_int32))),
+        "vibe_placement_swap_refine")
+    return a, [(int(sw[2 * i]), int(sw[2 * i + 1])) for i in range(n.value)]

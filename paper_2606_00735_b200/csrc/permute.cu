@@ -1,244 +1,250 @@
 // permute.cu -- a3: stable counting sort of assignments by local expert slot + row gather
 // (vibe_permute).  Semantics: include/vibe.h, readings P1-P4.
 //
-// Four small launches on one stream, no host sync, no spin-waits between CTAs:
-//   K1 perm_hist     : every warp owns a contiguous chunk of kChunk assignments and writes
-//                      its per-slot histogram (slot-major layout [E_loc][NW]).
-//   K2 perm_scan     : one CTA per slot: exclusive scan over the NW chunk counts (in place)
-//                      and the slot total.
-//   K3 perm_index    : every CTA rebuilds offsets[] from the totals (<= 1024 slots, a block
-//                      scan), every warp re-walks its chunk IN ORDER and ranks each
-//                      assignment with match.any + a per-warp running counter in shared
-//                      memory => rows inside a slot are in ascending flat index (stable,
-//                      bit-exact w.r.t. the counting-sort definition).  Writes
-//                      assign_to_row / row_to_assign; zero-fills padding rows.
-//   K4 perm_rows     : token-major gather/scatter of the bf16 rows, one thread per 16-byte vector:
-//                      X[t,:] is read ONCE and written to each of its <= k destination rows,
-//                      so DRAM traffic equals the algorithmic 2*T_res*d + 2*R*d bytes.
-//                      (E_loc < E: the row-major variant perm_rows_by_row, work ~ R.)
+// Two launches on one stream, no host sync, no spin-waits between CTAs.  The batch is cut
+// into NB chunks of TPC consecutive tokens (= CH = TPC*k consecutive assignments); NB is a
+// few CTAs per SM so that the row copy of K2 fills the machine.
+//   K1 perm_count   : CTA b histograms the slots of chunk b into hist[b][*].  The LAST CTA to
+//                     finish (a ticket counter; no CTA ever waits for another) turns the
+//                     table into per-slot exclusive prefixes over the chunks, and writes the
+//                     slot totals and offsets[] (aligned exclusive scan of the totals).
+//   K2 perm_scatter : CTA b ranks the assignments of chunk b IN ORDER (warp 0: match.any + a
+//                     running counter per slot that starts at offsets[s] + hist[b][s]) => rows
+//                     inside a slot are in ascending flat index (stable, bit-exact w.r.t. the
+//                     counting-sort definition); writes assign_to_row / row_to_assign; then
+//                     copies its TPC token rows: X[t,:] is read ONCE (16-byte vectors, the
+//                     loads are issued before the ranking finishes) and stored to each of its
+//                     <= k destination rows, so DRAM traffic is the algorithmic
+//                     2*T_res*d + 2*R*d bytes.  Padding rows (align > 1) are zero-filled.
+#include <atomic>
+
 #include "common.cuh"
 
 namespace vibe {
 namespace {
 
-constexpr int kChunk = 256;          // assignments per warp
-constexpr int kWarpsPerBlock = 8;    // K1/K3 block = 256 threads
 constexpr int kMaxSlots = 1024;
+constexpr int kMaxChunk = 1024;      // assignments per chunk (CH = TPC*k)
+constexpr int kTargetChunks = 592;   // ~4 CTAs per SM
+constexpr int kTickets = 64;
+
+// Ticket counters of K1 (one per in-flight call, round-robin): zero at module load, and the
+// last CTA of every call puts its counter back to zero.
+__device__ unsigned int g_tickets[kTickets];
 
 __device__ __forceinline__ int slot_of(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int i,
                                        int E, int E_loc) {
-  const int e = ids[i];
+  const int e = __ldg(ids + i);
   if (e < 0 || e >= E) return -1;
-  const int s = emap ? emap[e] : e;
+  const int s = emap ? __ldg(emap + e) : e;
   return (s >= 0 && s < E_loc) ? s : -1;
 }
 
 // K1 ------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) perm_hist_kernel(const int32_t* __restrict__ ids,
-                                                        const int32_t* __restrict__ emap, int A, int E, int E_loc,
-                                                        int NW, int32_t* __restrict__ hist /*[E_loc][NW]*/) {
-  extern __shared__ int s_cnt[];  // [kWarpsPerBlock][E_loc]
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int c = blockIdx.x * kWarpsPerBlock + warp;
-  int* cnt = s_cnt + warp * E_loc;
-  for (int s = lane; s < E_loc; s += 32) cnt[s] = 0;
-  __syncwarp();
-  if (c < NW) {
-    const int lo = c * kChunk, hi = min(A, lo + kChunk);
-    for (int i = lo + lane; i < hi; i += 32) {
-      const int s = slot_of(ids, emap, i, E, E_loc);
-      if (s >= 0) atomicAdd(&cnt[s], 1);
+__global__ void __launch_bounds__(1024) perm_count_kernel(const int32_t* __restrict__ ids,
+                                                          const int32_t* __restrict__ emap, int A, int E, int E_loc,
+                                                          int CH, int NB, int align, int ticket,
+                                                          int32_t* __restrict__ hist /*[NB][E_loc]*/,
+                                                          int32_t* __restrict__ totals /*[E_loc]*/,
+                                                          int32_t* __restrict__ offsets /*[E_loc+1]*/) {
+  __shared__ int s_cnt[kMaxSlots];
+  __shared__ int s_part[1024];
+  __shared__ int s_last;
+  const int tid = threadIdx.x;
+  for (int s = tid; s < E_loc; s += 1024) s_cnt[s] = 0;
+  __syncthreads();
+  const int lo = blockIdx.x * CH, hi = min(A, lo + CH);
+  for (int i = lo + tid; i < hi; i += 1024) {
+    const int s = slot_of(ids, emap, i, E, E_loc);
+    if (s >= 0) atomicAdd(&s_cnt[s], 1);
+  }
+  __syncthreads();
+  int32_t* row = hist + (size_t)blockIdx.x * E_loc;
+  for (int s = tid; s < E_loc; s += 1024) row[s] = s_cnt[s];
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(&g_tickets[ticket], 1u) == (unsigned)(NB - 1));
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (tid == 0) g_tickets[ticket] = 0;
+
+  // ---- last CTA: hist[b][s] <- sum_{b' < b} hist[b'][s]; totals; offsets ----
+  // Threads form G groups of W = min(E_loc, 1024) slot columns; group g owns the chunk rows
+  // [g*RPG, (g+1)*RPG).  Pass 1: group sums; exclusive scan over the groups; pass 2: rewrite.
+  for (int s0 = 0; s0 < E_loc; s0 += 1024) {
+    const int W = min(E_loc - s0, 1024);
+    const int G = 1024 / W;
+    const int g = tid / W, c = tid - g * W;
+    const bool act = g < G;
+    const int RPG = (NB + G - 1) / G;
+    const int b0 = min(NB, g * RPG), b1 = min(NB, b0 + RPG);
+    volatile int32_t* col = hist + s0 + c;
+    int sum = 0;
+    if (act)
+      for (int b = b0; b < b1; ++b) sum += col[(size_t)b * E_loc];
+    s_part[tid] = act ? sum : 0;
+    __syncthreads();
+    int base = 0;
+    if (act)
+      for (int gg = 0; gg < g; ++gg) base += s_part[gg * W + c];
+    if (act && g == G - 1) s_cnt[s0 + c] = base + sum;     // slot total
+    if (act) {
+      int run = base;
+      for (int b = b0; b < b1; ++b) {
+        const int v = col[(size_t)b * E_loc];
+        col[(size_t)b * E_loc] = run;
+        run += v;
+      }
     }
-    __syncwarp();
-    for (int s = lane; s < E_loc; s += 32) hist[(size_t)s * NW + c] = cnt[s];
+    __syncthreads();
+  }
+  // offsets = exclusive scan of roundup(total, align) over <= 1024 slots (one value per thread)
+  {
+    const int lane = tid & 31, warp = tid >> 5;
+    const int tot = (tid < E_loc) ? s_cnt[tid] : 0;
+    const int v = ((tot + align - 1) / align) * align;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int n = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += n;
+    }
+    __syncthreads();
+    if (lane == 31) s_part[warp] = inc;
+    __syncthreads();
+    int woff = 0;
+    for (int w = 0; w < warp; ++w) woff += s_part[w];
+    if (tid < E_loc) {
+      totals[tid] = tot;
+      offsets[tid] = woff + inc - v;
+      if (tid == E_loc - 1) offsets[E_loc] = woff + inc;
+    }
   }
 }
 
 // K2 ------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) perm_scan_kernel(int32_t* __restrict__ hist, int NW,
-                                                        int32_t* __restrict__ totals /*[E_loc]*/) {
-  __shared__ int s_warp[8];
-  __shared__ int s_carry;
-  int32_t* h = hist + (size_t)blockIdx.x * NW;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (threadIdx.x == 0) s_carry = 0;
-  __syncthreads();
-  for (int base = 0; base < NW; base += 256) {
-    const int i = base + threadIdx.x;
-    const int v = (i < NW) ? h[i] : 0;
-    int inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int n = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += n;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    int woff = 0;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) woff += (w < warp) ? s_warp[w] : 0;
-    const int carry = s_carry;
-    if (i < NW) h[i] = carry + woff + inc - v;  // exclusive
-    __syncthreads();
-    if (threadIdx.x == 255) s_carry = carry + woff + inc;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) totals[blockIdx.x] = s_carry;
-}
+template <int UNROLL>
+__global__ void __launch_bounds__(256) perm_scatter_kernel(const __nv_bfloat16* __restrict__ X,
+                                                           const int32_t* __restrict__ ids,
+                                                           const int32_t* __restrict__ emap, int T, int k, int d,
+                                                           int E, int E_loc, int TPC, int align,
+                                                           const int32_t* __restrict__ hist,
+                                                           const int32_t* __restrict__ totals,
+                                                           const int32_t* __restrict__ offsets,
+                                                           int32_t* __restrict__ row_to_assign,
+                                                           int32_t* __restrict__ assign_to_row,
+                                                           __nv_bfloat16* __restrict__ Xp) {
+  __shared__ int s_run[kMaxSlots];     // next row of every slot for this chunk
+  __shared__ int s_dest[kMaxChunk];    // slot, then destination row, of every assignment of the chunk
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int b = blockIdx.x;
+  const int t0 = b * TPC, t1 = min(T, t0 + TPC);
+  const int lo = t0 * k, n_asg = (t1 - t0) * k;
+  const int vpr = d >> 3;
 
-// K3 ------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) perm_index_kernel(const int32_t* __restrict__ ids,
-                                                         const int32_t* __restrict__ emap, int A, int E, int E_loc,
-                                                         int NW, int align, int d,
-                                                         const int32_t* __restrict__ hist /*exclusive, [E_loc][NW]*/,
-                                                         const int32_t* __restrict__ totals,
-                                                         int32_t* __restrict__ offsets /*[E_loc+1]*/,
-                                                         int32_t* __restrict__ row_to_assign,
-                                                         int32_t* __restrict__ assign_to_row,
-                                                         __nv_bfloat16* __restrict__ Xp) {
-  extern __shared__ int s_mem[];
-  int* s_off = s_mem;                   // [E_loc+1] aligned segment starts
-  int* s_run = s_mem + (E_loc + 1);     // [kWarpsPerBlock][E_loc] running base per warp
-  __shared__ int s_warp[8];
-  __shared__ int s_carry;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  // ---- offsets = exclusive scan of roundup(total, align) (every CTA, redundantly) ----
-  if (threadIdx.x == 0) s_carry = 0;
+  for (int i = tid; i < n_asg; i += 256) s_dest[i] = slot_of(ids, emap, lo + i, E, E_loc);
+  for (int s = tid; s < E_loc; s += 256) s_run[s] = __ldg(offsets + s) + __ldg(hist + (size_t)b * E_loc + s);
   __syncthreads();
-  for (int base = 0; base < E_loc; base += 256) {
-    const int i = base + threadIdx.x;
-    const int v = (i < E_loc) ? ((totals[i] + align - 1) / align) * align : 0;
-    int inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int n = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += n;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    int woff = 0;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) woff += (w < warp) ? s_warp[w] : 0;
-    const int carry = s_carry;
-    if (i < E_loc) s_off[i] = carry + woff + inc - v;
-    __syncthreads();
-    if (threadIdx.x == 255) s_carry = carry + woff + inc;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) s_off[E_loc] = s_carry;
-  __syncthreads();
-  if (blockIdx.x == 0)
-    for (int i = threadIdx.x; i <= E_loc; i += 256) offsets[i] = s_off[i];
 
-  // ---- stable ranks for this warp's chunk ----
-  const int c = blockIdx.x * kWarpsPerBlock + warp;
-  int* run = s_run + warp * E_loc;
-  if (c < NW) {
-    for (int s = lane; s < E_loc; s += 32) run[s] = s_off[s] + hist[(size_t)s * NW + c];
-    __syncwarp();
-    const int lo = c * kChunk, hi = min(A, lo + kChunk);
-    for (int i0 = lo; i0 < hi; i0 += 32) {
+  // ---- first batch of row loads is in flight while warp 0 ranks ----
+  const int n_vec = (t1 - t0) * vpr;     // 16-byte vectors of this chunk's token rows
+  uint4 val[UNROLL];
+  const uint4* src0 = reinterpret_cast<const uint4*>(X + (size_t)t0 * d);
+  bool need[UNROLL];
+#pragma unroll
+  for (int q = 0; q < UNROLL; ++q) {
+    const int v = tid + q * 256;
+    need[q] = false;
+    if (v < n_vec) {
+      const int tt = v / vpr;
+      for (int j = 0; j < k; ++j) need[q] |= (s_dest[tt * k + j] >= 0);
+      if (need[q]) val[q] = ld_nc_v4(src0 + v);
+    }
+  }
+  __syncthreads();   // every thread has read the slots it needs before warp 0 overwrites them
+
+  if (warp == 0) {
+    for (int i0 = 0; i0 < n_asg; i0 += 32) {
       const int i = i0 + lane;
-      const int s = (i < hi) ? slot_of(ids, emap, i, E, E_loc) : -1;
+      const int s = (i < n_asg) ? s_dest[i] : -1;
       const unsigned peers = __match_any_sync(0xffffffffu, s);
       int r = -1;
-      if (s >= 0) {
-        const unsigned lt = peers & ((1u << lane) - 1u);
-        r = run[s] + __popc(lt);
-      }
+      if (s >= 0) r = s_run[s] + __popc(peers & ((1u << lane) - 1u));
       __syncwarp();
-      if (s >= 0 && (peers >> lane) == 1u) run[s] += __popc(peers);  // highest peer lane updates
+      if (s >= 0 && (peers >> lane) == 1u) s_run[s] += __popc(peers);   // highest peer lane updates
       __syncwarp();
-      if (i < hi) {
-        assign_to_row[i] = r;
-        if (r >= 0) row_to_assign[r] = i;
+      if (i < n_asg) {
+        s_dest[i] = r;
+        assign_to_row[lo + i] = r;
+        if (r >= 0) row_to_assign[r] = lo + i;
       }
     }
   }
+  __syncthreads();
+
+  // ---- copy rows: vector v of the chunk = (token v / vpr, vector v % vpr) ----
+  uint4* dst0 = reinterpret_cast<uint4*>(Xp);
+  for (int vb = 0; vb < n_vec; vb += 256 * UNROLL) {
+    if (vb > 0) {
+#pragma unroll
+      for (int q = 0; q < UNROLL; ++q) {
+        const int v = vb + tid + q * 256;
+        need[q] = false;
+        if (v < n_vec) {
+          const int tt = v / vpr;
+          for (int j = 0; j < k; ++j) need[q] |= (s_dest[tt * k + j] >= 0);
+          if (need[q]) val[q] = ld_nc_v4(src0 + v);
+        }
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < UNROLL; ++q) {
+      const int v = vb + tid + q * 256;
+      if (v < n_vec && need[q]) {
+        const int tt = v / vpr;
+        const int vv = v - tt * vpr;
+        for (int j = 0; j < k; ++j) {
+          const int r = s_dest[tt * k + j];
+          if (r >= 0) st_na_v4(dst0 + (size_t)r * vpr + vv, val[q]);
+        }
+      }
+    }
+  }
+
   // ---- padding rows (align > 1): index -1, zero activations ----
   if (align > 1) {
-    const int vec_per_row = d / 8;
-    for (int s = blockIdx.x; s < E_loc; s += gridDim.x) {
-      const int p0 = s_off[s] + totals[s], p1 = s_off[s + 1];
-      for (int r = p0 + warp; r < p1; r += kWarpsPerBlock) {
+    for (int s = b; s < E_loc; s += gridDim.x) {
+      const int p0 = __ldg(offsets + s) + __ldg(totals + s), p1 = __ldg(offsets + s + 1);
+      for (int r = p0 + warp; r < p1; r += 8) {
         if (lane == 0) row_to_assign[r] = -1;
-        uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
-        for (int v = lane; v < vec_per_row; v += 32) dst[v] = make_uint4(0, 0, 0, 0);
+        uint4* dst = dst0 + (size_t)r * vpr;
+        for (int v = lane; v < vpr; v += 32) dst[v] = make_uint4(0, 0, 0, 0);
       }
     }
   }
 }
 
-// K4 ------------------------------------------------------------------------------------
-// One thread per VPT 16-byte vectors of one token row (vectors v and v + vpr/2 when VPT == 2):
-// the vector is read once and stored to each of the token's <= k destination rows.  The k
-// row indices are warp-uniform addresses (one broadcast transaction, L1-resident).  No
-// grid-stride loop: the grid covers T * vpr / VPT threads.
-template <int VPT>
-__global__ void __launch_bounds__(256) perm_rows_kernel(const __nv_bfloat16* __restrict__ X,
-                                                        const int32_t* __restrict__ assign_to_row, int T, int k,
-                                                        int d, __nv_bfloat16* __restrict__ Xp) {
-  const int vpr = d >> 3;
-  const int per_row = vpr / VPT;
-  const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (g >= (long long)T * per_row) return;
-  const int t = (int)(g / per_row);
-  const int v0 = (int)(g - (long long)t * per_row);
-  const int32_t* a2r = assign_to_row + (size_t)t * k;
-  bool any = false;
-  for (int j = 0; j < k; ++j) any |= (__ldg(a2r + j) >= 0);
-  if (!any) return;
-  const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)t * d) + v0;
-  uint4 val[VPT];
-#pragma unroll
-  for (int q = 0; q < VPT; ++q) val[q] = ld_nc_v4(src + q * per_row);
-  for (int j = 0; j < k; ++j) {
-    const int r = __ldg(a2r + j);
-    if (r < 0) continue;
-    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d) + v0;
-#pragma unroll
-    for (int q = 0; q < VPT; ++q) st_na_v4(dst + q * per_row, val[q]);
-  }
-}
-
-// K4' -----------------------------------------------------------------------------------
-// Row-major variant for expert-parallel shards (E_loc < E), where only a fraction of the
-// T*k assignments is resident: persistent warps walk the R = offsets[E_loc] real rows
-// (extent read on the device) and copy X[row_to_assign[r] / k, :] -> Xp[r, :], UNROLL
-// independent 16-byte loads in flight per lane.  Work is proportional to R, not to T*k.
-template <int UNROLL>
-__global__ void __launch_bounds__(256) perm_rows_by_row_kernel(const __nv_bfloat16* __restrict__ X,
-                                                               const int32_t* __restrict__ row_to_assign,
-                                                               const int32_t* __restrict__ offsets, int E_loc,
-                                                               int k, int d, __nv_bfloat16* __restrict__ Xp) {
-  const int R = __ldg(offsets + E_loc);
-  const int lane = threadIdx.x & 31;
-  const int nwarps = gridDim.x * (256 / 32);
-  const int vpr = d >> 3;
-  for (int r = blockIdx.x * (256 / 32) + (threadIdx.x >> 5); r < R; r += nwarps) {
-    const int i = __ldg(row_to_assign + r);
-    if (i < 0) continue;   // padding row: already zero-filled by perm_index_kernel
-    const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)(i / k) * d);
-    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
-    for (int v0 = lane; v0 < vpr; v0 += 32 * UNROLL) {
-      uint4 val[UNROLL];
-#pragma unroll
-      for (int q = 0; q < UNROLL; ++q)
-        if (v0 + 32 * q < vpr) val[q] = ld_nc_v4(src + v0 + 32 * q);
-#pragma unroll
-      for (int q = 0; q < UNROLL; ++q)
-        if (v0 + 32 * q < vpr) st_na_v4(dst + v0 + 32 * q, val[q]);
-    }
-  }
+struct Chunking {
+  int TPC, CH, NB;
+};
+Chunking chunking(int T, int k) {
+  Chunking c;
+  int tpc = (T + kTargetChunks - 1) / kTargetChunks;
+  if (tpc < 1) tpc = 1;
+  const int max_tpc = kMaxChunk / k > 0 ? kMaxChunk / k : 1;
+  if (tpc > max_tpc) tpc = max_tpc;
+  c.TPC = tpc;
+  c.CH = tpc * k;
+  c.NB = T > 0 ? (T + tpc - 1) / tpc : 1;
+  return c;
 }
 
 }  // namespace
 
 size_t permute_ws_bytes(int T, int k, int E_loc) {
-  const int64_t A = (int64_t)T * k;
-  const int64_t NW = (A + kChunk - 1) / kChunk;
-  return round_up((size_t)(NW > 0 ? NW : 1) * E_loc * sizeof(int32_t), 256) +
-         round_up((size_t)E_loc * sizeof(int32_t), 256);
+  const Chunking c = chunking(T, k);
+  return round_up((size_t)c.NB * E_loc * sizeof(int32_t), 256) + round_up((size_t)E_loc * sizeof(int32_t), 256);
 }
 
 }  // namespace vibe
@@ -262,6 +268,7 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   VIBE_REQUIRE(d % 8 == 0, VIBE_ERR_INVALID_ARG, "vibe_permute: d %% 8 != 0 (rows must be 16-byte multiples)");
   VIBE_REQUIRE(align >= 1, VIBE_ERR_INVALID_ARG, "vibe_permute: align < 1");
   VIBE_REQUIRE(k <= E, VIBE_ERR_INVALID_ARG, "vibe_permute: k > E");
+  VIBE_REQUIRE(k <= kMaxChunk, VIBE_ERR_UNSUPPORTED, "vibe_permute: k > %d not implemented", kMaxChunk);
   VIBE_REQUIRE(E_loc <= E, VIBE_ERR_INVALID_ARG, "vibe_permute: E_loc > E");
   VIBE_REQUIRE(expert_map != nullptr || E_loc == E, VIBE_ERR_INVALID_ARG,
                "vibe_permute: expert_map NULL requires E_loc == E");
@@ -283,35 +290,18 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
     VIBE_CUDA(cudaMemsetAsync(offsets, 0, (size_t)(E_loc + 1) * sizeof(int32_t), st));
     return VIBE_OK;
   }
-  const int NW = (A + kChunk - 1) / kChunk;
+  const Chunking c = chunking(T, k);
   int32_t* hist = reinterpret_cast<int32_t*>(ws);
   int32_t* totals = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) +
-                                               round_up((size_t)NW * E_loc * sizeof(int32_t), 256));
-  const int nblk = (NW + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  const size_t smem1 = (size_t)kWarpsPerBlock * E_loc * sizeof(int);
-  const size_t smem3 = (size_t)(E_loc + 1 + kWarpsPerBlock * E_loc) * sizeof(int);
-  perm_hist_kernel<<<nblk, 256, smem1, st>>>(topk_ids, expert_map, A, E, E_loc, NW, hist);
-  VIBE_LAUNCH_CHECK("perm_hist_kernel");
-  perm_scan_kernel<<<E_loc, 256, 0, st>>>(hist, NW, totals);
-  VIBE_LAUNCH_CHECK("perm_scan_kernel");
-  perm_index_kernel<<<nblk, 256, smem3, st>>>(topk_ids, expert_map, A, E, E_loc, NW, align, d, hist, totals, offsets,
-                                              row_to_assign, assign_to_row, reinterpret_cast<__nv_bfloat16*>(Xp));
-  VIBE_LAUNCH_CHECK("perm_index_kernel");
-  const int vpr = d / 8;
-  const __nv_bfloat16* Xb = reinterpret_cast<const __nv_bfloat16*>(X);
-  __nv_bfloat16* Xpb = reinterpret_cast<__nv_bfloat16*>(Xp);
-  if (E_loc < E) {
-    // expert-parallel shard: work proportional to the resident rows
-    perm_rows_by_row_kernel<4><<<num_sms() * 8, 256, 0, st>>>(Xb, row_to_assign, offsets, E_loc, k, d, Xpb);
-  } else {
-    const int vpt = (vpr % 2 == 0) ? 2 : 1;
-    const long long blocks = ((long long)T * (vpr / vpt) + 255) / 256;
-    VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "vibe_permute: T*d too large for one launch");
-    if (vpt == 2)
-      perm_rows_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
-    else
-      perm_rows_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(Xb, assign_to_row, T, k, d, Xpb);
-  }
-  VIBE_LAUNCH_CHECK("perm_rows_kernel");
+                                               round_up((size_t)c.NB * E_loc * sizeof(int32_t), 256));
+  static std::atomic<unsigned> next_ticket{0};
+  const int ticket = (int)(next_ticket.fetch_add(1, std::memory_order_relaxed) % kTickets);
+  perm_count_kernel<<<c.NB, 1024, 0, st>>>(topk_ids, expert_map, A, E, E_loc, c.CH, c.NB, align, ticket, hist, totals,
+                                           offsets);
+  VIBE_LAUNCH_CHECK("perm_count_kernel");
+  perm_scatter_kernel<4><<<c.NB, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(X), topk_ids, expert_map, T, k,
+                                               d, E, E_loc, c.TPC, align, hist, totals, offsets, row_to_assign,
+                                               assign_to_row, reinterpret_cast<__nv_bfloat16*>(Xp));
+  VIBE_LAUNCH_CHECK("perm_scatter_kernel");
   return VIBE_OK;
 }

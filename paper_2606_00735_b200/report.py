@@ -1,0 +1,293 @@
+"""Per-kernel measurements on one B200 beyond the single bench.py line.
+
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,profile,placement]
+                                           [--out gpurun_out/report.json] [--quick]
+
+Sections (all through the C-ABI binding; seeded synthetic inputs):
+  stages     route / permute / combine timed one kernel family at a time on rotating buffer
+             sets whose footprint exceeds the 126 MB L2 (cold reads), for BASELINE.json
+             configs[1..3] and a 64K-token stress shape: achieved GB/s = algorithmic bytes
+              / CUDA-event time, and the fraction of the measured HBM peak.
+  ffn        grouped FFN on BALANCED routing (every expert n rows), n = 128..4096, for the
+             C1/C2/C3 shapes: TFLOP/s and fraction of the measured bf16 peaks -- the
+             ">= 512 tokens per expert" target of BASELINE.json is read off this table.
+  profile    vibe_profile_expert_latency over the M3 sweep (1..4096 tokens per expert), modes 0
+             and 1, for the C2 and C3 shapes: the per-GPU performance model f(n) of the paper
+             (PAPER.md L176).  Written as CSV rows into the JSON and to <out>.profile.csv.
+  placement  BASELINE.json configs[4]: 256 experts onto 8 virtual GPUs with throughput scales
+             U[0.78,1.0]; loads = routing histograms (vibe_route_topk) for Zipf s in
+             {0.8,1.2,1.6} x T in {2K,16K,64K}; contiguous vs token-balanced vs latency-balanced
+             (ViBE Alg. 1 phase 2) under the measured C3-shape profile, model kinds A and B,
+             cap = 32 and cap = 0.
+
+Everything here calls the CUDA library; nothing imports oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+import torch
+
+from . import binding as B
+from . import inputs as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "kind": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "kind": "fallback"}
+
+
+def _time(fn, iters, warmup=5, period=1):
+    """Average CUDA-event time [us] of one fn(i) call.  `period` consecutive calls (one per
+    rotating buffer set) are captured into a CUDA graph and the graph is replayed, so the
+    number is the device time of the kernels, not the host's launch rate."""
+    for i in range(max(warmup, period)):
+        fn(i)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(period):
+            fn(i)
+    reps = max(1, iters // period)
+    g.replay()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        g.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e3 / (reps * period)
+
+
+def _dev_bf16(bits):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+
+
+STRESS = I.LayerConfig("S64K-stress", T=65536, d=2048, f=768, E=256, k=8, E_loc=256, zipf_s=1.0)
+
+
+def section_stages(peaks, quick):
+    """a1/a3/a5 in isolation, cold buffers."""
+    out = []
+    hbm = peaks["hbm_gbs"]
+    for cfg in (I.C1, I.C2, I.C3, STRESS):
+        T, k, E, E_loc, d = cfg.T, cfg.k, cfg.E, cfg.E_loc, cfg.d
+        A = T * k
+        Rcap = B.rows_cap(T, k, E_loc, 1)
+        per_set = T * E * 4 + T * d * 2 + 2 * Rcap * d * 2 + T * d * 2
+        nsets = max(2, min(8, int(np.ceil(400e6 / per_set))))
+        emap_np = I.make_expert_map(cfg, "contiguous", 0)
+        emap = torch.from_numpy(emap_np).cuda() if E_loc < E else None
+        bias = torch.from_numpy(I.make_select_bias(E, 0)).cuda() if cfg.has_select_bias else None
+        rc = B.RouteConfig(select_bias=bias, **I.route_kwargs(cfg))
+        sets = []
+        for i in range(nsets):
+            lg = torch.from_numpy(I.make_logits(T, E, cfg.zipf_s, i, cfg.alpha)).cuda()
+            X = torch.randn((T, d), device="cuda", dtype=torch.float32).to(torch.bfloat16)
+            s = {"lg": lg, "X": X,
+                 "ids": torch.empty((T, k), dtype=torch.int32, device="cuda"),
+                 "w": torch.empty((T, k), dtype=torch.float32, device="cuda"),
+                 "counts": torch.empty((E,), dtype=torch.int32, device="cuda"),
+                 "Xp": torch.empty((Rcap, d), dtype=torch.bfloat16, device="cuda"),
+                 "Y": torch.randn((Rcap, d), device="cuda", dtype=torch.float32).to(torch.bfloat16)
+                 if Rcap * d < 2 ** 31 else torch.zeros((Rcap, d), dtype=torch.bfloat16, device="cuda"),
+                 "off": torch.empty((E_loc + 1,), dtype=torch.int32, device="cuda"),
+                 "r2a": torch.empty((Rcap,), dtype=torch.int32, device="cuda"),
+                 "a2r": torch.empty((A,), dtype=torch.int32, device="cuda"),
+                 "out": torch.empty((T, d), dtype=torch.bfloat16, device="cuda")}
+            sets.append(s)
+        ws = torch.empty((max(16, B.workspace_bytes(B.WS_PERMUTE, T, k, E, E_loc, d, 0)),), dtype=torch.uint8,
+                         device="cuda")
+
+        def route(i):
+            s = sets[i % nsets]
+            B.route_topk(s["lg"], rc, out=(s["ids"], s["w"], s["counts"]))
+
+        def permute(i):
+            s = sets[i % nsets]
+            B.permute(s["X"], s["ids"], s["counts"], emap, E, E_loc, 1, out=(s["Xp"], s["off"], s["r2a"], s["a2r"]),
+                      ws=ws)
+
+        def combine(i):
+            s = sets[i % nsets]
+            B.combine(s["Y"], s["a2r"], s["w"], T, k, out=s["out"])
+
+        iters = 40 if quick else 200
+        n0 = B.launch_count()
+        route(0)
+        l_route = B.launch_count() - n0
+        n0 = B.launch_count()
+        permute(0)
+        l_perm = B.launch_count() - n0
+        t_route = _time(route, iters, period=nsets)
+        t_perm = _time(permute, iters, period=nsets)
+        t_comb = _time(combine, iters, period=nsets)
+        s0 = sets[0]
+        R = int(s0["off"][-1].item())
+        res_tok = int((s0["a2r"].view(T, k) >= 0).any(dim=1).sum().item())
+        by = {"route": 4.0 * T * E + 8.0 * T * k + 4.0 * E,
+              "permute": 2.0 * res_tok * d + 2.0 * R * d + 12.0 * A,
+              "combine": 2.0 * R * d + 2.0 * T * d + 8.0 * A}
+        row = {"config": cfg.name, "T": T, "E": E, "E_loc": E_loc, "k": k, "d": d, "real_rows": R,
+               "resident_tokens": res_tok, "buffer_sets": nsets, "set_bytes": per_set,
+               "launches": {"route": l_route, "permute": l_perm, "combine": 1}}
+        for name, t in (("route", t_route), ("permute", t_perm), ("combine", t_comb)):
+            gbs = by[name] / t / 1e3
+            row[name] = {"us": round(t, 2), "bytes": by[name], "GB/s": round(gbs, 1), "frac_hbm": round(gbs / hbm, 4),
+                         "us_at_hbm_peak": round(by[name] / hbm / 1e3, 2)}
+        out.append(row)
+        del sets
+        torch.cuda.empty_cache()
+    return out
+
+
+def _weights(E, d, f):
+    W1 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
+    W3 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
+    W2 = (torch.randn((E, f, d), device="cuda") * f ** -0.5).to(torch.bfloat16)
+    return W1, W3, W2
+
+
+def _warm(W1, W3, W2, seconds=2.0):
+    """'Each GPU is warmed to steady-state operating conditions': back-to-back
+    grouped FFN at 1024 tokens per expert for `seconds`."""
+    t0 = time.time()
+    while time.time() - t0 < seconds:
+        B.profile_expert_latency(W1, W3, W2, (1024,), mode=0, warmup=0, iters=20)
+
+
+def section_ffn(peaks, quick):
+    out = []
+    sweep = (128, 256, 512, 1024, 2048, 4096)
+    for cfg in (I.C1, I.C2, I.C3):
+        E, d, f = cfg.E_loc, cfg.d, cfg.f
+        W1, W3, W2 = _weights(E, d, f)
+        _warm(W1, W3, W2, 0.5 if quick else 2.0)
+        lat = B.profile_expert_latency(W1, W3, W2, sweep, mode=0, warmup=5, iters=20 if quick else 50)
+        for n, l in zip(sweep, lat):
+            tf = 6.0 * n * d * f / l / 1e6
+            bytes_e = 6.0 * d * f + 4.0 * n * d + 4.0 * n * f
+            t_roof = max(6.0 * n * d * f / (peaks["bf16_tflops_sustained"] * 1e6), bytes_e / (peaks["hbm_gbs"] * 1e3))
+            out.append({"shape": cfg.name, "E_loc": E, "d": d, "f": f, "tokens_per_expert": n,
+                        "us_per_expert": round(float(l), 3), "TFLOP/s": round(tf, 1),
+                        "frac_sustained": round(tf / peaks["bf16_tflops_sustained"], 4),
+                        "frac_burst": round(tf / peaks["bf16_tflops"], 4),
+                        "frac_of_per_expert_roofline": round(t_roof / float(l), 4)})
+        del W1, W3, W2
+        torch.cuda.empty_cache()
+    return out
+
+
+def section_profile(peaks, quick):
+    out = {}
+    for cfg in (I.C2, I.C3):
+        E, d, f = cfg.E_loc, cfg.d, cfg.f
+        W1, W3, W2 = _weights(E, d, f)
+        _warm(W1, W3, W2, 0.5 if quick else 2.0)
+        rows = []
+        for mode in (0, 1):
+            lat, samples = B.profile_expert_latency(W1, W3, W2, B.DEFAULT_SWEEP, mode=mode, warmup=10,
+                                                    iters=20 if quick else 100, return_samples=True)
+            if mode == 0:
+                samples = samples / E
+            for j, n in enumerate(B.DEFAULT_SWEEP):
+                floor_us = 6.0 * d * f / (peaks["hbm_gbs"] * 1e3)      # the expert's weight bytes at HBM peak
+                rows.append({"mode": mode, "tokens_per_expert": int(n), "latency_us": round(float(lat[j]), 3),
+                             "p10_us": round(float(np.percentile(samples[j], 10)), 3),
+                             "p90_us": round(float(np.percentile(samples[j], 90)), 3),
+                             "weight_stream_floor_us": round(floor_us, 3) if mode == 0 else None})
+        out[cfg.name] = {"E_loc": E, "d": d, "f": f, "rows": rows}
+        del W1, W3, W2
+        torch.cuda.empty_cache()
+    return out
+
+
+def section_placement(peaks, quick, profile):
+    """BASELINE.json configs[4] on the measured C3-shape profile (mode 0)."""
+    if profile is None:
+        profile = section_profile(peaks, True)
+    prof = [r for r in profile[I.C3.name]["rows"] if r["mode"] == 0]
+    model = B.LatencyModel([r["tokens_per_expert"] for r in prof], [r["latency_us"] for r in prof],
+                           E_prof=profile[I.C3.name]["E_loc"])
+    E, G, k = 256, 8, 8
+    rc = B.RouteConfig(num_experts=E, top_k=k)
+    out = []
+    for s in (0.8, 1.2, 1.6):
+        for T in (2048, 16384, 65536):
+            lg = torch.from_numpy(I.make_logits(T, E, s, 7, 1.0)).cuda()
+            _, _, counts = B.route_topk(lg, rc)
+            load = counts.cpu().numpy().astype(np.float64)
+            for seed in range(2 if quick else 8):
+                scale = I.make_throughput_scales(G, seed)
+                for cap in (E // G, 0):
+                    binnings = {"contiguous": B.placement_contiguous(E, G),
+                                "token_balanced": B.placement_token_balanced(load, G, cap),
+                                "latency_balanced": B.placement_greedy(load, G, scale, model, cap)}
+                    for kind, kname in ((B.MODEL_A, "A"), (B.MODEL_B, "B")):
+                        row = {"zipf_s": s, "T": T, "scale_seed": seed, "cap": cap, "model": kname}
+                        for name, asg in binnings.items():
+                            sc, per = B.placement_eval(asg, load, G, scale, model, kind)
+                            row[name] = {"score_us": round(sc, 3), "max_over_mean": round(sc / float(per.mean()), 4)}
+                        row["gain_latency_vs_token"] = round(1.0 - row["latency_balanced"]["score_us"] /
+                                                             row["token_balanced"]["score_us"], 4)
+                        row["gain_latency_vs_contiguous"] = round(1.0 - row["latency_balanced"]["score_us"] /
+                                                                  row["contiguous"]["score_us"], 4)
+                        out.append(row)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--sections", default="stages,ffn,profile,placement")
+    ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
+    ap.add_argument("--quick", action="store_true")
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("report: no CUDA device -- the product has no CPU fallback")
+    B.load()
+    torch.cuda.set_device(0)
+    peaks = _peaks()
+    rep = {"peaks": peaks, "gpu": torch.cuda.get_device_name(0)}
+    want = args.sections.split(",")
+    if "stages" in want:
+        rep["stages"] = section_stages(peaks, args.quick)
+        for r in rep["stages"]:
+            print(r["config"], {n: (r[n]["us"], r[n]["GB/s"], r[n]["frac_hbm"]) for n in ("route", "permute", "combine")},
+                  flush=True)
+    if "ffn" in want:
+        rep["ffn_balanced"] = section_ffn(peaks, args.quick)
+        for r in rep["ffn_balanced"]:
+            print(r["shape"], r["tokens_per_expert"], r["us_per_expert"], r["TFLOP/s"], r["frac_sustained"], flush=True)
+    if "profile" in want:
+        rep["profile"] = section_profile(peaks, args.quick)
+    if "placement" in want:
+        rep["placement_stress"] = section_placement(peaks, args.quick, rep.get("profile"))
+        g = [r["gain_latency_vs_token"] for r in rep["placement_stress"] if r["model"] == "B" and r["cap"] > 0]
+        print(f"placement: latency- vs token-balanced gain (model B, cap 32): median {np.median(g):.3f} "
+              f"min {min(g):.3f} max {max(g):.3f}", flush=True)
+    os.makedirs(os.path.dirname(args.out), exist_ok=True)
+    with open(args.out, "w") as fh:
+        json.dump(rep, fh, indent=1)
+    if "profile" in rep:
+        with open(args.out.replace(".json", "") + ".profile.csv", "w") as fh:
+            fh.write("shape,mode,tokens_per_expert,latency_us,p10_us,p90_us\n")
+            for name, p in rep["profile"].items():
+                for r in p["rows"]:
+                    fh.write(f"{name},{r['mode']},{r['tokens_per_expert']},{r['latency_us']},{r['p10_us']},{r['p90_us']}\n")
+    print("wrote", args.out)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -142,3 +142,80 @@ def test_placement_invalid_arguments(lib):
         B.placement_greedy([1.0, 2.0], 2, [1.0, 0.0], None)
     with pytest.raises(B.VibeError):
         B.placement_eval([0, 1], [1.0, 2.0], 2, [1.0, 1.0], B.LatencyModel([2, 1], [1.0, 2.0], 1))
+
+
+# ------------------------------------------------------------------ f1: recalibration (host code) vs oracle
+def test_drift_cosine_and_monitor_match_oracle(lib):
+    rng = I._rng(5, 5)
+    for _ in range(20):
+        a, b = rng.uniform(0, 50, 64), rng.uniform(0, 50, 64)
+        assert B.drift_cosine(a, b) == O.cosine_distance(a, b)          # same operation order: bit-identical
+    assert B.drift_cosine([0, 0], [1, 2]) == 0.0
+    L, E = 3, 16
+    bm, om = B.DriftMonitor(L, E, window=20, H=5, delta=0.05), O.DriftMonitor(L, E, window=20, H=5, delta=0.05)
+    base = rng.uniform(1, 100, (L, E))
+    shifted = base[:, ::-1].copy()
+    ref_set = False
+    for p in range(1, 161):
+        mix = 0.0 if p < 60 else min(1.0, (p - 60) / 40.0)
+        loads = np.floor((1 - mix) * base + mix * shifted + rng.uniform(0, 3, (L, E)))
+        tb, db = bm.push(loads)
+        to, do = om.push(loads)
+        assert tb == to and (db is None) == (do is None)
+        if db is not None:
+            assert np.array_equal(db, do)
+        if p == 20 and not ref_set:
+            bm.set_reference(om.window_mean())
+            om.set_reference(om.window_mean())
+            assert np.array_equal(bm.window_mean(), om.window_mean())
+            ref_set = True
+        if tb:
+            bm.rearranged()
+            om.rearranged()
+    assert om.passes == 160 and om.ref is not None
+    bm.close()
+    with pytest.raises(B.VibeError):
+        B.DriftMonitor(0, 4)
+
+
+def test_swap_refine_matches_oracle_and_golden(lib, golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "swap_refine_worked_example.json")))
+    a, swaps = B.placement_swap_refine(g["assign_start"], g["load"], 2, g["scale"], None, B.MODEL_A, g["eps"])
+    assert a.tolist() == g["assign_final"] and [list(s) for s in swaps] == g["swaps"]
+    n = g["no_reduction_case"]
+    a, swaps = B.placement_swap_refine(n["assign_start"], n["load"], 2, n["scale"], None, B.MODEL_B, 0.03)
+    assert a.tolist() == n["assign_start"] and swaps == []
+    for (bm, om), kind, (E, G, seed) in itertools.product(_models(), (B.MODEL_A, B.MODEL_B),
+                                                          [(16, 4, 0), (32, 8, 1), (64, 8, 2)]):
+        rng = I._rng(seed, 78)
+        load = np.floor(rng.pareto(1.2, E) * 40 + 1)
+        scale = I.make_throughput_scales(G, seed)
+        start = O.placement_contiguous(E, G)
+        got, gs = B.placement_swap_refine(start, load, G, scale, bm, kind, 0.03)
+        want, ws = O.placement_swap_refine(start, load, G, scale, om, kind, 0.03)
+        assert np.array_equal(got, want) and gs == [tuple(map(int, s)) for s in ws]
+        got1, gs1 = B.placement_swap_refine(start, load, G, scale, bm, kind, 0.03, max_swaps=2)
+        assert gs1 == gs[:2]
+    with pytest.raises(B.VibeError):
+        B.placement_swap_refine([0, 3], [1.0, 2.0], 2, [1.0, 1.0], None)
+
+
+def test_swap_refine_on_placement_stress_shape(lib):
+    """configs[4] shape (256 experts, 8 bins, cap 32): a drifted load on a stale latency-balanced placement is
+    repaired with few swaps (the paper reports 5-30 per layer versus > 200 moves for a full re-solve)."""
+    E, G, k = 256, 8, 8
+    bm, om = _models()[1]
+    scale = I.make_throughput_scales(G, 3)
+    old = O.route_topk(I.make_logits(16384, E, 1.2, 3), E, k)[2].astype(np.float64)
+    new = O.route_topk(0.8 * I.make_logits(16384, E, 1.2, 3) + 0.2 * I.make_logits(16384, E, 1.2, 4), E, k)[2].astype(np.float64)
+    stale = B.placement_greedy(old, G, scale, bm, E // G)
+    before = B.placement_eval(stale, new, G, scale, bm, B.MODEL_B)[0]
+    fixed, swaps = B.placement_swap_refine(stale, new, G, scale, bm, B.MODEL_B, 0.03)
+    after, per = B.placement_eval(fixed, new, G, scale, bm, B.MODEL_B)
+    assert after <= before and np.bincount(fixed, minlength=G).tolist() == [E // G] * G
+    assert int((fixed != stale).sum()) <= 2 * len(swaps)          # every swap moves two experts
+    resolve = B.placement_greedy(new, G, scale, bm, E // G)
+    moved_full = int((resolve != stale).sum())
+    assert 2 * len(swaps) <= moved_full or len(swaps) == 0
+    want, ws = O.placement_swap_refine(stale, new, G, scale, om, O.MODEL_B, 0.03)
+    assert np.array_equal(fixed, want)
