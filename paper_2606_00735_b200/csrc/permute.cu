@@ -1,21 +1,30 @@
 // permute.cu -- a3: stable counting sort of assignments by local expert slot + row gather
 // (vibe_permute).  Semantics: include/vibe.h, readings P1-P4.
 //
-// Two launches on one stream, no host sync, no spin-waits between CTAs.  The batch is cut
-// into NB chunks of TPC consecutive tokens (= CH = TPC*k consecutive assignments); NB is a
-// few CTAs per SM so that the row copy of K2 fills the machine.
-//   K1 perm_count   : CTA b histograms the slots of chunk b into hist[b][*].  The LAST CTA to
-//                     finish (a ticket counter; no CTA ever waits for another) turns the
-//                     table into per-slot exclusive prefixes over the chunks, and writes the
-//                     slot totals and offsets[] (aligned exclusive scan of the totals).
-//   K2 perm_scatter : CTA b ranks the assignments of chunk b IN ORDER (warp 0: match.any + a
-//                     running counter per slot that starts at offsets[s] + hist[b][s]) => rows
-//                     inside a slot are in ascending flat index (stable, bit-exact w.r.t. the
-//                     counting-sort definition); writes assign_to_row / row_to_assign; then
-//                     copies its TPC token rows: X[t,:] is read ONCE (16-byte vectors, the
-//                     loads are issued before the ranking finishes) and stored to each of its
-//                     <= k destination rows, so DRAM traffic is the algorithmic
-//                     2*T_res*d + 2*R*d bytes.  Padding rows (align > 1) are zero-filled.
+// Two launches on one stream, no host sync:
+//   K1 perm_index  : a COOPERATIVE launch of G <= #SMs CTAs x 1024 threads (all co-resident, so
+//                    the one grid-wide barrier below cannot deadlock).  Warp gw = 32*cta + w owns
+//                    the contiguous chunk [gw*WCH, (gw+1)*WCH) of the A = T*k assignments.
+//                      pass 1  lanes holding the same slot are matched with ballots (one per key
+//                              bit, fixed cost); per-warp slot histograms in shared memory; the
+//                              matching (lanes below me, group size, leader) is parked in
+//                              assign_to_row so that pass 2 needs no votes
+//                      scan    exclusive prefix over the 32 warps of the CTA per slot; the CTA
+//                              totals go to a [G][E_loc] table in the workspace; GRID BARRIER;
+//                              every CTA sums the rows of the CTAs before it (its base) and all
+//                              rows (slot totals), and derives offsets[] (aligned exclusive scan)
+//                      pass 2  every warp re-walks its chunk IN ORDER: row = base + running
+//                              counter + lanes below me => rows inside a slot are in ascending
+//                              flat index (stable, bit-exact w.r.t. the counting-sort
+//                              definition).  Writes assign_to_row / row_to_assign; zero-fills
+//                              padding rows (align > 1).
+//                    (A single 8-CTA cluster with a DSMEM exchange was measured first: 8 SMs are
+//                    too few -- the scattered 4-byte row_to_assign stores and the votes of 256
+//                    warps saturate their LSU/vote pipes: 17 us at A = 64K, 105 us at A = 512K.)
+//   K2 perm_rows   : token-major gather/scatter of the bf16 rows, one thread per 16-byte vector:
+//                    X[t,:] is read ONCE and written to each of its <= k destination rows,
+//                    so DRAM traffic equals the algorithmic 2*T_res*d + 2*R*d bytes.
+//                    (E_loc < E: the row-major variant perm_rows_by_row, work ~ R.)
 #include <atomic>
 
 #include "common.cuh"
@@ -24,13 +33,15 @@ namespace vibe {
 namespace {
 
 constexpr int kMaxSlots = 1024;
-constexpr int kMaxChunk = 1024;      // assignments per chunk (CH = TPC*k)
-constexpr int kTargetChunks = 592;   // ~4 CTAs per SM
-constexpr int kTickets = 64;
+constexpr int kIdxThreads = 1024;
+constexpr int kIdxWarps = kIdxThreads / 32;
+constexpr int kBatch = 8;            // id loads in flight per lane
+constexpr int kBarSlots = 64;
+static_assert(kIdxWarps == 32, "the offsets scan keeps one warp partial per lane");
 
-// Ticket counters of K1 (one per in-flight call, round-robin): zero at module load, and the
-// last CTA of every call puts its counter back to zero.
-__device__ unsigned int g_tickets[kTickets];
+// Grid-barrier state of K1, one slot per in-flight call (round-robin): {arrived, departed}.
+// Zero at module load; the last CTA to depart puts its slot back to zero.
+__device__ unsigned int g_bar[kBarSlots][2];
 
 __device__ __forceinline__ int slot_of(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int i,
                                        int E, int E_loc) {
@@ -40,69 +51,132 @@ __device__ __forceinline__ int slot_of(const int32_t* __restrict__ ids, const in
   return (s >= 0 && s < E_loc) ? s : -1;
 }
 
-// K1 ------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) perm_count_kernel(const int32_t* __restrict__ ids,
-                                                          const int32_t* __restrict__ emap, int A, int E, int E_loc,
-                                                          int CH, int NB, int align, int ticket,
-                                                          int32_t* __restrict__ hist /*[NB][E_loc]*/,
-                                                          int32_t* __restrict__ totals /*[E_loc]*/,
-                                                          int32_t* __restrict__ offsets /*[E_loc+1]*/) {
-  __shared__ int s_cnt[kMaxSlots];
-  __shared__ int s_part[1024];
-  __shared__ int s_last;
-  const int tid = threadIdx.x;
-  for (int s = tid; s < E_loc; s += 1024) s_cnt[s] = 0;
+// Lanes of the warp that hold the same key (key in [0, 2^nbits)): nbits ballots, fixed cost.
+__device__ __forceinline__ unsigned same_key_lanes(int key, int nbits) {
+  unsigned peers = 0xffffffffu;
+  for (int b = 0; b < nbits; ++b) {
+    const bool bit = (key >> b) & 1;
+    const unsigned bal = __ballot_sync(0xffffffffu, bit);
+    peers &= bit ? bal : ~bal;
+  }
+  return peers;
+}
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// All G CTAs of the (cooperative) grid meet here once.
+__device__ __forceinline__ void grid_barrier_once(unsigned* bar, unsigned G) {
   __syncthreads();
-  const int lo = blockIdx.x * CH, hi = min(A, lo + CH);
-  for (int i = lo + tid; i < hi; i += 1024) {
-    const int s = slot_of(ids, emap, i, E, E_loc);
-    if (s >= 0) atomicAdd(&s_cnt[s], 1);
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(&bar[0], 1u);
+    while (ld_acquire_u32(&bar[0]) < G) __nanosleep(32);
+    __threadfence();
+    if (atomicAdd(&bar[1], 1u) == G - 1) {   // everybody has seen arrived == G
+      bar[0] = 0;
+      bar[1] = 0;
+    }
   }
   __syncthreads();
-  int32_t* row = hist + (size_t)blockIdx.x * E_loc;
-  for (int s = tid; s < E_loc; s += 1024) row[s] = s_cnt[s];
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(&g_tickets[ticket], 1u) == (unsigned)(NB - 1));
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  if (tid == 0) g_tickets[ticket] = 0;
+}
 
-  // ---- last CTA: hist[b][s] <- sum_{b' < b} hist[b'][s]; totals; offsets ----
-  // Threads form G groups of W = min(E_loc, 1024) slot columns; group g owns the chunk rows
-  // [g*RPG, (g+1)*RPG).  Pass 1: group sums; exclusive scan over the groups; pass 2: rewrite.
-  for (int s0 = 0; s0 < E_loc; s0 += 1024) {
-    const int W = min(E_loc - s0, 1024);
-    const int G = 1024 / W;
+// K1 ------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kIdxThreads, 1)
+perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int A, int E, int E_loc,
+                  int WCH, int align, int d, int bar_slot, int32_t* __restrict__ tbl /*[G][E_loc]*/,
+                  int32_t* __restrict__ offsets /*[E_loc+1]*/, int32_t* __restrict__ row_to_assign,
+                  int32_t* __restrict__ assign_to_row, __nv_bfloat16* __restrict__ Xp) {
+  extern __shared__ int s_mem[];
+  int* s_wh = s_mem;                            // [kIdxWarps][E_loc] per-warp counts -> running row
+  int* s_base = s_wh + kIdxWarps * E_loc;       // [E_loc] offsets[s] + rows of the preceding CTAs
+  int* s_tot = s_base + E_loc;                  // [E_loc] slot totals of the whole batch
+  int* s_off = s_tot + E_loc;                   // [E_loc+1] aligned segment starts
+  int* s_red = s_off + E_loc + 1;               // [2][kIdxThreads] partial sums of the table walk
+  __shared__ int s_scan[kIdxWarps];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int cta = blockIdx.x, G = gridDim.x;
+  const int gw = cta * kIdxWarps + warp;
+  const int lo = min(A, gw * WCH), hi = min(A, lo + WCH);
+  int* wh = s_wh + warp * E_loc;
+  const int nbits = 32 - __clz(E_loc);   // keys are slot + 1 in [0, E_loc]
+
+  // programmatic dependent launch: K2's CTAs may become resident now; they wait in
+  // griddepcontrol.wait until this grid has completed and flushed
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  for (int s = lane; s < E_loc; s += 32) wh[s] = 0;
+  __syncwarp();
+  // ---- pass 1 (kBatch independent id loads are in flight before the first one is consumed) ----
+  for (int i0 = lo; i0 < hi; i0 += 32 * kBatch) {
+    int sl[kBatch];
+#pragma unroll
+    for (int q = 0; q < kBatch; ++q) {
+      const int i = i0 + q * 32 + lane;
+      sl[q] = (i < hi) ? slot_of(ids, emap, i, E, E_loc) : -1;
+    }
+#pragma unroll
+    for (int q = 0; q < kBatch; ++q) {
+      if (i0 + q * 32 >= hi) break;           // warp-uniform
+      const int i = i0 + q * 32 + lane;
+      const int s = sl[q];
+      const unsigned peers = same_key_lanes(s + 1, nbits);
+      const int below = __popc(peers & ((1u << lane) - 1u));
+      const int size = __popc(peers);
+      const bool leader = (peers >> lane) == 1u;           // highest lane of the group
+      if (s >= 0 && leader) wh[s] += size;
+      if (i < hi) assign_to_row[i] = (s >= 0) ? (below | (size << 6) | ((int)leader << 12)) : -1;
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  // ---- exclusive prefix over the warps of this CTA, per slot; CTA totals -> table ----
+  for (int s = tid; s < E_loc; s += kIdxThreads) {
+    int run = 0;
+#pragma unroll 8
+    for (int w = 0; w < kIdxWarps; ++w) {
+      const int v = s_wh[w * E_loc + s];
+      s_wh[w * E_loc + s] = run;
+      run += v;
+    }
+    tbl[(size_t)cta * E_loc + s] = run;
+  }
+  grid_barrier_once(g_bar[bar_slot], (unsigned)G);
+  // ---- walk the table: rows before mine (base) and all rows (totals).  W slot columns x
+  // NG row groups; group g takes rows g, g + NG, ... ----
+  for (int s0 = 0; s0 < E_loc; s0 += kIdxThreads) {
+    const int W = min(E_loc - s0, kIdxThreads);
+    const int NG = kIdxThreads / W;
     const int g = tid / W, c = tid - g * W;
-    const bool act = g < G;
-    const int RPG = (NB + G - 1) / G;
-    const int b0 = min(NB, g * RPG), b1 = min(NB, b0 + RPG);
-    volatile int32_t* col = hist + s0 + c;
-    int sum = 0;
-    if (act)
-      for (int b = b0; b < b1; ++b) sum += col[(size_t)b * E_loc];
-    s_part[tid] = act ? sum : 0;
-    __syncthreads();
-    int base = 0;
-    if (act)
-      for (int gg = 0; gg < g; ++gg) base += s_part[gg * W + c];
-    if (act && g == G - 1) s_cnt[s0 + c] = base + sum;     // slot total
-    if (act) {
-      int run = base;
-      for (int b = b0; b < b1; ++b) {
-        const int v = col[(size_t)b * E_loc];
-        col[(size_t)b * E_loc] = run;
-        run += v;
+    int pre = 0, total = 0;
+    if (g < NG) {
+      const int32_t* col = tbl + s0 + c;
+#pragma unroll 4
+      for (int r = g; r < G; r += NG) {
+        const int v = __ldcg(col + (size_t)r * E_loc);
+        pre += (r < cta) ? v : 0;
+        total += v;
       }
+    }
+    s_red[tid] = pre;
+    s_red[kIdxThreads + tid] = total;
+    __syncthreads();
+    if (tid < W) {
+      int p = 0, t = 0;
+      for (int gg = 0; gg < NG; ++gg) {
+        p += s_red[gg * W + tid];
+        t += s_red[kIdxThreads + gg * W + tid];
+      }
+      s_base[s0 + tid] = p;
+      s_tot[s0 + tid] = t;
     }
     __syncthreads();
   }
-  // offsets = exclusive scan of roundup(total, align) over <= 1024 slots (one value per thread)
+  // ---- offsets = exclusive scan of roundup(total, align) over <= 1024 slots (one per thread) ----
   {
-    const int lane = tid & 31, warp = tid >> 5;
-    const int tot = (tid < E_loc) ? s_cnt[tid] : 0;
+    const int tot = (tid < E_loc) ? s_tot[tid] : 0;
     const int v = ((tot + align - 1) / align) * align;
     int inc = v;
 #pragma unroll
@@ -110,141 +184,136 @@ __global__ void __launch_bounds__(1024) perm_count_kernel(const int32_t* __restr
       const int n = __shfl_up_sync(0xffffffffu, inc, o);
       if (lane >= o) inc += n;
     }
+    if (lane == 31) s_scan[warp] = inc;
     __syncthreads();
-    if (lane == 31) s_part[warp] = inc;
-    __syncthreads();
-    int woff = 0;
-    for (int w = 0; w < warp; ++w) woff += s_part[w];
+    int part = s_scan[lane];                 // kIdxWarps == 32: one partial per lane
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int n = __shfl_up_sync(0xffffffffu, part, o);
+      if (lane >= o) part += n;
+    }
+    const int woff = __shfl_sync(0xffffffffu, part, (warp + 31) & 31) * (warp > 0);
     if (tid < E_loc) {
-      totals[tid] = tot;
-      offsets[tid] = woff + inc - v;
-      if (tid == E_loc - 1) offsets[E_loc] = woff + inc;
+      const int start = woff + inc - v;
+      s_off[tid] = start;
+      s_base[tid] += start;
+      if (tid == E_loc - 1) s_off[E_loc] = woff + inc;
+    }
+    __syncthreads();
+    if (cta == 0)
+      for (int i = tid; i <= E_loc; i += kIdxThreads) offsets[i] = s_off[i];
+  }
+  // ---- pass 2: stable ranks (no votes: the parked matching + the running counters) ----
+  for (int i0 = lo; i0 < hi; i0 += 32 * kBatch) {
+    int sl[kBatch], pk[kBatch];
+#pragma unroll
+    for (int q = 0; q < kBatch; ++q) {
+      const int i = i0 + q * 32 + lane;
+      sl[q] = (i < hi) ? slot_of(ids, emap, i, E, E_loc) : -1;
+      pk[q] = (i < hi) ? assign_to_row[i] : -1;
+    }
+#pragma unroll
+    for (int q = 0; q < kBatch; ++q) {
+      if (i0 + q * 32 >= hi) break;           // warp-uniform
+      const int i = i0 + q * 32 + lane;
+      const int s = sl[q];
+      int r = -1;
+      if (s >= 0) r = s_base[s] + wh[s] + (pk[q] & 63);
+      __syncwarp();
+      if (s >= 0 && (pk[q] >> 12)) wh[s] += (pk[q] >> 6) & 63;
+      __syncwarp();
+      if (i < hi) {
+        assign_to_row[i] = r;
+        if (r >= 0) row_to_assign[r] = i;
+      }
+    }
+  }
+  // ---- padding rows (align > 1): index -1, zero activations ----
+  if (align > 1) {
+    const int vec_per_row = d / 8;
+    for (int s = cta; s < E_loc; s += G) {
+      const int p0 = s_off[s] + s_tot[s], p1 = s_off[s + 1];
+      for (int r = p0 + warp; r < p1; r += kIdxWarps) {
+        if (lane == 0) row_to_assign[r] = -1;
+        uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
+        for (int v = lane; v < vec_per_row; v += 32) dst[v] = make_uint4(0, 0, 0, 0);
+      }
     }
   }
 }
 
 // K2 ------------------------------------------------------------------------------------
-template <int UNROLL>
-__global__ void __launch_bounds__(256) perm_scatter_kernel(const __nv_bfloat16* __restrict__ X,
-                                                           const int32_t* __restrict__ ids,
-                                                           const int32_t* __restrict__ emap, int T, int k, int d,
-                                                           int E, int E_loc, int TPC, int align,
-                                                           const int32_t* __restrict__ hist,
-                                                           const int32_t* __restrict__ totals,
-                                                           const int32_t* __restrict__ offsets,
-                                                           int32_t* __restrict__ row_to_assign,
-                                                           int32_t* __restrict__ assign_to_row,
-                                                           __nv_bfloat16* __restrict__ Xp) {
-  __shared__ int s_run[kMaxSlots];     // next row of every slot for this chunk
-  __shared__ int s_dest[kMaxChunk];    // slot, then destination row, of every assignment of the chunk
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int b = blockIdx.x;
-  const int t0 = b * TPC, t1 = min(T, t0 + TPC);
-  const int lo = t0 * k, n_asg = (t1 - t0) * k;
+// One thread per VPT 16-byte vectors of one token row (vectors v and v + vpr/2 when VPT == 2):
+// the vector is read once and stored to each of the token's <= k destination rows.  The k
+// row indices are warp-uniform addresses (one broadcast transaction, L1-resident).  No
+// grid-stride loop: the grid covers T * vpr / VPT threads.
+template <int VPT>
+__global__ void __launch_bounds__(256) perm_rows_kernel(const __nv_bfloat16* __restrict__ X,
+                                                        const int32_t* __restrict__ assign_to_row, int T, int k,
+                                                        int d, __nv_bfloat16* __restrict__ Xp) {
   const int vpr = d >> 3;
-
-  for (int i = tid; i < n_asg; i += 256) s_dest[i] = slot_of(ids, emap, lo + i, E, E_loc);
-  for (int s = tid; s < E_loc; s += 256) s_run[s] = __ldg(offsets + s) + __ldg(hist + (size_t)b * E_loc + s);
-  __syncthreads();
-
-  // ---- first batch of row loads is in flight while warp 0 ranks ----
-  const int n_vec = (t1 - t0) * vpr;     // 16-byte vectors of this chunk's token rows
-  uint4 val[UNROLL];
-  const uint4* src0 = reinterpret_cast<const uint4*>(X + (size_t)t0 * d);
-  bool need[UNROLL];
+  const int per_row = vpr / VPT;
+  asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
+  const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (g >= (long long)T * per_row) return;
+  const int t = (int)(g / per_row);
+  const int v0 = (int)(g - (long long)t * per_row);
+  const int32_t* a2r = assign_to_row + (size_t)t * k;
+  bool any = false;
+  for (int j = 0; j < k; ++j) any |= (__ldg(a2r + j) >= 0);
+  if (!any) return;
+  const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)t * d) + v0;
+  uint4 val[VPT];
 #pragma unroll
-  for (int q = 0; q < UNROLL; ++q) {
-    const int v = tid + q * 256;
-    need[q] = false;
-    if (v < n_vec) {
-      const int tt = v / vpr;
-      for (int j = 0; j < k; ++j) need[q] |= (s_dest[tt * k + j] >= 0);
-      if (need[q]) val[q] = ld_nc_v4(src0 + v);
-    }
-  }
-  __syncthreads();   // every thread has read the slots it needs before warp 0 overwrites them
-
-  if (warp == 0) {
-    for (int i0 = 0; i0 < n_asg; i0 += 32) {
-      const int i = i0 + lane;
-      const int s = (i < n_asg) ? s_dest[i] : -1;
-      const unsigned peers = __match_any_sync(0xffffffffu, s);
-      int r = -1;
-      if (s >= 0) r = s_run[s] + __popc(peers & ((1u << lane) - 1u));
-      __syncwarp();
-      if (s >= 0 && (peers >> lane) == 1u) s_run[s] += __popc(peers);   // highest peer lane updates
-      __syncwarp();
-      if (i < n_asg) {
-        s_dest[i] = r;
-        assign_to_row[lo + i] = r;
-        if (r >= 0) row_to_assign[r] = lo + i;
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- copy rows: vector v of the chunk = (token v / vpr, vector v % vpr) ----
-  uint4* dst0 = reinterpret_cast<uint4*>(Xp);
-  for (int vb = 0; vb < n_vec; vb += 256 * UNROLL) {
-    if (vb > 0) {
+  for (int q = 0; q < VPT; ++q) val[q] = ld_nc_v4(src + q * per_row);
+  for (int j = 0; j < k; ++j) {
+    const int r = __ldg(a2r + j);
+    if (r < 0) continue;
+    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d) + v0;
 #pragma unroll
-      for (int q = 0; q < UNROLL; ++q) {
-        const int v = vb + tid + q * 256;
-        need[q] = false;
-        if (v < n_vec) {
-          const int tt = v / vpr;
-          for (int j = 0; j < k; ++j) need[q] |= (s_dest[tt * k + j] >= 0);
-          if (need[q]) val[q] = ld_nc_v4(src0 + v);
-        }
-      }
-    }
-#pragma unroll
-    for (int q = 0; q < UNROLL; ++q) {
-      const int v = vb + tid + q * 256;
-      if (v < n_vec && need[q]) {
-        const int tt = v / vpr;
-        const int vv = v - tt * vpr;
-        for (int j = 0; j < k; ++j) {
-          const int r = s_dest[tt * k + j];
-          if (r >= 0) st_na_v4(dst0 + (size_t)r * vpr + vv, val[q]);
-        }
-      }
-    }
-  }
-
-  // ---- padding rows (align > 1): index -1, zero activations ----
-  if (align > 1) {
-    for (int s = b; s < E_loc; s += gridDim.x) {
-      const int p0 = __ldg(offsets + s) + __ldg(totals + s), p1 = __ldg(offsets + s + 1);
-      for (int r = p0 + warp; r < p1; r += 8) {
-        if (lane == 0) row_to_assign[r] = -1;
-        uint4* dst = dst0 + (size_t)r * vpr;
-        for (int v = lane; v < vpr; v += 32) dst[v] = make_uint4(0, 0, 0, 0);
-      }
-    }
+    for (int q = 0; q < VPT; ++q) st_na_v4(dst + q * per_row, val[q]);
   }
 }
 
-struct Chunking {
-  int TPC, CH, NB;
-};
-Chunking chunking(int T, int k) {
-  Chunking c;
-  int tpc = (T + kTargetChunks - 1) / kTargetChunks;
-  if (tpc < 1) tpc = 1;
-  const int max_tpc = kMaxChunk / k > 0 ? kMaxChunk / k : 1;
-  if (tpc > max_tpc) tpc = max_tpc;
-  c.TPC = tpc;
-  c.CH = tpc * k;
-  c.NB = T > 0 ? (T + tpc - 1) / tpc : 1;
-  return c;
+// K2' -----------------------------------------------------------------------------------
+// Row-major variant for expert-parallel shards (E_loc < E), where only a fraction of the
+// T*k assignments is resident: persistent warps walk the R = offsets[E_loc] real rows
+// (extent read on the device) and copy X[row_to_assign[r] / k, :] -> Xp[r, :], UNROLL
+// independent 16-byte loads in flight per lane.  Work is proportional to R, not to T*k.
+template <int UNROLL>
+__global__ void __launch_bounds__(256) perm_rows_by_row_kernel(const __nv_bfloat16* __restrict__ X,
+                                                               const int32_t* __restrict__ row_to_assign,
+                                                               const int32_t* __restrict__ offsets, int E_loc,
+                                                               int k, int d, __nv_bfloat16* __restrict__ Xp) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
+  const int R = __ldg(offsets + E_loc);
+  const int lane = threadIdx.x & 31;
+  const int nwarps = gridDim.x * (256 / 32);
+  const int vpr = d >> 3;
+  for (int r = blockIdx.x * (256 / 32) + (threadIdx.x >> 5); r < R; r += nwarps) {
+    const int i = __ldg(row_to_assign + r);
+    if (i < 0) continue;   // padding row: already zero-filled by perm_index_kernel
+    const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)(i / k) * d);
+    uint4* dst = reinterpret_cast<uint4*>(Xp + (size_t)r * d);
+    for (int v0 = lane; v0 < vpr; v0 += 32 * UNROLL) {
+      uint4 val[UNROLL];
+#pragma unroll
+      for (int q = 0; q < UNROLL; ++q)
+        if (v0 + 32 * q < vpr) val[q] = ld_nc_v4(src + v0 + 32 * q);
+#pragma unroll
+      for (int q = 0; q < UNROLL; ++q)
+        if (v0 + 32 * q < vpr) st_na_v4(dst + v0 + 32 * q, val[q]);
+    }
+  }
 }
 
 }  // namespace
 
 size_t permute_ws_bytes(int T, int k, int E_loc) {
-  const Chunking c = chunking(T, k);
-  return round_up((size_t)c.NB * E_loc * sizeof(int32_t), 256) + round_up((size_t)E_loc * sizeof(int32_t), 256);
+  (void)T;
+  (void)k;
+  // [G][E_loc] table of CTA slot totals, G <= number of SMs
+  return round_up((size_t)num_sms() * E_loc * sizeof(int32_t), 256);
 }
 
 }  // namespace vibe
@@ -268,7 +337,6 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   VIBE_REQUIRE(d % 8 == 0, VIBE_ERR_INVALID_ARG, "vibe_permute: d %% 8 != 0 (rows must be 16-byte multiples)");
   VIBE_REQUIRE(align >= 1, VIBE_ERR_INVALID_ARG, "vibe_permute: align < 1");
   VIBE_REQUIRE(k <= E, VIBE_ERR_INVALID_ARG, "vibe_permute: k > E");
-  VIBE_REQUIRE(k <= kMaxChunk, VIBE_ERR_UNSUPPORTED, "vibe_permute: k > %d not implemented", kMaxChunk);
   VIBE_REQUIRE(E_loc <= E, VIBE_ERR_INVALID_ARG, "vibe_permute: E_loc > E");
   VIBE_REQUIRE(expert_map != nullptr || E_loc == E, VIBE_ERR_INVALID_ARG,
                "vibe_permute: expert_map NULL requires E_loc == E");
@@ -290,18 +358,54 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
     VIBE_CUDA(cudaMemsetAsync(offsets, 0, (size_t)(E_loc + 1) * sizeof(int32_t), st));
     return VIBE_OK;
   }
-  const Chunking c = chunking(T, k);
-  int32_t* hist = reinterpret_cast<int32_t*>(ws);
-  int32_t* totals = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) +
-                                               round_up((size_t)c.NB * E_loc * sizeof(int32_t), 256));
-  static std::atomic<unsigned> next_ticket{0};
-  const int ticket = (int)(next_ticket.fetch_add(1, std::memory_order_relaxed) % kTickets);
-  perm_count_kernel<<<c.NB, 1024, 0, st>>>(topk_ids, expert_map, A, E, E_loc, c.CH, c.NB, align, ticket, hist, totals,
-                                           offsets);
-  VIBE_LAUNCH_CHECK("perm_count_kernel");
-  perm_scatter_kernel<4><<<c.NB, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(X), topk_ids, expert_map, T, k,
-                                               d, E, E_loc, c.TPC, align, hist, totals, offsets, row_to_assign,
-                                               assign_to_row, reinterpret_cast<__nv_bfloat16*>(Xp));
-  VIBE_LAUNCH_CHECK("perm_scatter_kernel");
+  // K1: G CTAs, all co-resident (cooperative launch); WCH assignments per warp, a multiple of 32
+  int G = (A + kIdxThreads - 1) / kIdxThreads;
+  if (G > num_sms()) G = num_sms();
+  const int warps = G * kIdxWarps;
+  int WCH = (((A + warps - 1) / warps) + 31) / 32 * 32;
+  const size_t smem1 = (size_t)((kIdxWarps + 3) * E_loc + 1 + 2 * kIdxThreads) * sizeof(int);
+  static std::atomic<size_t> smem_set{0};
+  if (smem1 > 48 * 1024 && smem1 > smem_set.load()) {
+    VIBE_CUDA(cudaFuncSetAttribute(perm_index_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
+    smem_set.store(smem1);
+  }
+  static std::atomic<unsigned> next_slot{0};
+  int bar_slot = (int)(next_slot.fetch_add(1, std::memory_order_relaxed) % kBarSlots);
+  __nv_bfloat16* Xpb = reinterpret_cast<__nv_bfloat16*>(Xp);
+  int32_t* tbl = reinterpret_cast<int32_t*>(ws);
+  int A_ = A, E_ = E, El_ = E_loc, al_ = align, d_ = d;
+  void* args[] = {(void*)&topk_ids, (void*)&expert_map, &A_, &E_, &El_, &WCH, &al_, &d_, &bar_slot, &tbl, &offsets,
+                  &row_to_assign, &assign_to_row, &Xpb};
+  VIBE_CUDA(cudaLaunchCooperativeKernel((const void*)perm_index_kernel, dim3(G), dim3(kIdxThreads), args, smem1, st));
+  count_launch();
+  const int vpr = d / 8;
+  const __nv_bfloat16* Xb = reinterpret_cast<const __nv_bfloat16*>(X);
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t lc = {};
+  lc.blockDim = dim3(256);
+  lc.dynamicSmemBytes = 0;
+  lc.stream = st;
+  lc.attrs = pdl;
+  lc.numAttrs = 1;
+  const int32_t* r2a_c = row_to_assign;
+  const int32_t* a2r_c = assign_to_row;
+  const int32_t* off_c = offsets;
+  if (E_loc < E) {
+    // expert-parallel shard: work proportional to the resident rows
+    lc.gridDim = dim3(num_sms() * 8);
+    VIBE_CUDA(cudaLaunchKernelEx(&lc, perm_rows_by_row_kernel<4>, Xb, r2a_c, off_c, (int)E_loc, (int)k, (int)d, Xpb));
+  } else {
+    const int vpt = (vpr % 2 == 0) ? 2 : 1;
+    const long long blocks = ((long long)T * (vpr / vpt) + 255) / 256;
+    VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "vibe_permute: T*d too large for one launch");
+    lc.gridDim = dim3((unsigned)blocks);
+    if (vpt == 2)
+      VIBE_CUDA(cudaLaunchKernelEx(&lc, perm_rows_kernel<2>, Xb, a2r_c, (int)T, (int)k, (int)d, Xpb));
+    else
+      VIBE_CUDA(cudaLaunchKernelEx(&lc, perm_rows_kernel<1>, Xb, a2r_c, (int)T, (int)k, (int)d, Xpb));
+  }
+  VIBE_LAUNCH_CHECK("perm_rows_kernel");
   return VIBE_OK;
 }

@@ -78,11 +78,13 @@ def _dev_bf16(bits):
 STRESS = I.LayerConfig("S64K-stress", T=65536, d=2048, f=768, E=256, k=8, E_loc=256, zipf_s=1.0)
 
 
-def section_stages(peaks, quick):
+def section_stages(peaks, quick, only=None):
     """a1/a3/a5 in isolation, cold buffers."""
     out = []
     hbm = peaks["hbm_gbs"]
     for cfg in (I.C1, I.C2, I.C3, STRESS):
+        if only and cfg.name.split("-")[0] not in only:
+            continue
         T, k, E, E_loc, d = cfg.T, cfg.k, cfg.E, cfg.E_loc, cfg.d
         A = T * k
         Rcap = B.rows_cap(T, k, E_loc, 1)
@@ -253,6 +255,7 @@ def main():
     ap.add_argument("--sections", default="stages,ffn,profile,placement")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--configs", default="", help="stages section only: comma list out of C1,C2,C3,S64K")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("report: no CUDA device -- the product has no CPU fallback")
@@ -262,7 +265,7 @@ def main():
     rep = {"peaks": peaks, "gpu": torch.cuda.get_device_name(0)}
     want = args.sections.split(",")
     if "stages" in want:
-        rep["stages"] = section_stages(peaks, args.quick)
+        rep["stages"] = section_stages(peaks, args.quick, [c for c in args.configs.split(",") if c])
         for r in rep["stages"]:
             print(r["config"], {n: (r[n]["us"], r[n]["GB/s"], r[n]["frac_hbm"]) for n in ("route", "permute", "combine")},
                   flush=True)
