@@ -148,6 +148,24 @@ VIBE_API vibe_status vibe_combine(const void* Y, const int32_t* assign_to_row, c
                                   int32_t k, int32_t d, void* out, void* stream);
 
 /* ------------------------------------------------------------------------------------
+ * a4 + a5 fused ("gate-weighted scatter fused into the down projection", BJ:north_star).
+ * vibe_grouped_ffn_scatter computes the same FFN as vibe_grouped_ffn, but the epilogue of the
+ * down projection multiplies row r by the gate weight of its assignment i = row_to_assign[r]
+ * and stores it at row i of Yw -- Yw [T*k, d] bf16 is in ASSIGNMENT order:
+ *     Yw[i,:] = bf16( topk_w[i] * y(assign_to_row[i]) )        (one rounding of the product)
+ * Rows of non-resident assignments are NOT written.  vibe_combine_scattered then reduces k
+ * CONTIGUOUS rows per token:  out[t,:] = bf16( sum_{j: assign_to_row[t*k+j] >= 0} Yw[t*k+j,:] ),
+ * fp32, slot order.  Same layouts, ownership and errors as vibe_grouped_ffn / vibe_combine.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_grouped_ffn_scatter(const void* Xp, const int32_t* offsets, int32_t E_loc,
+                                              int32_t R_cap, int32_t d, int32_t f, const void* W1,
+                                              const void* W3, const void* W2, const int32_t* row_to_assign,
+                                              const float* topk_w, void* H_ws, void* Yw, void* ws,
+                                              size_t ws_bytes, void* stream);
+VIBE_API vibe_status vibe_combine_scattered(const void* Yw, const int32_t* assign_to_row, int32_t T, int32_t k,
+                                            int32_t d, void* out, void* stream);
+
+/* ------------------------------------------------------------------------------------
  * a6.  Per-expert latency profile: measured vibe_grouped_ffn time versus tokens per
  * expert, at warmed steady state -- "Each GPU is warmed to steady-state operating
  * conditions and profiled independently using the fused MoE kernel across a range of

@@ -35,6 +35,7 @@ EXPORTED_SYMBOLS = (
     "vibe_moe_layer_forward", "vibe_moe_layer_forward_host", "vibe_workspace_bytes", "vibe_rows_cap",
     "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
+    "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -99,6 +100,8 @@ def load() -> C.CDLL:
     lib.vibe_permute.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_grouped_ffn.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_combine.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
+    lib.vibe_grouped_ffn_scatter.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_combine_scattered.argtypes = [vp, vp, i32, i32, i32, vp, vp]
     lib.vibe_profile_expert_latency.argtypes = [i32, i32, i32, vp, vp, vp, C.POINTER(i32), i32, i32, i32, i32,
                                                 C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
     lib.vibe_moe_layer_forward.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
@@ -133,7 +136,8 @@ def load() -> C.CDLL:
     lib.vibe_drift_monitor_window_mean.argtypes = [vp, dp]
     lib.vibe_placement_swap_refine.argtypes = [C.POINTER(i32), dp, i32, i32, dp, C.POINTER(_LatencyModel), i32,
                                                C.c_double, i32, C.POINTER(i32), C.POINTER(i32)]
-    for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine",
+    for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_grouped_ffn_scatter",
+                 "vibe_combine_scattered",
                  "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
                  "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
@@ -245,6 +249,44 @@ def grouped_ffn(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: t
     _ok(lib.vibe_grouped_ffn(Xp.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1.data_ptr(), W3.data_ptr(),
                              W2.data_ptr(), H.data_ptr(), Y.data_ptr(), None, 0, _stream(stream)), "vibe_grouped_ffn")
     return Y, H
+
+
+def grouped_ffn_scatter(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: torch.Tensor,
+                        W2: torch.Tensor, row_to_assign: torch.Tensor, topk_w: torch.Tensor,
+                        H: Optional[torch.Tensor] = None, Yw: Optional[torch.Tensor] = None, stream=None):
+    """-> Yw bf16 [T*k, d] in assignment order, gate-weighted (rows of non-resident assignments untouched)"""
+    lib = load()
+    for t, n in ((Xp, "Xp"), (W1, "W1"), (W3, "W3"), (W2, "W2")):
+        _check(t, torch.bfloat16, n)
+    _check(offsets, torch.int32, "offsets")
+    _check(row_to_assign, torch.int32, "row_to_assign")
+    _check(topk_w, torch.float32, "topk_w")
+    Rcap, d = Xp.shape
+    E_loc, d1, f = W1.shape
+    if d1 != d or tuple(W3.shape) != (E_loc, d, f) or tuple(W2.shape) != (E_loc, f, d):
+        raise VibeError("weight shapes must be W1,W3 [E_loc,d,f], W2 [E_loc,f,d]")
+    if H is None:
+        H = torch.empty((Rcap, f), dtype=torch.bfloat16, device=Xp.device)
+    if Yw is None:
+        Yw = torch.empty((topk_w.numel(), d), dtype=torch.bfloat16, device=Xp.device)
+    _ok(lib.vibe_grouped_ffn_scatter(Xp.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1.data_ptr(),
+                                     W3.data_ptr(), W2.data_ptr(), row_to_assign.data_ptr(), topk_w.data_ptr(),
+                                     H.data_ptr(), Yw.data_ptr(), None, 0, _stream(stream)),
+        "vibe_grouped_ffn_scatter")
+    return Yw, H
+
+
+def combine_scattered(Yw: torch.Tensor, assign_to_row: torch.Tensor, T: int, k: int,
+                      out: Optional[torch.Tensor] = None, stream=None):
+    lib = load()
+    _check(Yw, torch.bfloat16, "Yw")
+    _check(assign_to_row, torch.int32, "assign_to_row")
+    d = Yw.shape[1]
+    if out is None:
+        out = torch.empty((T, d), dtype=torch.bfloat16, device=Yw.device)
+    _ok(lib.vibe_combine_scattered(Yw.data_ptr(), assign_to_row.data_ptr(), T, k, d, out.data_ptr(),
+                                   _stream(stream)), "vibe_combine_scattered")
+    return out
 
 
 # ------------------------------------------------------------------------------------ a5

@@ -28,7 +28,9 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 // branch (a warp never straddles tokens when vpr/VPT % 32 == 0; otherwise it merely diverges).
 // No grid-stride loop and no block barrier: the grid covers T * vpr / VPT threads and the
 // hardware scheduler keeps ~2048 threads x up to 4*VPT independent 16-byte loads in flight per SM.
-template <int VPT, bool K4>
+// SCAT: Y holds gate-weighted rows in ASSIGNMENT order (vibe_grouped_ffn_scatter): slot j of
+// token t reads row t*k + j with weight 1 when assign_to_row[t*k + j] >= 0 (topk_w unused).
+template <int VPT, bool K4, bool SCAT>
 __global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __restrict__ Y,
                                                       const int32_t* __restrict__ assign_to_row,
                                                       const float* __restrict__ topk_w, int T, int k, int d,
@@ -51,14 +53,23 @@ __global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __res
     float w[4];
     if (K4) {
       const int4 rr = __ldg(reinterpret_cast<const int4*>(a2r + j0));
-      const float4 ww = __ldg(reinterpret_cast<const float4*>(wt + j0));
       r[0] = rr.x; r[1] = rr.y; r[2] = rr.z; r[3] = rr.w;
-      w[0] = ww.x; w[1] = ww.y; w[2] = ww.z; w[3] = ww.w;
+      if (!SCAT) {
+        const float4 ww = __ldg(reinterpret_cast<const float4*>(wt + j0));
+        w[0] = ww.x; w[1] = ww.y; w[2] = ww.z; w[3] = ww.w;
+      }
     } else {
 #pragma unroll
       for (int jj = 0; jj < 4; ++jj) {
         r[jj] = (j0 + jj < k) ? __ldg(a2r + j0 + jj) : -1;
-        w[jj] = (j0 + jj < k) ? __ldg(wt + j0 + jj) : 0.0f;
+        if (!SCAT) w[jj] = (j0 + jj < k) ? __ldg(wt + j0 + jj) : 0.0f;
+      }
+    }
+    if (SCAT) {
+#pragma unroll
+      for (int jj = 0; jj < 4; ++jj) {
+        r[jj] = (r[jj] >= 0) ? t * k + j0 + jj : -1;
+        w[jj] = 1.0f;
       }
     }
     if ((r[0] & r[1] & r[2] & r[3]) < 0) continue;   // all four slots non-resident (sign bits)
@@ -95,34 +106,52 @@ __global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __res
 }  // namespace
 }  // namespace vibe
 
-extern "C" vibe_status vibe_combine(const void* Y, const int32_t* assign_to_row, const float* topk_w, int32_t T,
-                                    int32_t k, int32_t d, void* out, void* stream) {
-  using namespace vibe;
+namespace vibe {
+namespace {
+vibe_status combine_impl(const char* who, const void* Y, const int32_t* assign_to_row, const float* topk_w, int T,
+                         int k, int d, void* out, void* stream, bool scat) {
   clear_error();
-  VIBE_REQUIRE(T >= 0 && k >= 1 && d >= 8, VIBE_ERR_INVALID_ARG, "vibe_combine: bad sizes T=%d k=%d d=%d", T, k, d);
-  VIBE_REQUIRE(d % 8 == 0, VIBE_ERR_INVALID_ARG, "vibe_combine: d %% 8 != 0");
-  VIBE_REQUIRE(k <= 32, VIBE_ERR_UNSUPPORTED, "vibe_combine: k > 32 not implemented (vibe_route_topk limit)");
+  VIBE_REQUIRE(T >= 0 && k >= 1 && d >= 8, VIBE_ERR_INVALID_ARG, "%s: bad sizes T=%d k=%d d=%d", who, T, k, d);
+  VIBE_REQUIRE(d % 8 == 0, VIBE_ERR_INVALID_ARG, "%s: d %% 8 != 0", who);
+  VIBE_REQUIRE(k <= 32, VIBE_ERR_UNSUPPORTED, "%s: k > 32 not implemented (vibe_route_topk limit)", who);
   if (T == 0) return VIBE_OK;
-  VIBE_REQUIRE(Y && assign_to_row && topk_w && out, VIBE_ERR_INVALID_ARG, "vibe_combine: NULL tensor");
-  VIBE_REQUIRE(aligned16(Y) && aligned16(out), VIBE_ERR_INVALID_ARG, "vibe_combine: Y / out must be 16-byte aligned");
+  VIBE_REQUIRE(Y && assign_to_row && (scat || topk_w) && out, VIBE_ERR_INVALID_ARG, "%s: NULL tensor", who);
+  VIBE_REQUIRE(aligned16(Y) && aligned16(out), VIBE_ERR_INVALID_ARG, "%s: Y / out must be 16-byte aligned", who);
+  VIBE_REQUIRE((int64_t)T * k < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG, "%s: T*k >= 2^31", who);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const int vpr = d / 8;
   const __nv_bfloat16* Yb = reinterpret_cast<const __nv_bfloat16*>(Y);
   __nv_bfloat16* ob = reinterpret_cast<__nv_bfloat16*>(out);
   const int vpt = (vpr % 2 == 0) ? 2 : 1;
-  const bool k4 = (k % 4 == 0) && aligned16(assign_to_row) && aligned16(topk_w);
+  const bool k4 = (k % 4 == 0) && aligned16(assign_to_row) && (scat || aligned16(topk_w));
   const long long threads = (long long)T * (vpr / vpt);
   const long long blocks = (threads + 255) / 256;
-  VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "vibe_combine: T*d too large for one launch");
+  VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "%s: T*d too large for one launch", who);
   const unsigned gb = (unsigned)blocks;
-  if (vpt == 2 && k4)
-    combine_kernel<2, true><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
-  else if (vpt == 2)
-    combine_kernel<2, false><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
-  else if (k4)
-    combine_kernel<1, true><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
-  else
-    combine_kernel<1, false><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
+#define VIBE_COMBINE_CASE(V, K, S)                                                              \
+  if (vpt == V && k4 == K && scat == S)                                                         \
+    combine_kernel<V, K, S><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
+  VIBE_COMBINE_CASE(2, true, false)
+  VIBE_COMBINE_CASE(2, false, false)
+  VIBE_COMBINE_CASE(1, true, false)
+  VIBE_COMBINE_CASE(1, false, false)
+  VIBE_COMBINE_CASE(2, true, true)
+  VIBE_COMBINE_CASE(2, false, true)
+  VIBE_COMBINE_CASE(1, true, true)
+  VIBE_COMBINE_CASE(1, false, true)
+#undef VIBE_COMBINE_CASE
   VIBE_LAUNCH_CHECK("combine_kernel");
   return VIBE_OK;
+}
+}  // namespace
+}  // namespace vibe
+
+extern "C" vibe_status vibe_combine(const void* Y, const int32_t* assign_to_row, const float* topk_w, int32_t T,
+                                    int32_t k, int32_t d, void* out, void* stream) {
+  return vibe::combine_impl("vibe_combine", Y, assign_to_row, topk_w, T, k, d, out, stream, false);
+}
+
+extern "C" vibe_status vibe_combine_scattered(const void* Yw, const int32_t* assign_to_row, int32_t T, int32_t k,
+                                              int32_t d, void* out, void* stream) {
+  return vibe::combine_impl("vibe_combine_scattered", Yw, assign_to_row, nullptr, T, k, d, out, stream, true);
 }

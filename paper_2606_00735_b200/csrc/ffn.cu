@@ -107,11 +107,43 @@ __device__ __forceinline__ void store_block_T(const float (&v)[32], __nv_bfloat1
   }
 }
 
-template <bool kGateUp>
+// The same block, gate-weighted and scattered: token i of the block (permuted row row0 + i)
+// goes to row row_to_assign[row0 + i] of `out` (assignment order) scaled by that assignment's
+// gate weight; the product is rounded to bf16 once.  Lane L fetches (destination, weight) of
+// token L; the store loop reads them with shuffles.
+__device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv_bfloat16* __restrict__ out,
+                                                      size_t ld, int row0, int n_rows, int feat, bool feat_ok,
+                                                      int lane, const int32_t* __restrict__ row_to_assign,
+                                                      const float* __restrict__ topk_w) {
+  int asg = -1;
+  float wt = 0.0f;
+  if (lane < n_rows) {
+    asg = __ldg(row_to_assign + row0 + lane);
+    if (asg >= 0) wt = __ldg(topk_w + asg);
+  }
+  const bool odd = lane & 1;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    const float send = odd ? v[i] : v[i + 1];
+    const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
+    const int tok = i + (odd ? 1 : 0);
+    const int dst = __shfl_sync(0xffffffffu, asg, tok);
+    const float w = __shfl_sync(0xffffffffu, wt, tok);
+    const uint32_t pk = odd ? pack2_bf16(recv * w, v[i + 1] * w) : pack2_bf16(v[i] * w, recv * w);
+    if (feat_ok && dst >= 0)
+      *reinterpret_cast<uint32_t*>(out + (size_t)dst * ld + (feat - (odd ? 1 : 0))) = pk;
+  }
+}
+
+// kMode: 0 = gate|up + SwiGLU (GEMM-1), 1 = down (GEMM-2), 2 = down with the gate-weighted
+// scatter fused into the epilogue (vibe_grouped_ffn_scatter).
+template <int kMode>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
                 const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
-                int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out) {
+                int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out,
+                const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w) {
+  constexpr bool kGateUp = (kMode == 0);
   constexpr int FB = kGateUp ? 128 : 256;   // output features per pair tile
   constexpr int FC = FB / 2;                // ... per CTA
   extern __shared__ uint8_t smem_raw[];
@@ -312,7 +344,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
           float v[32];
 #pragma unroll
           for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]);
-          store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+          if (kMode == 2)
+            store_block_T_scatter(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane, row_to_assign,
+                                  topk_w);
+          else
+            store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
         }
       }
       ptx::tc_fence_before();
@@ -413,7 +449,7 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
 
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y,
-                             cudaStream_t st) {
+                             cudaStream_t st, const int32_t* row_to_assign, const float* topk_w) {
   CUtensorMap tmX, tmH, tmW1, tmW3, tmW2;
   vibe_status s;
   if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
@@ -424,20 +460,25 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   static std::once_flag once;
   static cudaError_t attr_err = cudaSuccess;
   std::call_once(once, [] {
-    attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)SMEM_BYTES);
+    attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
     if (attr_err == cudaSuccess)
-      attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)SMEM_BYTES);
+      attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    if (attr_err == cudaSuccess)
+      attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
   });
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn_gemm_kernel<true><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
-                                                               reinterpret_cast<__nv_bfloat16*>(H_ws), f);
+  ffn_gemm_kernel<0><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
+                                                            reinterpret_cast<__nv_bfloat16*>(H_ws), f, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
-  ffn_gemm_kernel<false><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
-                                                                reinterpret_cast<__nv_bfloat16*>(Y), d);
+  if (row_to_assign != nullptr)
+    ffn_gemm_kernel<2><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+                                                              reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign,
+                                                              topk_w);
+  else
+    ffn_gemm_kernel<1><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+                                                              reinterpret_cast<__nv_bfloat16*>(Y), d, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
 }
@@ -467,5 +508,20 @@ extern "C" vibe_status vibe_grouped_ffn(const void* Xp, const int32_t* offsets, 
   vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Y);
   if (s != VIBE_OK) return s;
   return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Y,
-                          reinterpret_cast<cudaStream_t>(stream));
+                          reinterpret_cast<cudaStream_t>(stream), nullptr, nullptr);
+}
+
+extern "C" vibe_status vibe_grouped_ffn_scatter(const void* Xp, const int32_t* offsets, int32_t E_loc, int32_t R_cap,
+                                                int32_t d, int32_t f, const void* W1, const void* W3,
+                                                const void* W2, const int32_t* row_to_assign, const float* topk_w,
+                                                void* H_ws, void* Yw, void* ws, size_t ws_bytes, void* stream) {
+  using namespace vibe;
+  (void)ws;
+  (void)ws_bytes;
+  clear_error();
+  vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Yw);
+  if (s != VIBE_OK) return s;
+  VIBE_REQUIRE(row_to_assign && topk_w, VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_scatter: NULL row_to_assign / topk_w");
+  return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Yw,
+                          reinterpret_cast<cudaStream_t>(stream), row_to_assign, topk_w);
 }

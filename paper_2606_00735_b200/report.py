@@ -1,6 +1,6 @@
 """Per-kernel measurements on one B200 beyond the single bench.py line.
 
-    python -m paper_2606_00735_b200.report [--sections stages,ffn,profile,placement]
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,profile,placement]
                                            [--out gpurun_out/report.json] [--quick]
 
 Sections (all through the C-ABI binding; seeded synthetic inputs):
@@ -11,6 +11,8 @@ Sections (all through the C-ABI binding; seeded synthetic inputs, DESIGN.md sect
   ffn        grouped FFN on BALANCED routing (every expert n rows), n = 128..4096, for the
              C1/C2/C3 shapes: TFLOP/s and fraction of the measured bf16 peaks -- the
              ">= 512 tokens per expert" target of BASELINE.json is read off this table.
+  fused      vibe_grouped_ffn + vibe_combine versus the fused gate-weighted scatter path
+             (vibe_grouped_ffn_scatter + vibe_combine_scattered) on the routed C1 / C2 batches.
   profile    vibe_profile_expert_latency over the M3 sweep (1..4096 tokens per expert), modes 0
              and 1, for the C2 and C3 shapes: the per-GPU performance model f(n) of the paper
              (PAPER.md L176).  Written as CSV rows into the JSON and to <out>.profile.csv.
@@ -155,6 +157,45 @@ def section_stages(peaks, quick, only=None):
     return out
 
 
+def section_fused(peaks, quick):
+    """a4+a5: vibe_grouped_ffn + vibe_combine versus vibe_grouped_ffn_scatter + vibe_combine_scattered
+    (gate-weighted scatter fused into the down projection) on the routed C1 / C2 batches."""
+    out = []
+    for cfg in (I.C1, I.C2):
+        T, k, E, d, f = cfg.T, cfg.k, cfg.E, cfg.d, cfg.f
+        W1, W3, W2 = _weights(E, d, f)
+        rc = B.RouteConfig(**I.route_kwargs(cfg))
+        lg = torch.from_numpy(I.make_logits(T, E, cfg.zipf_s, 0, cfg.alpha)).cuda()
+        X = torch.randn((T, d), device="cuda").to(torch.bfloat16)
+        ids, w, counts = B.route_topk(lg, rc)
+        Xp, off, r2a, a2r = B.permute(X, ids, counts, None, E, E, 1)
+        H = torch.empty((Xp.shape[0], f), dtype=torch.bfloat16, device="cuda")
+        Y = torch.empty_like(Xp)
+        Yw = torch.empty((T * k, d), dtype=torch.bfloat16, device="cuda")
+        o = torch.empty((T, d), dtype=torch.bfloat16, device="cuda")
+
+        def plain(i):
+            B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y)
+            B.combine(Y, a2r, w, T, k, out=o)
+
+        def fused(i):
+            B.grouped_ffn_scatter(Xp, off, W1, W3, W2, r2a, w, H=H, Yw=Yw)
+            B.combine_scattered(Yw, a2r, T, k, out=o)
+
+        t0 = time.time()
+        while time.time() - t0 < (0.3 if quick else 1.5):
+            plain(0)
+            torch.cuda.synchronize()
+        iters = 20 if quick else 100
+        tp = _time(plain, iters)
+        tf = _time(fused, iters)
+        out.append({"config": cfg.name, "ffn_plus_combine_us": round(tp, 2), "fused_scatter_us": round(tf, 2),
+                    "speedup": round(tp / tf, 4)})
+        del W1, W3, W2
+        torch.cuda.empty_cache()
+    return out
+
+
 def _weights(E, d, f):
     W1 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
     W3 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
@@ -177,7 +218,10 @@ def section_ffn(peaks, quick):
         E, d, f = cfg.E_loc, cfg.d, cfg.f
         W1, W3, W2 = _weights(E, d, f)
         _warm(W1, W3, W2, 0.5 if quick else 2.0)
-        lat = B.profile_expert_latency(W1, W3, W2, sweep, mode=0, warmup=5, iters=20 if quick else 50)
+        # largest point first: the sweep starts in the power-capped steady state the warm loop left, and
+        # every point gets enough untimed calls to ride out the DVFS transient of a change in intensity
+        lat = B.profile_expert_latency(W1, W3, W2, sweep[::-1], mode=0, warmup=10 if quick else 30,
+                                       iters=20 if quick else 50)[::-1]
         for n, l in zip(sweep, lat):
             tf = 6.0 * n * d * f / l / 1e6
             bytes_e = 6.0 * d * f + 4.0 * n * d + 4.0 * n * f
@@ -200,8 +244,10 @@ def section_profile(peaks, quick):
         _warm(W1, W3, W2, 0.5 if quick else 2.0)
         rows = []
         for mode in (0, 1):
-            lat, samples = B.profile_expert_latency(W1, W3, W2, B.DEFAULT_SWEEP, mode=mode, warmup=10,
-                                                    iters=20 if quick else 100, return_samples=True)
+            lat, samples = B.profile_expert_latency(W1, W3, W2, B.DEFAULT_SWEEP[::-1], mode=mode,
+                                                    warmup=10 if quick else 30, iters=20 if quick else 100,
+                                                    return_samples=True)
+            lat, samples = lat[::-1], samples[::-1]      # measured from the largest point down (steady state)
             if mode == 0:
                 samples = samples / E
             for j, n in enumerate(B.DEFAULT_SWEEP):
@@ -252,7 +298,7 @@ def section_placement(peaks, quick, profile):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--sections", default="stages,ffn,profile,placement")
+    ap.add_argument("--sections", default="stages,ffn,fused,profile,placement")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--configs", default="", help="stages section only: comma list out of C1,C2,C3,S64K")
@@ -273,6 +319,10 @@ def main():
         rep["ffn_balanced"] = section_ffn(peaks, args.quick)
         for r in rep["ffn_balanced"]:
             print(r["shape"], r["tokens_per_expert"], r["us_per_expert"], r["TFLOP/s"], r["frac_sustained"], flush=True)
+    if "fused" in want:
+        rep["fused_scatter"] = section_fused(peaks, args.quick)
+        for r in rep["fused_scatter"]:
+            print(r, flush=True)
     if "profile" in want:
         rep["profile"] = section_profile(peaks, args.quick)
     if "placement" in want:
