@@ -107,20 +107,13 @@ __device__ __forceinline__ void store_block_T(const float (&v)[32], __nv_bfloat1
   }
 }
 
-// The same block, gate-weighted and scattered: token i of the block (permuted row row0 + i)
-// goes to row row_to_assign[row0 + i] of `out` (assignment order) scaled by that assignment's
-// gate weight; the product is rounded to bf16 once.  Lane L fetches (destination, weight) of
-// token L; the store loop reads them with shuffles.
+// The same block, gate-weighted and scattered: token i of the block goes to row asg (its flat
+// assignment index, assignment order) of `out`, scaled by that assignment's gate weight wt; the
+// product is rounded to bf16 once.  Lane L holds (asg, wt) of token L of the block -- fetched
+// for the whole tile before the accumulator is ready, so no global latency sits in this loop.
 __device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv_bfloat16* __restrict__ out,
-                                                      size_t ld, int row0, int n_rows, int feat, bool feat_ok,
-                                                      int lane, const int32_t* __restrict__ row_to_assign,
-                                                      const float* __restrict__ topk_w) {
-  int asg = -1;
-  float wt = 0.0f;
-  if (lane < n_rows) {
-    asg = __ldg(row_to_assign + row0 + lane);
-    if (asg >= 0) wt = __ldg(topk_w + asg);
-  }
+                                                      size_t ld, int feat, bool feat_ok, int lane, int asg,
+                                                      float wt) {
   const bool odd = lane & 1;
 #pragma unroll
   for (int i = 0; i < 32; i += 2) {
@@ -302,6 +295,19 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       const int n_rows = min(TN, tail->off[e + 1] - row0);
       const int acc = it & 1;
       const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
+      // fused scatter: destination row and gate weight of this tile's tokens, lane L of block b
+      // holds token 32*b + L; loaded while the MMAs of the tile are still running
+      int sc_asg[kMode == 2 ? TN / 32 : 1];
+      float sc_wt[kMode == 2 ? TN / 32 : 1];
+      if (kMode == 2) {
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) {
+          const int c = b * 32 + lane;
+          sc_asg[b] = (c < n_rows) ? __ldg(row_to_assign + row0 + c) : -1;
+        }
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) sc_wt[b] = (sc_asg[b] >= 0) ? __ldg(topk_w + sc_asg[b]) : 0.0f;
+      }
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
@@ -337,7 +343,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       } else {
         const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
         const bool feat_ok = feat < n_total;
-        for (int c0 = 0; c0 < n_rows; c0 += 32) {
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) {
+          const int c0 = b * 32;
+          if (c0 >= n_rows) break;
           uint32_t a[32];
           ptx::tmem_ld_32x32(taddr + c0, a);
           ptx::tmem_ld_wait();
@@ -345,8 +354,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 #pragma unroll
           for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]);
           if (kMode == 2)
-            store_block_T_scatter(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane, row_to_assign,
-                                  topk_w);
+            store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_asg[kMode == 2 ? b : 0],
+                                  sc_wt[kMode == 2 ? b : 0]);
           else
             store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
         }
