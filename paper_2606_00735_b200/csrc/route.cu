@@ -196,32 +196,55 @@ __global__ void __launch_bounds__(256) route_topk_kernel(const RouteParams p) {
       }
     }
     // ---- k rounds of arg-max, ties -> lowest index (R3) ----
-    int my_id = 0;
-    float my_x = 0.0f;
-    for (int j = 0; j < k; ++j) {
-      uint32_t lm = uk[0];
+    // Pick order = (key descending, expert index ascending).  Every lane keeps the FIRST TWO of its
+    // not-yet-picked experts in that order (m1/v1, m2/v2) and the last one it gave away (lk/lv); a
+    // round is then redux-max over the lane heads + ballot (lowest lane = lowest index among equal
+    // keys) + a pop in the winner -- no scan of the VPL registers.  A lane that has given away both
+    // of its candidates rebuilds them from its registers ("strictly after (lk, lv) in pick order");
+    // with VPL experts per lane that happens about once per token.
+    uint32_t lk = 0xffffffffu, m1 = kTaken, m2 = kTaken;
+    int lv = -1, v1 = 0, v2 = 0;
 #pragma unroll
-      for (int v = 1; v < VPL; ++v) lm = max(lm, uk[v]);
-      const uint32_t gm = group_max_u32<LANES>(gmask, lm);
-      const unsigned b = __ballot_sync(gmask, lm == gm) & gmask;
+    for (int v = 0; v < VPL; ++v) {             // first fill: everything is eligible
+      const uint32_t c = uk[v];
+      if (c > m1) { m2 = m1; v2 = v1; m1 = c; v1 = v; }
+      else if (c > m2) { m2 = c; v2 = v; }
+    }
+    bool dry = false;                            // this lane has no expert left at all
+    int my_id = 0;
+    uint32_t my_key = 0;
+    for (int j = 0; j < k; ++j) {
+      const uint32_t gm = group_max_u32<LANES>(gmask, m1);
+      const unsigned b = __ballot_sync(gmask, m1 == gm) & gmask;
       const int win = __ffs(b) - 1;
-      int id_local = 0;
-      float xv = 0.0f;
-      if (lane == win) {
-        bool found = false;
+      const int id = __shfl_sync(gmask, e0 + v1, win);
+      if (sub == j) { my_id = id; my_key = gm; }
+      const bool iw = (lane == win);
+      lk = iw ? m1 : lk;
+      lv = iw ? v1 : lv;
+      m1 = iw ? m2 : m1;
+      v1 = iw ? v2 : v1;
+      m2 = iw ? kTaken : m2;
+      const bool need = (m1 == kTaken) && !dry;
+      if (__any_sync(gmask, need)) {
+        m1 = kTaken; m2 = kTaken; v1 = 0; v2 = 0;
 #pragma unroll
         for (int v = 0; v < VPL; ++v) {
-          if (!found && uk[v] == gm) {
-            id_local = e0 + v;
-            xv = x[v];
-            uk[v] = kTaken;
-            found = true;
-          }
+          const uint32_t c0 = uk[v];
+          const bool elig = (c0 < lk) || (c0 == lk && v > lv);
+          const uint32_t c = elig ? c0 : kTaken;
+          if (c > m1) { m2 = m1; v2 = v1; m1 = c; v1 = v; }
+          else if (c > m2) { m2 = c; v2 = v; }
         }
+        dry = (m1 == kTaken);
       }
-      const int id = __shfl_sync(gmask, id_local, win);
-      const float xs = __shfl_sync(gmask, xv, win);
-      if (sub == j) { my_id = id; my_x = xs; }
+    }
+    // the picked expert's logit: for softmax the key IS the logit (-0 arrives as +0, same exp);
+    // for sigmoid it is read back from the row (an L1/L2 hit, one load per pick)
+    float my_x = 0.0f;
+    if (sub < k) {
+      if (SIGMOID) my_x = __ldg(row + my_id);
+      else my_x = __uint_as_float((my_key & 0x80000000u) ? (my_key & 0x7fffffffu) : ~my_key);
     }
     // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
     double wj = 0.0;
