@@ -296,11 +296,60 @@ def section_placement(peaks, quick, profile):
     return out
 
 
+def write_markdown(r, path, command):
+    """The JSON report as markdown tables (what profiles/r1_report.md holds)."""
+    import collections
+    import statistics as st
+    o=[]
+    o.append("# r1: per-kernel measurements on one B200 (`python -m paper_2606_00735_b200.report`)\n")
+    o.append("Command (under gpurun, one B200, no profiler attached):\n\n    " + command + "\n")
+    o.append(f"Peaks ({r['peaks']['kind']}, MEASURED_PEAKS.json): HBM copy {r['peaks']['hbm_gbs']} GB/s; cuBLAS bf16 {r['peaks']['bf16_tflops']} TFLOP/s burst, {r['peaks']['bf16_tflops_sustained']} sustained.  GPU: {r['gpu']}.\n")
+    o.append("## stages: route / permute / combine, each timed alone from a CUDA graph over rotating cold buffer sets\n")
+    o.append("achieved = algorithmic bytes (DESIGN.md section 7) / device time; `frac` = achieved / measured HBM copy peak.\n")
+    o.append("| config | T | E (resident) | k | d | real rows | route us | GB/s | frac | permute us | GB/s | frac | combine us | GB/s | frac |")
+    o.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for s in r['stages']:
+        o.append(f"| {s['config']} | {s['T']} | {s['E']} ({s['E_loc']}) | {s['k']} | {s['d']} | {s['real_rows']} | "+" | ".join(f"{s[n]['us']} | {s[n]['GB/s']} | {s[n]['frac_hbm']}" for n in ('route','permute','combine'))+" |")
+    o.append("\nRoute is issue-bound, not HBM-bound (`r1_route_s64k_ncu.md`); permute = 2 launches (cooperative index kernel + row kernel), combine = 1.\n")
+    o.append("## ffn_balanced: grouped FFN, every expert n rows (vibe_profile_expert_latency mode 0, largest n first, 2 s warm loop)\n")
+    o.append("| shape | E_loc | d | f | tokens/expert | us/expert | TFLOP/s | of sustained | of burst | of per-expert roofline max(flops/sustained, bytes/HBM) |")
+    o.append("|---|---|---|---|---|---|---|---|---|---|")
+    for x in r['ffn_balanced']:
+        o.append(f"| {x['shape']} | {x['E_loc']} | {x['d']} | {x['f']} | {x['tokens_per_expert']} | {x['us_per_expert']} | {x['TFLOP/s']} | {x['frac_sustained']} | {x['frac_burst']} | {x['frac_of_per_expert_roofline']} |")
+    o.append("\n## fused_scatter: vibe_grouped_ffn + vibe_combine vs vibe_grouped_ffn_scatter + vibe_combine_scattered (routed batches)\n")
+    o.append("| config | ffn + combine us | fused scatter us | speedup |\n|---|---|---|---|")
+    for x in r['fused_scatter']:
+        o.append(f"| {x['config']} | {x['ffn_plus_combine_us']} | {x['fused_scatter_us']} | {x['speedup']} |")
+    o.append("\n## profile: per-expert latency l(n) [us], median of 100 calls per point (p10..p90), modes 0 (all experts n rows; time / E_loc) and 1 (one expert n rows)\n")
+    for name,p in r['profile'].items():
+        o.append(f"### {name}: E_loc={p['E_loc']} d={p['d']} f={p['f']}\n")
+        o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 |\n|---|---|---|---|---|---|---|---|")
+        m0={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==0}
+        m1={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==1}
+        for n in sorted(m0):
+            a,b=m0[n],m1[n]
+            o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} |")
+        o.append("")
+    o.append("## placement_stress (BASELINE.json configs[4]): 256 experts -> 8 virtual GPUs, sigma ~ U[0.78,1.0] (8 seeds), measured C3-shape profile\n")
+    o.append("score = max over bins of modelled latency / sigma [us]; gain = 1 - latency-balanced / token-balanced.  Medians over the 8 scale draws.\n")
+    o.append("| zipf s | T | cap | model | contiguous | token-balanced | latency-balanced (ViBE) | gain vs token-balanced (median, min..max) | gain vs contiguous (median) |")
+    o.append("|---|---|---|---|---|---|---|---|---|")
+    g=collections.defaultdict(list)
+    for x in r['placement_stress']: g[(x['zipf_s'],x['T'],x['cap'],x['model'])].append(x)
+    for k_,v in sorted(g.items()):
+        med=lambda f: round(st.median(f(y) for y in v),2)
+        gt=[y['gain_latency_vs_token'] for y in v]
+        o.append(f"| {k_[0]} | {k_[1]} | {k_[2]} | {k_[3]} | {med(lambda y:y['contiguous']['score_us'])} | {med(lambda y:y['token_balanced']['score_us'])} | {med(lambda y:y['latency_balanced']['score_us'])} | {round(st.median(gt),4)} ({min(gt)}..{max(gt)}) | {med(lambda y:y['gain_latency_vs_contiguous'])} |")
+    with open(path, "w") as fh:
+        fh.write("\n".join(o) + "\n")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sections", default="stages,ffn,fused,profile,placement")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--md", default="", help="also write the report as markdown tables (needs all sections)")
     ap.add_argument("--configs", default="", help="stages section only: comma list out of C1,C2,C3,S64K")
     args = ap.parse_args()
     if not torch.cuda.is_available():
@@ -339,6 +388,8 @@ def main():
             for name, p in rep["profile"].items():
                 for r in p["rows"]:
                     fh.write(f"{name},{r['mode']},{r['tokens_per_expert']},{r['latency_us']},{r['p10_us']},{r['p90_us']}\n")
+    if args.md:
+        write_markdown(rep, args.md, "python -m paper_2606_00735_b200.report " + " ".join(sys.argv[1:]))
     print("wrote", args.out)
 
 
