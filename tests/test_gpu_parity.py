@@ -189,6 +189,39 @@ def test_permute_edge_cases():
     assert off.cpu().tolist() == [0] * 9
 
 
+def test_permute_full_grid_max_slots_and_barrier_slot_reuse():
+    """The cooperative index kernel at its limits: more assignments than 148 x 1024 threads (several
+    batches per warp), the maximum number of slots (1024, 147 KB of shared memory), and 150 calls in a
+    row -- more than twice the 64 round-robin grid-barrier slots -- each checked bit for bit."""
+    rng = I._rng(11, 11)
+    # A = 400 000 > 148 * 1024: every CTA of the grid works, warps own 96 assignments
+    T, k, E = 50000, 8, 64
+    ids = np.argsort(rng.random((T, E)), axis=1)[:, :k].astype(np.int32)       # k distinct experts per token
+    check_permute(I.make_X(T, 32, 3), ids, None, E, E, 1)
+    # 1024 slots, an expert map with holes, padding to 16
+    T, k, E = 3000, 4, 2048
+    ids = np.argsort(rng.random((T, 64)), axis=1)[:, :k].astype(np.int32) * 32 + rng.integers(0, 32, (T, k)).astype(np.int32)
+    emap = np.full(E, -1, np.int32)
+    res = rng.permutation(E)[:1024]
+    emap[res] = rng.permutation(1024).astype(np.int32)
+    check_permute(I.make_X(T, 64, 4), ids, emap, E, 1024, 16)
+    # barrier slots are recycled: 150 back-to-back calls on two alternating inputs
+    Xa, Xb = I.make_X(700, 128, 5), I.make_X(900, 128, 6)
+    ia = np.argsort(rng.random((700, 16)), axis=1)[:, :2].astype(np.int32)
+    ib = np.argsort(rng.random((900, 16)), axis=1)[:, :3].astype(np.int32)
+    ref = [O.permute(Xa, ia, None, 16, 1), O.permute(Xb, ib, None, 16, 1)]
+    dX, dI = [dev_bf16(Xa), dev_bf16(Xb)], [dev(ia), dev(ib)]
+    outs = []
+    for it in range(150):
+        outs.append(B.permute(dX[it & 1], dI[it & 1], None, None, 16, 16, 1))
+    torch.cuda.synchronize()
+    for it in (0, 1, 63, 64, 65, 127, 128, 129, 148, 149):
+        Xp, off, r2a, a2r = outs[it]
+        off_o, r2a_o, a2r_o, Xp_o, R = ref[it & 1]
+        assert np.array_equal(off.cpu().numpy(), off_o) and np.array_equal(a2r.cpu().numpy(), a2r_o), it
+        assert np.array_equal(r2a.cpu().numpy()[:R], r2a_o[:R]) and np.array_equal(host_bits(Xp)[:R], Xp_o[:R]), it
+
+
 # =========================================================================== a4
 def ffn_case(cfg, seed, align=1, policy="contiguous", balanced=False):
     L = I.make_layer(cfg, seed, map_policy=policy)
