@@ -1,6 +1,6 @@
 """Per-kernel measurements on one B200 beyond the single bench.py line.
 
-    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,profile,placement]
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,profile,placement,variability,rack,recalibration]
                                            [--out gpurun_out/report.json] [--quick]
 
 Sections (all through the C-ABI binding; seeded synthetic inputs):
@@ -21,6 +21,11 @@ Sections (all through the C-ABI binding; seeded synthetic inputs, DESIGN.md sect
              {0.8,1.2,1.6} x T in {2K,16K,64K}; contiguous vs token-balanced vs latency-balanced
              (ViBE Alg. 1 phase 2) under the measured C3-shape profile, model kinds A and B,
              cap = 32 and cap = 0.
+  variability    1000 consecutive executions at 4K tokens per expert on this device: time per
+                 execution from a cold start into the power-capped steady state, SM clock and power alongside.
+  rack           rack-scale projection: the three policies for G = 8..128 virtual GPUs.
+  recalibration  drift monitor + Algorithm 2 on a routing distribution that drifts: when it fires, how many
+                 swaps repair the placement versus how many experts a full re-solve moves.
 
 Everything here calls the CUDA library; nothing imports oracle/.
 """
@@ -264,11 +269,7 @@ def section_profile(peaks, quick):
 
 def section_placement(peaks, quick, profile):
     """BASELINE.json configs[4] on the measured C3-shape profile (mode 0)."""
-    if profile is None:
-        profile = section_profile(peaks, True)
-    prof = [r for r in profile[I.C3.name]["rows"] if r["mode"] == 0]
-    model = B.LatencyModel([r["tokens_per_expert"] for r in prof], [r["latency_us"] for r in prof],
-                           E_prof=profile[I.C3.name]["E_loc"])
+    model, _ = _c3_model(peaks, profile)
     E, G, k = 256, 8, 8
     rc = B.RouteConfig(num_experts=E, top_k=k)
     out = []
@@ -296,6 +297,132 @@ def section_placement(peaks, quick, profile):
     return out
 
 
+def _c3_model(peaks, profile):
+    if profile is None:
+        profile = section_profile(peaks, True)
+    prof = [r for r in profile[I.C3.name]["rows"] if r["mode"] == 0]
+    return B.LatencyModel([r["tokens_per_expert"] for r in prof], [r["latency_us"] for r in prof],
+                          E_prof=profile[I.C3.name]["E_loc"]), profile
+
+
+def section_variability(peaks, quick):
+    """The paper's variability protocol on THIS device: "4K tokens per expert ... 1000 consecutive MoE
+    layer executions" under perfect balance, C3 shape: per-execution kernel time and the
+    SM clock over the run -- how much one GPU's own DVFS moves f(n) between a cold start and steady state."""
+    cfg = I.C3
+    E, d, f = cfg.E_loc, cfg.d, cfg.f
+    W1, W3, W2 = _weights(E, d, f)
+    n_exec = 200 if quick else 1000
+    clocks, power = [], []
+    try:
+        import pynvml
+        import threading
+        pynvml.nvmlInit()
+        h = pynvml.nvmlDeviceGetHandleByIndex(torch.cuda.current_device())
+        stop = threading.Event()
+
+        def sample():
+            while not stop.is_set():
+                clocks.append(int(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                time.sleep(0.01)
+        th = threading.Thread(target=sample, daemon=True)
+        th.start()
+    except Exception:
+        stop, th = None, None
+    time.sleep(1.0)                                  # let the device idle: the run starts cold
+    lat, samples = B.profile_expert_latency(W1, W3, W2, (4096,), mode=0, warmup=0, iters=n_exec, return_samples=True)
+    if stop is not None:
+        stop.set()
+        th.join(timeout=2)
+    t = samples[0]                                   # whole-kernel time per execution [us]
+    flops = 6.0 * E * 4096 * d * f
+    q = lambda a, p: float(np.percentile(a, p))
+    out = {"shape": cfg.name, "tokens_per_expert": 4096, "executions": n_exec,
+           "us_first_10": round(float(t[:10].mean()), 1), "us_last_100": round(float(t[-100:].mean()), 1),
+           "us_median": round(q(t, 50), 1), "us_p1": round(q(t, 1), 1), "us_p99": round(q(t, 99), 1),
+           "slowdown_steady_vs_cold": round(float(t[-100:].mean() / t[:10].mean()), 4),
+           "spread_p99_over_p1": round(q(t, 99) / q(t, 1), 4),
+           "tflops_first_10": round(flops / float(t[:10].mean()) / 1e6, 1),
+           "tflops_last_100": round(flops / float(t[-100:].mean()) / 1e6, 1),
+           "sm_mhz_max": max(clocks) if clocks else None, "sm_mhz_min_under_load": min(clocks) if clocks else None,
+           "sm_mhz_last": clocks[-1] if clocks else None, "power_w_max": round(max(power), 1) if power else None}
+    del W1, W3, W2
+    torch.cuda.empty_cache()
+    return out
+
+
+def section_rack(peaks, quick, profile):
+    """Rack-scale projection (Fig. 15): the same three policies as G grows
+    from 8 to 128 virtual GPUs, sigma_g resampled per G, equal experts per GPU (cap = E/G), model B."""
+    model, _ = _c3_model(peaks, profile)
+    E, k = 256, 8
+    rc = B.RouteConfig(num_experts=E, top_k=k)
+    lg = torch.from_numpy(I.make_logits(16384, E, 1.2, 7, 1.0)).cuda()
+    load = B.route_topk(lg, rc)[2].cpu().numpy().astype(np.float64)
+    out = []
+    for G in (8, 16, 32, 64, 128):
+        gains_t, gains_c, ratio = [], [], []
+        for seed in range(4 if quick else 16):
+            scale = I.make_throughput_scales(G, 100 + seed)
+            cap = E // G
+            tb = B.placement_token_balanced(load, G, cap)
+            lb = B.placement_greedy(load, G, scale, model, cap)
+            ct = B.placement_contiguous(E, G)
+            s_tb = B.placement_eval(tb, load, G, scale, model, B.MODEL_B)[0]
+            s_lb, per = B.placement_eval(lb, load, G, scale, model, B.MODEL_B)
+            s_ct = B.placement_eval(ct, load, G, scale, model, B.MODEL_B)[0]
+            gains_t.append(1.0 - s_lb / s_tb)
+            gains_c.append(1.0 - s_lb / s_ct)
+            ratio.append(s_lb / float(per.mean()))
+        out.append({"G": G, "experts_per_gpu": E // G,
+                    "gain_latency_vs_token_median": round(float(np.median(gains_t)), 4),
+                    "gain_latency_vs_token_min": round(float(min(gains_t)), 4),
+                    "gain_latency_vs_token_max": round(float(max(gains_t)), 4),
+                    "gain_latency_vs_contiguous_median": round(float(np.median(gains_c)), 4),
+                    "latency_balanced_max_over_mean_median": round(float(np.median(ratio)), 4)})
+    return out
+
+
+def section_recalibration(peaks, quick, profile):
+    """Online recalibration (Alg. 1 phase 3 + Alg. 2): the routing distribution drifts from one Zipf
+    permutation to another over 200 passes; the drift monitor (window 100, H 10, delta 0.05) fires, the swap
+    solver repairs the stale latency-balanced placement; swaps applied versus experts a full re-solve moves."""
+    model, _ = _c3_model(peaks, profile)
+    E, G, k, T = 256, 8, 8, 4096
+    rc = B.RouteConfig(num_experts=E, top_k=k)
+    scale = I.make_throughput_scales(G, 3)
+    base_a = torch.from_numpy(I.make_logits(T, E, 1.2, 21, 1.0)).cuda()
+    bias_a = torch.from_numpy(I.zipf_bias(E, 1.2, 21)).cuda()
+    bias_b = torch.from_numpy(I.zipf_bias(E, 1.2, 22)).cuda()
+    mon = B.DriftMonitor(1, E, 100, 10, 0.05)
+    events, assign, passes = [], None, 300 if quick else 600
+    for p in range(1, passes + 1):
+        mix = 0.0 if p <= 150 else min(1.0, (p - 150) / 200.0)
+        lg = base_a - bias_a[None, :] + ((1 - mix) * bias_a + mix * bias_b)[None, :]
+        load = B.route_topk(lg.contiguous(), rc)[2].cpu().numpy().astype(np.float64)
+        trig, dist = mon.push(load[None, :])
+        if p == 100:
+            w = mon.window_mean()[0]
+            mon.set_reference(w[None, :])
+            assign = B.placement_greedy(w, G, scale, model, E // G)
+        if trig:
+            w = mon.window_mean()[0]
+            before = B.placement_eval(assign, w, G, scale, model, B.MODEL_B)[0]
+            fixed, swaps = B.placement_swap_refine(assign, w, G, scale, model, B.MODEL_B, 0.03)
+            after = B.placement_eval(fixed, w, G, scale, model, B.MODEL_B)[0]
+            full = B.placement_greedy(w, G, scale, model, E // G)
+            events.append({"pass": p, "cosine_distance": round(float(dist[0]), 4), "swaps": len(swaps),
+                           "experts_moved_by_swaps": int((fixed != assign).sum()),
+                           "experts_moved_by_full_resolve": int((full != assign).sum()),
+                           "score_before_us": round(before, 2), "score_after_swaps_us": round(after, 2),
+                           "score_full_resolve_us": round(B.placement_eval(full, w, G, scale, model, B.MODEL_B)[0], 2)})
+            assign = fixed
+            mon.rearranged()
+    mon.close()
+    return {"passes": passes, "drift": "Zipf(1.2) expert permutation A -> B, linear over passes 150..350", "events": events}
+
+
 def write_markdown(r, path, command):
     """The JSON report as markdown tables (what profiles/r1_report.md holds)."""
     import collections
@@ -304,49 +431,78 @@ def write_markdown(r, path, command):
     o.append("# r1: per-kernel measurements on one B200 (`python -m paper_2606_00735_b200.report`)\n")
     o.append("Command (under gpurun, one B200, no profiler attached):\n\n    " + command + "\n")
     o.append(f"Peaks ({r['peaks']['kind']}, MEASURED_PEAKS.json): HBM copy {r['peaks']['hbm_gbs']} GB/s; cuBLAS bf16 {r['peaks']['bf16_tflops']} TFLOP/s burst, {r['peaks']['bf16_tflops_sustained']} sustained.  GPU: {r['gpu']}.\n")
-    o.append("## stages: route / permute / combine, each timed alone from a CUDA graph over rotating cold buffer sets\n")
-    o.append("achieved = algorithmic bytes (DESIGN.md section 7) / device time; `frac` = achieved / measured HBM copy peak.\n")
-    o.append("| config | T | E (resident) | k | d | real rows | route us | GB/s | frac | permute us | GB/s | frac | combine us | GB/s | frac |")
-    o.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
-    for s in r['stages']:
-        o.append(f"| {s['config']} | {s['T']} | {s['E']} ({s['E_loc']}) | {s['k']} | {s['d']} | {s['real_rows']} | "+" | ".join(f"{s[n]['us']} | {s[n]['GB/s']} | {s[n]['frac_hbm']}" for n in ('route','permute','combine'))+" |")
-    o.append("\nRoute is issue-bound, not HBM-bound (`r1_route_s64k_ncu.md`); permute = 2 launches (cooperative index kernel + row kernel), combine = 1.\n")
-    o.append("## ffn_balanced: grouped FFN, every expert n rows (vibe_profile_expert_latency mode 0, largest n first, 2 s warm loop)\n")
-    o.append("| shape | E_loc | d | f | tokens/expert | us/expert | TFLOP/s | of sustained | of burst | of per-expert roofline max(flops/sustained, bytes/HBM) |")
-    o.append("|---|---|---|---|---|---|---|---|---|---|")
-    for x in r['ffn_balanced']:
-        o.append(f"| {x['shape']} | {x['E_loc']} | {x['d']} | {x['f']} | {x['tokens_per_expert']} | {x['us_per_expert']} | {x['TFLOP/s']} | {x['frac_sustained']} | {x['frac_burst']} | {x['frac_of_per_expert_roofline']} |")
-    o.append("\n## fused_scatter: vibe_grouped_ffn + vibe_combine vs vibe_grouped_ffn_scatter + vibe_combine_scattered (routed batches)\n")
-    o.append("| config | ffn + combine us | fused scatter us | speedup |\n|---|---|---|---|")
-    for x in r['fused_scatter']:
-        o.append(f"| {x['config']} | {x['ffn_plus_combine_us']} | {x['fused_scatter_us']} | {x['speedup']} |")
-    o.append("\n## profile: per-expert latency l(n) [us], median of 100 calls per point (p10..p90), modes 0 (all experts n rows; time / E_loc) and 1 (one expert n rows)\n")
-    for name,p in r['profile'].items():
-        o.append(f"### {name}: E_loc={p['E_loc']} d={p['d']} f={p['f']}\n")
-        o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 |\n|---|---|---|---|---|---|---|---|")
-        m0={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==0}
-        m1={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==1}
-        for n in sorted(m0):
-            a,b=m0[n],m1[n]
-            o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} |")
-        o.append("")
-    o.append("## placement_stress (BASELINE.json configs[4]): 256 experts -> 8 virtual GPUs, sigma ~ U[0.78,1.0] (8 seeds), measured C3-shape profile\n")
-    o.append("score = max over bins of modelled latency / sigma [us]; gain = 1 - latency-balanced / token-balanced.  Medians over the 8 scale draws.\n")
-    o.append("| zipf s | T | cap | model | contiguous | token-balanced | latency-balanced (ViBE) | gain vs token-balanced (median, min..max) | gain vs contiguous (median) |")
-    o.append("|---|---|---|---|---|---|---|---|---|")
-    g=collections.defaultdict(list)
-    for x in r['placement_stress']: g[(x['zipf_s'],x['T'],x['cap'],x['model'])].append(x)
-    for k_,v in sorted(g.items()):
-        med=lambda f: round(st.median(f(y) for y in v),2)
-        gt=[y['gain_latency_vs_token'] for y in v]
-        o.append(f"| {k_[0]} | {k_[1]} | {k_[2]} | {k_[3]} | {med(lambda y:y['contiguous']['score_us'])} | {med(lambda y:y['token_balanced']['score_us'])} | {med(lambda y:y['latency_balanced']['score_us'])} | {round(st.median(gt),4)} ({min(gt)}..{max(gt)}) | {med(lambda y:y['gain_latency_vs_contiguous'])} |")
+    if "stages" in r:
+        o.append("## stages: route / permute / combine, each timed alone from a CUDA graph over rotating cold buffer sets\n")
+        o.append("achieved = algorithmic bytes (DESIGN.md section 7) / device time; `frac` = achieved / measured HBM copy peak.\n")
+        o.append("| config | T | E (resident) | k | d | real rows | route us | GB/s | frac | permute us | GB/s | frac | combine us | GB/s | frac |")
+        o.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+        for s in r['stages']:
+            o.append(f"| {s['config']} | {s['T']} | {s['E']} ({s['E_loc']}) | {s['k']} | {s['d']} | {s['real_rows']} | "+" | ".join(f"{s[n]['us']} | {s[n]['GB/s']} | {s[n]['frac_hbm']}" for n in ('route','permute','combine'))+" |")
+        o.append("\nRoute is issue-bound, not HBM-bound (`r1_route_s64k_ncu.md`); permute = 2 launches (cooperative index kernel + row kernel), combine = 1.\n")
+    if "ffn_balanced" in r:
+        o.append("## ffn_balanced: grouped FFN, every expert n rows (vibe_profile_expert_latency mode 0, largest n first, 2 s warm loop)\n")
+        o.append("| shape | E_loc | d | f | tokens/expert | us/expert | TFLOP/s | of sustained | of burst | of per-expert roofline max(flops/sustained, bytes/HBM) |")
+        o.append("|---|---|---|---|---|---|---|---|---|---|")
+        for x in r['ffn_balanced']:
+            o.append(f"| {x['shape']} | {x['E_loc']} | {x['d']} | {x['f']} | {x['tokens_per_expert']} | {x['us_per_expert']} | {x['TFLOP/s']} | {x['frac_sustained']} | {x['frac_burst']} | {x['frac_of_per_expert_roofline']} |")
+    if "fused_scatter" in r:
+        o.append("\n## fused_scatter: vibe_grouped_ffn + vibe_combine vs vibe_grouped_ffn_scatter + vibe_combine_scattered (routed batches)\n")
+        o.append("| config | ffn + combine us | fused scatter us | speedup |\n|---|---|---|---|")
+        for x in r['fused_scatter']:
+            o.append(f"| {x['config']} | {x['ffn_plus_combine_us']} | {x['fused_scatter_us']} | {x['speedup']} |")
+    if "profile" in r:
+        o.append("\n## profile: per-expert latency l(n) [us], median of 100 calls per point (p10..p90), modes 0 (all experts n rows; time / E_loc) and 1 (one expert n rows)\n")
+        for name,p in r['profile'].items():
+            o.append(f"### {name}: E_loc={p['E_loc']} d={p['d']} f={p['f']}\n")
+            o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 |\n|---|---|---|---|---|---|---|---|")
+            m0={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==0}
+            m1={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==1}
+            for n in sorted(m0):
+                a,b=m0[n],m1[n]
+                o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} |")
+            o.append("")
+    if "placement_stress" in r:
+        o.append("## placement_stress (BASELINE.json configs[4]): 256 experts -> 8 virtual GPUs, sigma ~ U[0.78,1.0] (8 seeds), measured C3-shape profile\n")
+        o.append("score = max over bins of modelled latency / sigma [us]; gain = 1 - latency-balanced / token-balanced.  Medians over the 8 scale draws.\n")
+        o.append("| zipf s | T | cap | model | contiguous | token-balanced | latency-balanced (ViBE) | gain vs token-balanced (median, min..max) | gain vs contiguous (median) |")
+        o.append("|---|---|---|---|---|---|---|---|---|")
+        g=collections.defaultdict(list)
+        for x in r['placement_stress']: g[(x['zipf_s'],x['T'],x['cap'],x['model'])].append(x)
+        for k_,v in sorted(g.items()):
+            med=lambda f: round(st.median(f(y) for y in v),2)
+            gt=[y['gain_latency_vs_token'] for y in v]
+            o.append(f"| {k_[0]} | {k_[1]} | {k_[2]} | {k_[3]} | {med(lambda y:y['contiguous']['score_us'])} | {med(lambda y:y['token_balanced']['score_us'])} | {med(lambda y:y['latency_balanced']['score_us'])} | {round(st.median(gt),4)} ({min(gt)}..{max(gt)}) | {med(lambda y:y['gain_latency_vs_contiguous'])} |")
+    if "variability" in r:
+        v = r["variability"]
+        o.append("\n## variability: " + str(v["executions"]) + " consecutive executions, " + v["shape"] +
+                 ", 4096 tokens per expert, from an idle device (PAPER.md L335 protocol)\n")
+        o.append("| us first 10 | us last 100 | median | p1 | p99 | steady / cold | p99 / p1 | TFLOP/s first 10 | TFLOP/s last 100 | SM MHz max | min under load | last | power W max |")
+        o.append("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+        o.append("| " + " | ".join(str(v[k_]) for k_ in ("us_first_10", "us_last_100", "us_median", "us_p1", "us_p99",
+                 "slowdown_steady_vs_cold", "spread_p99_over_p1", "tflops_first_10", "tflops_last_100", "sm_mhz_max",
+                 "sm_mhz_min_under_load", "sm_mhz_last", "power_w_max")) + " |")
+    if "rack_projection" in r:
+        o.append("\n## rack_projection: 256 experts, Zipf 1.2, 16K tokens, sigma ~ U[0.78,1.0] resampled 16x per G, cap = E/G, model B\n")
+        o.append("| G | experts/GPU | gain vs token-balanced: median | min | max | gain vs contiguous (median) | latency-balanced max/mean (median) |")
+        o.append("|---|---|---|---|---|---|---|")
+        for x in r["rack_projection"]:
+            o.append(f"| {x['G']} | {x['experts_per_gpu']} | {x['gain_latency_vs_token_median']} | {x['gain_latency_vs_token_min']} | "
+                     f"{x['gain_latency_vs_token_max']} | {x['gain_latency_vs_contiguous_median']} | {x['latency_balanced_max_over_mean_median']} |")
+    if "recalibration" in r:
+        c = r["recalibration"]
+        o.append("\n## recalibration: drift monitor (window 100, H 10, delta 0.05) + Algorithm 2 (eps 0.03); " + c["drift"] + "\n")
+        o.append("| pass | cosine distance | swaps | experts moved by swaps | moved by a full re-solve | score before us | after swaps | full re-solve |")
+        o.append("|---|---|---|---|---|---|---|---|")
+        for e in c["events"]:
+            o.append(f"| {e['pass']} | {e['cosine_distance']} | {e['swaps']} | {e['experts_moved_by_swaps']} | "
+                     f"{e['experts_moved_by_full_resolve']} | {e['score_before_us']} | {e['score_after_swaps_us']} | {e['score_full_resolve_us']} |")
     with open(path, "w") as fh:
         fh.write("\n".join(o) + "\n")
 
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--sections", default="stages,ffn,fused,profile,placement")
+    ap.add_argument("--sections", default="stages,ffn,fused,profile,placement,variability,rack,recalibration")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--md", default="", help="also write the report as markdown tables (needs all sections)")
@@ -379,6 +535,17 @@ def main():
         g = [r["gain_latency_vs_token"] for r in rep["placement_stress"] if r["model"] == "B" and r["cap"] > 0]
         print(f"placement: latency- vs token-balanced gain (model B, cap 32): median {np.median(g):.3f} "
               f"min {min(g):.3f} max {max(g):.3f}", flush=True)
+    if "variability" in want:
+        rep["variability"] = section_variability(peaks, args.quick)
+        print("variability", rep["variability"], flush=True)
+    if "rack" in want:
+        rep["rack_projection"] = section_rack(peaks, args.quick, rep.get("profile"))
+        for r in rep["rack_projection"]:
+            print("rack", r, flush=True)
+    if "recalibration" in want:
+        rep["recalibration"] = section_recalibration(peaks, args.quick, rep.get("profile"))
+        for e in rep["recalibration"]["events"]:
+            print("recalibration", e, flush=True)
     os.makedirs(os.path.dirname(args.out), exist_ok=True)
     with open(args.out, "w") as fh:
         json.dump(rep, fh, indent=1)
