@@ -328,7 +328,7 @@ def main():
     cpu_baseline = None
     if group.is_main and group.world == 1 and not args.no_cpu_baseline:
         from oracle import vibe_oracle as O
-        S = min(T, 128)
+        S = min(T, 512)
         L = {"logits": sets_h[0][0].numpy(), "X": sets_h[0][1].view(torch.int16).numpy().view(np.uint16),
              "select_bias": bias_np, "expert_map": emap_np,
              "W1": Wh[0].view(torch.int16).numpy().view(np.uint16),
