@@ -203,7 +203,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 
   if (warp == 0) {
     // ================================================================ TMA producer (both CTAs)
-    if (lane == 0) {
+    // The WHOLE warp walks the tile list (warp-uniform control flow and operands); one elected
+    // lane issues the expect_tx and the TMA instructions.
+    {
       // Both operands are re-read through L2: an activation tile by every feature block of its
       // expert, a weight tile by the pairs working on the other token tiles of the same expert.
       // Those pairs are NOT in lock-step (tile costs differ with the ragged N), so a weight line
@@ -211,6 +213,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       // (measured, profiles/), evict_last keeps them at the algorithmic bytes.
       const uint64_t pol_act = ptx::policy_evict_last();
       const uint64_t pol_w = ptx::policy_evict_last();
+      const uint32_t smem_base = ptx::smem_u32(smem);
+      const uint32_t full0 = ptx::mapa_u32(ptx::smem_u32(&tail->full[0]), 0);   // the leader's barriers
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
@@ -225,28 +229,37 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         const int n0 = f_blk * FB + (int)rank * FC;
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
-          const uint32_t full_local = ptx::smem_u32(&tail->full[stage]);
-          if (rank == 0) ptx::mbar_arrive_expect_tx(full_local, 2 * STAGE_BYTES);
-          const uint32_t full = ptx::mapa_u32(full_local, 0);   // the leader's barrier
-          const uint32_t a_s = ptx::smem_u32(smem + (size_t)stage * STAGE_BYTES);
-          const uint32_t b_s = a_s + A_BYTES;
-          const int k0 = kb * BK;
-          if (kGateUp) {
-            ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);                 // gate -> lanes 0..63
-            ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, n0, k0, e, pol_w);    // up   -> lanes 64..127
-          } else {
-            ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);
-            ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, n0 + 64, k0, e, pol_w);
+          if (ptx::elect_one()) {
+            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), 2 * STAGE_BYTES);
+            const uint32_t full = full0 + (uint32_t)stage * 8u;
+            const uint32_t a_s = smem_base + (uint32_t)stage * STAGE_BYTES;
+            const uint32_t b_s = a_s + A_BYTES;
+            const int k0 = kb * BK;
+            if (kGateUp) {
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);                 // gate -> lanes 0..63
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, n0, k0, e, pol_w);    // up   -> lanes 64..127
+            } else {
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, n0 + 64, k0, e, pol_w);
+            }
+            ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
           }
-          ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
     // ================================================================ UMMA issuer (leader CTA)
-    if (rank == 0 && lane == 0) {
+    // The whole warp runs the loop; one elected lane issues the MMAs and the commits (always the
+    // same lane: tcgen05.commit tracks the MMAs of the issuing thread).
+    if (rank == 0) {
       constexpr uint32_t idesc0 = ptx::make_idesc_bf16_f32(256, 0, /*a_mn=*/true, /*b_mn=*/false);
+      // descriptor = constant high word | low word (start address >> 4 in bits [0,14), LBO in [16,30))
+      constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+      const uint32_t smem_base = ptx::smem_u32(smem);
+      const uint32_t a_lo0 = ((smem_base >> 4) & 0x3fffu) | ((uint32_t)(ATOM_BYTES >> 4) << 16);
+      const uint32_t b_lo0 = (((smem_base + A_BYTES) >> 4) & 0x3fffu) | ((16u >> 4) << 16);
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
@@ -266,20 +279,24 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->full[stage]), phase);
           ptx::tc_fence_after();
-          const uint32_t a_s = ptx::smem_u32(smem + (size_t)stage * STAGE_BYTES);
-          const uint32_t b_s = a_s + A_BYTES;
+          if (ptx::elect_one()) {
+            // A: MN-major SW128 -> 16 K-rows = 2 swizzle atoms of 1024 B (+128 in units of 16 B);
+            // B: K-major SW128 -> 16 elements = 32 bytes inside the 128-byte row (+2)
+            const uint32_t a_lo = a_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
+            const uint32_t b_lo = b_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
 #pragma unroll
-          for (int k = 0; k < BK / UMMA_K; ++k) {
-            // A: MN-major SW128 -> 16 K-rows = 2 swizzle atoms of 1024 B; next 64 features at LBO
-            const uint64_t da = ptx::make_smem_desc_sw128(a_s + k * (UMMA_K * 128), ATOM_BYTES, 1024);
-            // B: K-major SW128 -> advance 16 elements = 32 bytes inside the 128-byte row
-            const uint64_t db = ptx::make_smem_desc_sw128(b_s + k * (UMMA_K * 2), 16, 1024);
-            ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
+            for (int k = 0; k < BK / UMMA_K; ++k) {
+              const uint64_t da = ((uint64_t)DESC_HI << 32) | (uint64_t)(a_lo + (uint32_t)k * (UMMA_K * 128 / 16));
+              const uint64_t db = ((uint64_t)DESC_HI << 32) | (uint64_t)(b_lo + (uint32_t)k * (UMMA_K * 2 / 16));
+              ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
+            }
+            ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
+            if (kb == KB - 1)
+              ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->tfull[acc]), 3);   // accumulator ready in both CTAs
           }
-          ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
-        ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->tfull[acc]), 3);       // accumulator ready in both CTAs
       }
     }
   } else {

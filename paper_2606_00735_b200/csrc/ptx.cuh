@@ -135,6 +135,20 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&r)[32])
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// One lane of the (converged) warp: the code around it stays warp-uniform, so the compiler keeps
+// descriptors, addresses and barriers in UNIFORM registers.  Wrapping a whole loop in
+// `if (lane == 0)` instead makes every operand "possibly divergent" and costs an ELECT /
+// R2UR.BROADCAST x7 / BRA.U.ANY sequence per tcgen05.mma or TMA instruction.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 // ---------------------------------------------------------------- clusters / CTA pairs
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
