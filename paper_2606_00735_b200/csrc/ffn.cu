@@ -84,6 +84,12 @@ struct TileCursor {
   }
 };
 
+// Tile of CTA pair `pair` in round `rnd`: round r hands out tiles [r*P, (r+1)*P) ROTATED by r.
+// Tile ids stay increasing per pair, every tile is taken exactly once, and a pair does not keep
+// the same position inside a repeating cost pattern (with the plain stride P = 74, a layer whose
+// experts all have a 256-row and a 128-row token tile gave half the pairs only the large tiles).
+__device__ __forceinline__ int tile_of(int rnd, int pair, int P) { return rnd * P + (pair + rnd) % P; }
+
 __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<const uint32_t*>(&h);
@@ -218,7 +224,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = pair; tile < total_tiles; tile += num_pairs) {
+      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, tile = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
@@ -264,7 +270,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int tile = pair; tile < total_tiles; tile += num_pairs, ++it) {
+      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
@@ -304,7 +310,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     const int q = warp & 3;  // TMEM lane quarter this warp may access
     TileCursor cur;
     int it = 0;
-    for (int tile = pair; tile < total_tiles; tile += num_pairs, ++it) {
+    for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
       int f_blk, t_blk;
       cur.decode(tail, tile, NB, f_blk, t_blk);
       const int e = cur.e;
