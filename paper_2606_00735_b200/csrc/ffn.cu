@@ -68,6 +68,7 @@ struct SmemTail {
   int32_t total_t_tiles;
   int32_t off[MAX_SLOTS + 1];     // segment starts (rows)
   int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
+  int32_t tsz[MAX_SLOTS];         // rows per token tile of the slot (multiple of 16, <= TN)
 };
 constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + sizeof(SmemTail);
 static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB dynamic shared memory of sm_100");
@@ -183,7 +184,13 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         hi = offsets[e + 1];
         tail->off[e] = lo;
       }
+      // An expert's rows are cut into nt EQUAL token tiles (not 256, 256, ..., remainder): the pairs
+      // that share its weight tile (same feature block, other token tiles) and its activation tile
+      // (same token tile, other feature blocks) then run K steps of the same length and stay in
+      // step, which is what lets L2 serve the second reader.  With a short last tile the readers
+      // drift apart by more than L2 holds and DRAM traffic doubles (measured, profiles/).
       const int nt = (hi - lo + TN - 1) / TN;
+      if (e < E_loc) tail->tsz[e] = nt > 0 ? ((((hi - lo + nt - 1) / nt) + 15) & ~15) : TN;
       int inc = nt;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -228,8 +235,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         int f_blk, t_blk;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
-        const int row0 = tail->off[e] + t_blk * TN;
-        const int n_rows = min(TN, tail->off[e + 1] - row0);
+        const int tsz = tail->tsz[e];
+        const int row0 = tail->off[e] + t_blk * tsz;
+        const int n_rows = min(tsz, tail->off[e + 1] - row0);
         const int half = ((n_rows + 15) >> 4) << 3;          // UMMA N / 2: this CTA's share of the columns
         const int row_b = row0 + (int)rank * half;
         const int n0 = f_blk * FB + (int)rank * FC;
@@ -274,7 +282,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         int f_blk, t_blk;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
-        const int n_rows = min(TN, tail->off[e + 1] - (tail->off[e] + t_blk * TN));
+        const int tsz = tail->tsz[e];
+        const int n_rows = min(tsz, tail->off[e + 1] - (tail->off[e] + t_blk * tsz));
         const uint32_t n_mma = (uint32_t)((n_rows + 15) >> 4) << 4;
         const uint32_t idesc = idesc0 | ((n_mma >> 3) << 17);
         const int acc = it & 1;
@@ -314,8 +323,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       int f_blk, t_blk;
       cur.decode(tail, tile, NB, f_blk, t_blk);
       const int e = cur.e;
-      const int row0 = tail->off[e] + t_blk * TN;
-      const int n_rows = min(TN, tail->off[e + 1] - row0);
+      const int tsz = tail->tsz[e];
+      const int row0 = tail->off[e] + t_blk * tsz;
+      const int n_rows = min(tsz, tail->off[e + 1] - row0);
       const int acc = it & 1;
       const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
       // fused scatter: destination row and gate weight of this tile's tokens, lane L of block b
