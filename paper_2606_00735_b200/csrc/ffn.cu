@@ -55,7 +55,12 @@ constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumul
 constexpr int B_BYTES = (TN / 2) * BK * 2;      // 16 KB: this CTA's half of the token tile
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
 constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
-constexpr int NUM_THREADS = 192;
+// warps: 0 = TMA producer, 1 = MMA issuer, 2.. = epilogue.  GEMM-1 has 4 epilogue warps (its SwiGLU
+// epilogue needs ~200 registers per thread); the down projection has 8 -- two per TMEM lane quarter,
+// alternating 32-column blocks -- because with a short K loop (f = 768: 12 K steps per tile) one warp
+// per quarter could not drain a 256-column accumulator as fast as the tensor pipe fills the next
+// (ncu at the C2 shape: tensor pipe 33 % active with 4 warps).
+__host__ __device__ constexpr int num_threads(int mode) { return mode == 0 ? 192 : 320; }
 constexpr int MAX_SLOTS = 512;
 constexpr int TMEM_COLS = 512;
 
@@ -138,7 +143,7 @@ __device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv
 // kMode: 0 = gate|up + SwiGLU (GEMM-1), 1 = down (GEMM-2), 2 = down with the gate-weighted
 // scatter fused into the epilogue (vibe_grouped_ffn_scatter).
 template <int kMode>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
                 const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
                 int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out,
@@ -167,7 +172,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(ptx::smem_u32(&tail->tfull[a]), 1);
-      ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 8);
+      ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 2 * (num_threads(kMode) / 32 - 2));   // epilogue warps of the pair
     }
     ptx::fence_barrier_init();
   } else if (warp == 1) {
@@ -317,6 +322,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   } else {
     // ================================================================ epilogue (warps 2..5, both CTAs)
     const int q = warp & 3;  // TMEM lane quarter this warp may access
+    const int blk_par = (warp - 2) >> 2;   // down projection: which 32-column blocks (even / odd) are mine
     TileCursor cur;
     int it = 0;
     for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
@@ -380,6 +386,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         for (int b = 0; b < TN / 32; ++b) {
           const int c0 = b * 32;
           if (c0 >= n_rows) break;
+          if ((b & 1) != blk_par) continue;
           uint32_t a[32];
           ptx::tmem_ld_32x32(taddr + c0, a);
           ptx::tmem_ld_wait();
@@ -511,15 +518,15 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn_gemm_kernel<0><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
+  ffn_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
                                                             reinterpret_cast<__nv_bfloat16*>(H_ws), f, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
   if (row_to_assign != nullptr)
-    ffn_gemm_kernel<2><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+    ffn_gemm_kernel<2><<<grid, num_threads(2), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
                                                               reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign,
                                                               topk_w);
   else
-    ffn_gemm_kernel<1><<<grid, NUM_THREADS, SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+    ffn_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
                                                               reinterpret_cast<__nv_bfloat16*>(Y), d, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
