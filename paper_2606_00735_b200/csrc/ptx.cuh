@@ -165,8 +165,12 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
   return r;
 }
 // arrive on an mbarrier that may live in the peer CTA (address from mapa_u32)
+// (default .release.cta semantics: the arrive orders this thread's tcgen05.ld results -- after
+// tcgen05.fence::before_thread_sync -- for the waiting MMA thread; a .release.cluster here made
+// ptxas emit MEMBAR.ALL.GPU + ERRBAR, i.e. every epilogue warp waited for its global stores of
+// the tile to be acknowledged before freeing the accumulator: 10 % of the kernel's stall samples.)
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
