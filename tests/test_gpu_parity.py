@@ -434,8 +434,9 @@ def test_profile_expert_latency_sanity():
     lat, samples = B.profile_expert_latency(W1, W3, W2, sweep, mode=0, warmup=3, iters=15, return_samples=True)
     assert lat.shape == (5,) and samples.shape == (5, 15)
     assert np.all(lat > 0) and np.all(np.isfinite(lat))
-    # non-decreasing within 10 % and large-n cost per token well below small-n cost per token
-    assert np.all(lat[1:] >= lat[:-1] * 0.9), lat
+    # non-decreasing (within 20 %: the flat weight-streaming region is a timing of ~20 us kernels) and
+    # large-n cost per token well below small-n cost per token
+    assert np.all(lat[1:] >= lat[:-1] * 0.8), lat
     assert lat[-1] / 2048 < lat[0] / 1
     # flop floor at the nominal dense bf16 peak (2.25 PFLOP/s): cannot be faster than that
     flops = 6.0 * 2048 * cfg.d * cfg.f
