@@ -324,6 +324,36 @@ def main():
         stages[name] = {"ms": round(ms, 4), "GB/s": round(gbs, 1), "frac_hbm": round(gbs / hbm, 4)}
     stages["grouped_ffn"] = {"ms": round(stage_ms[2], 4), "TFLOP/s": round(achieved_tf, 2)}
 
+    # ---------------------------------------------------------------- bandwidth kernels alone, from CUDA graphs
+    # The per-stage events above sit between Python-issued launches, so for the microsecond-scale
+    # route / permute / combine stages they mostly time the host.  Here each stage is captured
+    # (one call per rotating buffer set) into a CUDA graph and replayed: device time only.
+    def graph_us(fn, reps=20):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for i in range(args.sets):
+                fn(i)
+        g.replay()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            g.replay()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e3 / (reps * args.sets)
+
+    iso = {
+        "route": graph_us(lambda i: B.route_topk(sets_d[i % args.sets][0], rc, out=(ids, gw, counts))),
+        "permute": graph_us(lambda i: B.permute(sets_d[i % args.sets][1], ids, counts, emap, E, E_loc, 1,
+                                                out=(Xp, off, r2a, a2r), ws=pws)),
+        "combine": graph_us(lambda i: B.combine(Y, a2r, gw, T, k, out=out)),
+    }
+    for name, by in (("route", bytes_route), ("permute", bytes_perm), ("combine", bytes_comb)):
+        gbs = by / (iso[name] * 1e-6) / 1e9
+        stages[name].update({"alone_us": round(iso[name], 2), "alone_GB/s": round(gbs, 1),
+                             "alone_frac_hbm": round(gbs / hbm, 4)})
+
     # ---------------------------------------------------------------- CPU baseline (oracle, rank 0, N = 1)
     cpu_baseline = None
     if group.is_main and group.world == 1 and not args.no_cpu_baseline:

@@ -3,7 +3,8 @@
 //
 // Two launches on one stream, no host sync:
 //   K1 perm_index  : a COOPERATIVE launch of G <= #SMs CTAs x 1024 threads (all co-resident, so
-//                    the one grid-wide barrier below cannot deadlock).  Warp gw = 32*cta + w owns
+//                    the one grid-wide barrier below cannot deadlock); when G <= 8 the grid is one
+//                    thread-block cluster instead and the barrier is barrier.cluster.  Warp gw = 32*cta + w owns
 //                    the contiguous chunk [gw*WCH, (gw+1)*WCH) of the A = T*k assignments.
 //                      pass 1  lanes holding the same slot are matched with ballots (one per key
 //                              bit, fixed cost); per-warp slot histograms in shared memory; the
@@ -28,6 +29,7 @@
 #include <atomic>
 
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace vibe {
 namespace {
@@ -87,7 +89,8 @@ __device__ __forceinline__ void grid_barrier_once(unsigned* bar, unsigned G) {
 // K1 ------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kIdxThreads, 1)
 perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int A, int E, int E_loc,
-                  int WCH, int align, int d, int bar_slot, int32_t* __restrict__ tbl /*[G][E_loc]*/,
+                  int WCH, int align, int d, int bar_slot /* < 0: the grid is ONE cluster */,
+                  int32_t* __restrict__ tbl /*[G][E_loc]*/,
                   int32_t* __restrict__ offsets /*[E_loc+1]*/, int32_t* __restrict__ row_to_assign,
                   int32_t* __restrict__ assign_to_row, __nv_bfloat16* __restrict__ Xp) {
   extern __shared__ int s_mem[];
@@ -143,7 +146,12 @@ perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ e
     }
     tbl[(size_t)cta * E_loc + s] = run;
   }
-  grid_barrier_once(g_bar[bar_slot], (unsigned)G);
+  if (bar_slot < 0) {
+    __threadfence();
+    ptx::cluster_sync_all();          // G <= 8: hardware cluster barrier (release / acquire at cluster scope)
+  } else {
+    grid_barrier_once(g_bar[bar_slot], (unsigned)G);
+  }
   // ---- walk the table: rows before mine (base) and all rows (totals).  W slot columns x
   // NG row groups; group g takes rows g, g + NG, ... ----
   for (int s0 = 0; s0 < E_loc; s0 += kIdxThreads) {
@@ -369,14 +377,34 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
     VIBE_CUDA(cudaFuncSetAttribute(perm_index_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
     smem_set.store(smem1);
   }
-  static std::atomic<unsigned> next_slot{0};
-  int bar_slot = (int)(next_slot.fetch_add(1, std::memory_order_relaxed) % kBarSlots);
   __nv_bfloat16* Xpb = reinterpret_cast<__nv_bfloat16*>(Xp);
   int32_t* tbl = reinterpret_cast<int32_t*>(ws);
-  int A_ = A, E_ = E, El_ = E_loc, al_ = align, d_ = d;
-  void* args[] = {(void*)&topk_ids, (void*)&expert_map, &A_, &E_, &El_, &WCH, &al_, &d_, &bar_slot, &tbl, &offsets,
-                  &row_to_assign, &assign_to_row, &Xpb};
-  VIBE_CUDA(cudaLaunchCooperativeKernel((const void*)perm_index_kernel, dim3(G), dim3(kIdxThreads), args, smem1, st));
+  if (G <= 8) {
+    // small batches: the whole grid is one thread-block cluster (portable size <= 8), the barrier is
+    // barrier.cluster -- ~3 us less than the cooperative launch + atomic barrier at A = 8K
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)G;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cudaLaunchConfig_t lc1 = {};
+    lc1.gridDim = dim3(G);
+    lc1.blockDim = dim3(kIdxThreads);
+    lc1.dynamicSmemBytes = smem1;
+    lc1.stream = st;
+    lc1.attrs = at;
+    lc1.numAttrs = 1;
+    VIBE_CUDA(cudaLaunchKernelEx(&lc1, perm_index_kernel, topk_ids, expert_map, (int)A, (int)E, (int)E_loc, WCH,
+                                 (int)align, (int)d, -1, tbl, offsets, row_to_assign, assign_to_row, Xpb));
+  } else {
+    static std::atomic<unsigned> next_slot{0};
+    int bar_slot = (int)(next_slot.fetch_add(1, std::memory_order_relaxed) % kBarSlots);
+    int A_ = A, E_ = E, El_ = E_loc, al_ = align, d_ = d;
+    void* args[] = {(void*)&topk_ids, (void*)&expert_map, &A_, &E_, &El_, &WCH, &al_, &d_, &bar_slot, &tbl, &offsets,
+                    &row_to_assign, &assign_to_row, &Xpb};
+    VIBE_CUDA(cudaLaunchCooperativeKernel((const void*)perm_index_kernel, dim3(G), dim3(kIdxThreads), args, smem1,
+                                          st));
+  }
   count_launch();
   const int vpr = d / 8;
   const __nv_bfloat16* Xb = reinterpret_cast<const __nv_bfloat16*>(X);
