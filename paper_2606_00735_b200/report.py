@@ -1,6 +1,6 @@
 """Per-kernel measurements on one B200 beyond the single bench.py line.
 
-    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,profile,placement,variability,rack,recalibration]
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,layer,profile,placement,variability,rack,recalibration]
                                            [--out gpurun_out/report.json] [--quick]
 
 Sections (all through the C-ABI binding; seeded synthetic inputs):
@@ -13,6 +13,7 @@ Sections (all through the C-ABI binding; seeded synthetic inputs, DESIGN.md sect
              ">= 512 tokens per expert" target of BASELINE.json is read off this table.
   fused      vibe_grouped_ffn + vibe_combine versus the fused gate-weighted scatter path
              (vibe_grouped_ffn_scatter + vibe_combine_scattered) on the routed C1 / C2 batches.
+  layer      the whole layer through vibe_moe_layer_forward, eager launches versus one CUDA graph.
   profile    vibe_profile_expert_latency over the M3 sweep (1..4096 tokens per expert), modes 0
              and 1, for the C2 and C3 shapes: the per-GPU performance model f(n) of the paper
              (PAPER.md L176).  Written as CSV rows into the JSON and to <out>.profile.csv.
@@ -197,6 +198,47 @@ def section_fused(peaks, quick):
         out.append({"config": cfg.name, "ffn_plus_combine_us": round(tp, 2), "fused_scatter_us": round(tf, 2),
                     "speedup": round(tp / tf, 4)})
         del W1, W3, W2
+        torch.cuda.empty_cache()
+    return out
+
+
+def section_layer(peaks, quick):
+    """The whole layer (route -> permute -> grouped FFN -> combine) through vibe_moe_layer_forward: eager
+    launches (6 kernels + 1 memset enqueued by one C call) versus the same call captured in a CUDA graph."""
+    out = []
+    for cfg in (I.C1, I.C2, I.C3):
+        T, k, E, E_loc, d, f = cfg.T, cfg.k, cfg.E, cfg.E_loc, cfg.d, cfg.f
+        W1, W3, W2 = _weights(E_loc, d, f)
+        emap = torch.from_numpy(I.make_expert_map(cfg, "contiguous", 0)).cuda() if E_loc < E else None
+        bias = torch.from_numpy(I.make_select_bias(E, 0)).cuda() if cfg.has_select_bias else None
+        rc = B.RouteConfig(select_bias=bias, **I.route_kwargs(cfg))
+        nsets = 4
+        lgs = [torch.from_numpy(I.make_logits(T, E, cfg.zipf_s, i, cfg.alpha)).cuda() for i in range(nsets)]
+        Xs = [torch.randn((T, d), device="cuda").to(torch.bfloat16) for _ in range(nsets)]
+        o = torch.empty((T, d), dtype=torch.bfloat16, device="cuda")
+        cnt = torch.empty((E,), dtype=torch.int32, device="cuda")
+        arena = torch.empty((B.workspace_bytes(B.WS_LAYER, T, k, E, E_loc, d, f),), dtype=torch.uint8, device="cuda")
+
+        def layer(i):
+            B.moe_layer_forward(rc, lgs[i % nsets], Xs[i % nsets], emap, W1, W3, W2, out=o, counts=cnt, arena=arena)
+
+        t0 = time.time()
+        while time.time() - t0 < (0.3 if quick else 1.5):
+            for i in range(8):
+                layer(i)
+            torch.cuda.synchronize()
+        iters = 40 if quick else 200
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(iters):
+            layer(i)
+        e1.record()
+        torch.cuda.synchronize()
+        eager = e0.elapsed_time(e1) * 1e3 / iters
+        graph = _time(layer, iters, period=nsets)
+        out.append({"config": cfg.name, "eager_us": round(eager, 1), "graph_us": round(graph, 1),
+                    "tokens_per_s_eager": round(T / eager * 1e6), "tokens_per_s_graph": round(T / graph * 1e6)})
+        del W1, W3, W2, Xs, lgs, arena
         torch.cuda.empty_cache()
     return out
 
@@ -472,6 +514,11 @@ def write_markdown(r, path, command):
             med=lambda f: round(st.median(f(y) for y in v),2)
             gt=[y['gain_latency_vs_token'] for y in v]
             o.append(f"| {k_[0]} | {k_[1]} | {k_[2]} | {k_[3]} | {med(lambda y:y['contiguous']['score_us'])} | {med(lambda y:y['token_balanced']['score_us'])} | {med(lambda y:y['latency_balanced']['score_us'])} | {round(st.median(gt),4)} ({min(gt)}..{max(gt)}) | {med(lambda y:y['gain_latency_vs_contiguous'])} |")
+    if "layer" in r:
+        o.append("\n## layer: vibe_moe_layer_forward (route + permute + grouped FFN + combine), zipf-routed batches, 4 rotating input sets\n")
+        o.append("| config | eager us | CUDA graph us | tokens/s eager | tokens/s graph |\n|---|---|---|---|---|")
+        for x in r["layer"]:
+            o.append(f"| {x['config']} | {x['eager_us']} | {x['graph_us']} | {x['tokens_per_s_eager']} | {x['tokens_per_s_graph']} |")
     if "variability" in r:
         v = r["variability"]
         o.append("\n## variability: " + str(v["executions"]) + " consecutive executions, " + v["shape"] +
@@ -502,7 +549,7 @@ def write_markdown(r, path, command):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--sections", default="stages,ffn,fused,profile,placement,variability,rack,recalibration")
+    ap.add_argument("--sections", default="stages,ffn,fused,layer,profile,placement,variability,rack,recalibration")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--md", default="", help="also write the report as markdown tables (needs all sections)")
@@ -527,6 +574,10 @@ def main():
     if "fused" in want:
         rep["fused_scatter"] = section_fused(peaks, args.quick)
         for r in rep["fused_scatter"]:
+            print(r, flush=True)
+    if "layer" in want:
+        rep["layer"] = section_layer(peaks, args.quick)
+        for r in rep["layer"]:
             print(r, flush=True)
     if "profile" in want:
         rep["profile"] = section_profile(peaks, args.quick)
