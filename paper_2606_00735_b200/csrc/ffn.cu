@@ -103,40 +103,56 @@ __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
 __device__ __forceinline__ float swiglu(float g, float u) { return __fdividef(g, 1.0f + __expf(-g)) * u; }
 
 // Store a 32-lane x 32-column block held one lane (= feature) per thread, v[i] = column
-// (= token) i, into row-major out[token][feature].  Lanes pair up so that every store is a
-// bf16x2 of two adjacent features: even lanes store the even columns, odd lanes the odd ones.
+// (= token) i, into row-major out[token][feature].  Every lane first packs its OWN two tokens
+// (i, i+1) of its feature into one bf16x2 word; lanes 2j / 2j+1 swap that word with one shuffle
+// and a byte permute picks {token i: features f, f+1} in the even lane and {token i+1: f, f+1}
+// in the odd lane -- per token pair: 1 cvt.bf16x2 + 1 shfl + 1 prmt + 1 store (the first version
+// shuffled fp32 values and selected operands with SELs: 365 instructions per block against ~120
+// now, and the down projection at K = 768 was bound by exactly this epilogue).
 __device__ __forceinline__ void store_block_T(const float (&v)[32], __nv_bfloat16* __restrict__ out, size_t ld,
                                               int row0, int n_rows, int feat, bool feat_ok, int lane) {
-  const bool odd = lane & 1;
-  __nv_bfloat16* base = out + (size_t)row0 * ld + (feat - (odd ? 1 : 0));
+  const int odd = lane & 1;
+  const uint32_t sel = odd ? 0x3276u : 0x5410u;
+  __nv_bfloat16* p = out + (size_t)(row0 + odd) * ld + (feat - odd);
+  const size_t step = 2 * ld;
+  if (n_rows >= 32) {
 #pragma unroll
-  for (int i = 0; i < 32; i += 2) {
-    const float send = odd ? v[i] : v[i + 1];
-    const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
-    const int tok = i + (odd ? 1 : 0);
-    const uint32_t pk = odd ? pack2_bf16(recv, v[i + 1]) : pack2_bf16(v[i], recv);
-    if (feat_ok && tok < n_rows) *reinterpret_cast<uint32_t*>(base + (size_t)tok * ld) = pk;
+    for (int i = 0; i < 32; i += 2) {
+      const uint32_t own = pack2_bf16(v[i], v[i + 1]);
+      const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+      const uint32_t pk = __byte_perm(own, got, sel);
+      if (feat_ok) *reinterpret_cast<uint32_t*>(p) = pk;
+      p += step;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 32; i += 2) {
+      const uint32_t own = pack2_bf16(v[i], v[i + 1]);
+      const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+      const uint32_t pk = __byte_perm(own, got, sel);
+      if (feat_ok && i + odd < n_rows) *reinterpret_cast<uint32_t*>(p) = pk;
+      p += step;
+    }
   }
 }
 
-// The same block, gate-weighted and scattered: token i of the block goes to row asg (its flat
-// assignment index, assignment order) of `out`, scaled by that assignment's gate weight wt; the
-// product is rounded to bf16 once.  Lane L holds (asg, wt) of token L of the block -- fetched
-// for the whole tile before the accumulator is ready, so no global latency sits in this loop.
+// The same block, gate-weighted and scattered: token i of the block goes to row asg[i] (its flat
+// assignment index, assignment order) of `out`, scaled by that assignment's gate weight wt[i]; the
+// product is rounded to bf16 once.  asg / wt of the tile's tokens sit in this warp's slice of shared
+// memory (written before the accumulator was ready): broadcast LDS, no shuffles, no global latency.
 __device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv_bfloat16* __restrict__ out,
-                                                      size_t ld, int feat, bool feat_ok, int lane, int asg,
-                                                      float wt) {
-  const bool odd = lane & 1;
+                                                      size_t ld, int feat, bool feat_ok, int lane,
+                                                      const float* __restrict__ wt, const int* __restrict__ asg) {
+  const int odd = lane & 1;
+  const uint32_t sel = odd ? 0x3276u : 0x5410u;
 #pragma unroll
   for (int i = 0; i < 32; i += 2) {
-    const float send = odd ? v[i] : v[i + 1];
-    const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
-    const int tok = i + (odd ? 1 : 0);
-    const int dst = __shfl_sync(0xffffffffu, asg, tok);
-    const float w = __shfl_sync(0xffffffffu, wt, tok);
-    const uint32_t pk = odd ? pack2_bf16(recv * w, v[i + 1] * w) : pack2_bf16(v[i] * w, recv * w);
-    if (feat_ok && dst >= 0)
-      *reinterpret_cast<uint32_t*>(out + (size_t)dst * ld + (feat - (odd ? 1 : 0))) = pk;
+    const float2 w = *reinterpret_cast<const float2*>(wt + i);
+    const int dst = asg[i + odd];
+    const uint32_t own = pack2_bf16(v[i] * w.x, v[i + 1] * w.y);
+    const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+    const uint32_t pk = __byte_perm(own, got, sel);
+    if (feat_ok && dst >= 0) *reinterpret_cast<uint32_t*>(out + (size_t)dst * ld + (feat - odd)) = pk;
   }
 }
 
@@ -334,18 +350,20 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       const int n_rows = min(tsz, tail->off[e + 1] - row0);
       const int acc = it & 1;
       const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
-      // fused scatter: destination row and gate weight of this tile's tokens, lane L of block b
-      // holds token 32*b + L; loaded while the MMAs of the tile are still running
-      int sc_asg[kMode == 2 ? TN / 32 : 1];
-      float sc_wt[kMode == 2 ? TN / 32 : 1];
+      // fused scatter: destination row and gate weight of this tile's tokens go to this warp's
+      // 2 KB slice of the (otherwise unused) exchange buffer while the MMAs of the tile still run
+      float* sc_wt = xchg + (warp - 2) * (2 * TN);
+      int* sc_asg = reinterpret_cast<int*>(sc_wt + TN);
       if (kMode == 2) {
+        __syncwarp();                       // the previous tile's reads of the slice are done
 #pragma unroll
         for (int b = 0; b < TN / 32; ++b) {
           const int c = b * 32 + lane;
-          sc_asg[b] = (c < n_rows) ? __ldg(row_to_assign + row0 + c) : -1;
+          const int a = (c < n_rows) ? __ldg(row_to_assign + row0 + c) : -1;
+          sc_asg[c] = a;
+          sc_wt[c] = (a >= 0) ? __ldg(topk_w + a) : 0.0f;
         }
-#pragma unroll
-        for (int b = 0; b < TN / 32; ++b) sc_wt[b] = (sc_asg[b] >= 0) ? __ldg(topk_w + sc_asg[b]) : 0.0f;
+        __syncwarp();
       }
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
@@ -394,8 +412,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 #pragma unroll
           for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]);
           if (kMode == 2)
-            store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_asg[kMode == 2 ? b : 0],
-                                  sc_wt[kMode == 2 ? b : 0]);
+            store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_wt + c0, sc_asg + c0);
           else
             store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
         }
