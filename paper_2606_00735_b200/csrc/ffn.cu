@@ -28,11 +28,16 @@
 // and masked at the store (columns are independent, nothing leaks); rows past R_cap are
 // zero-filled by TMA.
 // Pipeline: warp 0 = TMA producer (both CTAs), warp 1 = UMMA issuer (leader CTA) + TMEM owner,
-// warps 2..5 = epilogue.  6 smem stages x 32 KB, 2 TMEM accumulator stages x 256 columns so the
-// epilogue of tile i overlaps the MMAs of tile i+1.
-// Tile order: expert-major, then feature block, then token tile fastest, so pairs that run at
-// the same time share a weight tile through L2 (both operands evict_last) and each weight byte
-// leaves HBM once.
+// warps 2.. = epilogue (4 for GEMM-1, 8 for GEMM-2).  Producer and issuer are warp-uniform loops
+// with elect.sync around the instructions (operands stay in uniform registers).  6 smem stages
+// x 32 KB, 2 TMEM accumulator stages x 256 columns so the epilogue of tile i overlaps the MMAs
+// of tile i+1.
+// Tiles: an expert's rows are cut into EQUAL token tiles (multiples of 16, <= 256); tile order is
+// expert-major, then feature block, then token tile fastest, handed to the pairs round by round
+// with a rotation (tile_of), so pairs that run at the same time share a weight tile through L2
+// (both operands evict_last), run K steps of equal length, and each weight byte leaves HBM once.
+// Epilogue: tcgen05.ld 32 lanes x 32 columns, bf16x2 pack + one shuffle + byte permute per token
+// pair (the output is the TRANSPOSE of the accumulator), 4-byte stores of two adjacent features.
 //
 // Semantics: include/vibe.h (vibe_grouped_ffn); F1-F4.
 #include <mutex>
