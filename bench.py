@@ -279,9 +279,17 @@ def main():
     value, max_ms = D.aggregate_throughput(group, float(T) * args.steps, my_ms)
     stage_ms = [sum(e[j].elapsed_time(e[j + 1]) for e in evs) / args.steps for j in range(4)]
 
-    # real rows / resident tokens of the routed batch (for algorithmic bytes and flops)
-    R_real = int(off[-1].item())
-    res_tok = int((a2r.view(T, k) >= 0).any(dim=1).sum().item())
+    # real rows / resident tokens of the routed batches (for algorithmic bytes and flops): the buffer sets differ
+    # when only a shard of the experts is resident, so average over the sets in the proportion they were used
+    R_set, tok_set = [], []
+    for i in range(args.sets):
+        step(i)
+        torch.cuda.synchronize()
+        R_set.append(int(off[-1].item()))
+        tok_set.append(int((a2r.view(T, k) >= 0).any(dim=1).sum().item()))
+    uses = [len(range(i, args.steps, args.sets)) for i in range(args.sets)]
+    R_real = sum(r * u for r, u in zip(R_set, uses)) / max(1, sum(uses))
+    res_tok = sum(r * u for r, u in zip(tok_set, uses)) / max(1, sum(uses))
 
     # ---------------------------------------------------------------- end to end from host buffers
     arena = torch.empty((B.workspace_bytes(B.WS_LAYER_HOST, T, k, E, E_loc, d, f),), dtype=torch.uint8, device=dev)
@@ -377,7 +385,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": cfg.name, "T": T, "d": d, "f": f, "E": E, "k": k, "E_loc": E_loc,
-                       "routing": f"zipf_s={cfg.zipf_s} alpha={cfg.alpha}", "real_rows": R_real,
+                       "routing": f"zipf_s={cfg.zipf_s} alpha={cfg.alpha}", "real_rows": round(R_real, 1),
+                       "real_rows_per_set": R_set,
                        "parallelism": "replicas" if group.world > 1 else "single-gpu",
                        "l2": f"inputs rotate over {args.sets} buffer sets; "
                              f"{(3 * E_loc * d * f * 2) / 1e9:.2f} GB of weights stream through the 126 MB L2 every step"},
