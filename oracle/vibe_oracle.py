@@ -590,6 +590,117 @@ def placement_swap_refine(assign, load, G, scale, model, model_kind=MODEL_B, eps
 
 
 # ======================================================================================
+# O11  FP8 (e4m3) grouped FFN (f2).  The paper runs both models in FP8 (Table 2a) but says
+#      nothing about the recipe; reading Q1-Q4: OCP e4m3 ("fn": no infinities, max 448,
+#      round-to-nearest-even, saturating), per-expert weight scales absmax/448, per-row activation
+#      scales rowabsmax/448, a STATIC per-expert scale for the intermediate H, products accumulated
+#      exactly (f64 here, fp32 in the tensor core), scales applied to the accumulators.
+# ======================================================================================
+
+E4M3_MAX = 448.0
+
+
+def e4m3_decode_table():
+    """All 256 codes of OCP FP8 E4M3 (fn): 1 sign, 4 exponent (bias 7), 3 mantissa bits; exponent field 0 =
+    subnormals (m/8 * 2^-6); S.1111.111 = NaN; no infinities."""
+    t = np.zeros(256, dtype=np.float64)
+    for code in range(256):
+        sgn = -1.0 if code & 0x80 else 1.0
+        ex = (code >> 3) & 0xF
+        m = code & 0x7
+        if ex == 0xF and m == 0x7:
+            t[code] = np.nan
+        elif ex == 0:
+            t[code] = sgn * (m / 8.0) * 2.0 ** -6
+        else:
+            t[code] = sgn * (1.0 + m / 8.0) * 2.0 ** (ex - 7)
+    return t
+
+
+def e4m3_encode(x):
+    """f64 -> e4m3 codes (uint8): round to nearest, ties to even mantissa, saturate at +-448 (no NaN made)."""
+    x = np.asarray(x, dtype=np.float64)
+    out = np.zeros(x.shape, dtype=np.uint8)
+    flat, o = x.reshape(-1), out.reshape(-1)
+    for i in range(flat.size):
+        v = flat[i]
+        sgn = 0x80 if (v < 0 or (v == 0 and np.signbit(v))) else 0
+        a = min(abs(v), E4M3_MAX)
+        if a < 2.0 ** -6:                       # subnormal range: step 2^-9
+            q = a / 2.0 ** -9
+            n = int(np.floor(q))
+            r = q - n
+            if r > 0.5 or (r == 0.5 and (n & 1)):
+                n += 1
+            o[i] = sgn | n                      # n = 8 rolls over into the first normal (0001.000) correctly
+            continue
+        ex = int(np.floor(np.log2(a)))
+        if 2.0 ** ex > a:                        # guard log2 rounding
+            ex -= 1
+        q = a / 2.0 ** ex * 8.0 - 8.0            # mantissa in [0, 8)
+        n = int(np.floor(q))
+        r = q - n
+        if r > 0.5 or (r == 0.5 and (n & 1)):
+            n += 1
+        if n == 8:
+            n, ex = 0, ex + 1
+        code = ((ex + 7) << 3) | n
+        o[i] = sgn | min(code, 0x7E)            # 0x7E = 448
+    return out
+
+
+def fp8_pack_weights(W_bits):
+    """bf16 bits [E,K,N] -> (codes uint8 [E,N,K] (K contiguous), scale f32 [E] = absmax/448; all-zero expert: 1)."""
+    W = bf16_bits_to_f64(W_bits)
+    E = W.shape[0]
+    scale = np.ones(E, dtype=np.float32)
+    codes = np.zeros((E, W.shape[2], W.shape[1]), dtype=np.uint8)
+    for e in range(E):
+        amax = float(np.max(np.abs(W[e])))
+        if amax > 0:
+            scale[e] = np.float32(amax / E4M3_MAX)
+        codes[e] = e4m3_encode(W[e].T / np.float64(scale[e]))
+    return codes, scale
+
+
+def fp8_quantize_rows(X_bits):
+    """bf16 bits [R,d] -> (codes uint8 [R,d], row_scale f32 [R] = rowabsmax/448; all-zero row: 1)."""
+    X = bf16_bits_to_f64(X_bits)
+    R = X.shape[0]
+    scale = np.ones(R, dtype=np.float32)
+    for r in range(R):
+        amax = float(np.max(np.abs(X[r]))) if X.shape[1] else 0.0
+        if amax > 0:
+            scale[r] = np.float32(amax / E4M3_MAX)
+    codes = e4m3_encode(X / scale.astype(np.float64)[:, None]) if R else np.zeros_like(X_bits, dtype=np.uint8)
+    return codes, scale
+
+
+def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q, s2, h_scale):
+    """Per resident expert e and real row r:  g = sx[r] s1[e] (xq . w1q),  u = sx[r] s3[e] (xq . w3q),
+    h = silu(g) u,  hq = e4m3(h / sh[e]),  y = sh[e] s2[e] (hq . w2q).  Returns (Y f64 [R,d], Hq codes [R,f])."""
+    T8 = e4m3_decode_table()
+    R = int(offsets[-1])
+    f, d = W1q.shape[1], W1q.shape[2]
+    Y = np.zeros((R, d), dtype=np.float64)
+    Hq = np.zeros((R, f), dtype=np.uint8)
+    for e in range(len(offsets) - 1):
+        lo, hi = int(offsets[e]), int(offsets[e + 1])
+        rows = [r for r in range(lo, hi) if row_to_assign[r] >= 0]
+        if not rows:
+            continue
+        x = T8[Xq[rows]]                                            # [n,d] exact e4m3 values
+        sx = row_scale[rows].astype(np.float64)[:, None]
+        g = (x @ T8[W1q[e]].T) * sx * np.float64(s1[e])
+        u = (x @ T8[W3q[e]].T) * sx * np.float64(s3[e])
+        h = g / (1.0 + np.exp(-g)) * u
+        hq = e4m3_encode(h / np.float64(h_scale[e]))
+        Hq[rows] = hq
+        Y[rows] = (T8[hq] @ T8[W2q[e]].T) * np.float64(h_scale[e]) * np.float64(s2[e])
+    return Y, Hq
+
+
+# ======================================================================================
 # parity metrics (F3): max|err| / RMS(ref)  and  mean|err| / mean|ref|
 # ======================================================================================
 
