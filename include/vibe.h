@@ -166,6 +166,34 @@ VIBE_API vibe_status vibe_combine_scattered(const void* Yw, const int32_t* assig
                                             int32_t d, void* out, void* stream);
 
 /* ------------------------------------------------------------------------------------
+ * f2.  The grouped FFN with FP8 (e4m3) operands -- "Precision: FP8" for both evaluated
+ * models (Table 2a); the recipe is DESIGN.md readings Q1-Q4:
+ *   e4m3 = OCP FP8 E4M3 (no infinities, max 448), round-to-nearest-even, saturating;
+ *   scale = binary32(absmax / 448), 1 for an all-zero row / expert; code = e4m3(binary32(x / scale)).
+ *
+ * vibe_fp8_quantize_rows: X bf16 [R,d] -> Xq e4m3 [R,d] (uint8 codes), row_scale f32 [R].   d % 8 == 0.
+ * vibe_fp8_pack_weights : W bf16 [E_loc,K,N] (the layout of W1/W3/W2) -> Wq e4m3 [E_loc,N,K] (K contiguous)
+ *                         and scale f32 [E_loc]; a one-time pass (weights are static in serving).
+ * vibe_grouped_ffn_fp8  : per resident expert e and row r of its segment
+ *        g = sx[r] s1[e] (xq . w1q),  u = sx[r] s3[e] (xq . w3q),  h = silu(g) u,
+ *        Hq[r,:] = e4m3(h / h_scale[e]),   Y[r,:] = bf16( h_scale[e] s2[e] (hq . w2q) )
+ *   e4m3 x e4m3 products accumulated in fp32 on the tensor cores (tcgen05 kind::f8f6f4).
+ *   Xq [R_cap,d], Hq_ws [R_cap,f] e4m3; W1q,W3q [E_loc,f,d], W2q [E_loc,d,f] e4m3; Y [R_cap,d] bf16;
+ *   row_scale [R_cap], s1,s3,s2,h_scale [E_loc] f32 (h_scale: a STATIC, caller-chosen scale of the
+ *   intermediate, e.g. a calibrated absmax / 448).  d % 128 == 0, f % 128 == 0.  All device pointers,
+ *   asynchronous on `stream`, same offsets / ownership / error conventions as vibe_grouped_ffn.
+ * ---------------------------------------------------------------------------------- */
+VIBE_API vibe_status vibe_fp8_quantize_rows(const void* X, int32_t R, int32_t d, void* Xq, float* row_scale,
+                                            void* stream);
+VIBE_API vibe_status vibe_fp8_pack_weights(const void* W, int32_t E_loc, int32_t K, int32_t N, void* Wq,
+                                           float* scale, void* stream);
+VIBE_API vibe_status vibe_grouped_ffn_fp8(const void* Xq, const float* row_scale, const int32_t* offsets,
+                                          int32_t E_loc, int32_t R_cap, int32_t d, int32_t f, const void* W1q,
+                                          const float* s1, const void* W3q, const float* s3, const void* W2q,
+                                          const float* s2, const float* h_scale, void* Hq_ws, void* Y,
+                                          void* stream);
+
+/* ------------------------------------------------------------------------------------
  * a6.  Per-expert latency profile: measured vibe_grouped_ffn time versus tokens per
  * expert, at warmed steady state -- "Each GPU is warmed to steady-state operating
  * conditions and profiled independently using the fused MoE kernel across a range of

@@ -659,7 +659,8 @@ def fp8_pack_weights(W_bits):
         amax = float(np.max(np.abs(W[e])))
         if amax > 0:
             scale[e] = np.float32(amax / E4M3_MAX)
-        codes[e] = e4m3_encode(W[e].T / np.float64(scale[e]))
+        # the quotient is formed in binary32 (Q3), as the kernel does, then rounded ONCE to e4m3
+        codes[e] = e4m3_encode((W[e].T.astype(np.float32) / scale[e]).astype(np.float64))
     return codes, scale
 
 
@@ -672,7 +673,8 @@ def fp8_quantize_rows(X_bits):
         amax = float(np.max(np.abs(X[r]))) if X.shape[1] else 0.0
         if amax > 0:
             scale[r] = np.float32(amax / E4M3_MAX)
-    codes = e4m3_encode(X / scale.astype(np.float64)[:, None]) if R else np.zeros_like(X_bits, dtype=np.uint8)
+    codes = (e4m3_encode((X.astype(np.float32) / scale[:, None]).astype(np.float64)) if R
+             else np.zeros_like(X_bits, dtype=np.uint8))
     return codes, scale
 
 

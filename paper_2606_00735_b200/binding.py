@@ -36,6 +36,7 @@ EXPORTED_SYMBOLS = (
     "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
+    "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -102,6 +103,9 @@ def load() -> C.CDLL:
     lib.vibe_combine.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     lib.vibe_grouped_ffn_scatter.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_combine_scattered.argtypes = [vp, vp, i32, i32, i32, vp, vp]
+    lib.vibe_fp8_quantize_rows.argtypes = [vp, i32, i32, vp, vp, vp]
+    lib.vibe_fp8_pack_weights.argtypes = [vp, i32, i32, i32, vp, vp, vp]
+    lib.vibe_grouped_ffn_fp8.argtypes = [vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vibe_profile_expert_latency.argtypes = [i32, i32, i32, vp, vp, vp, C.POINTER(i32), i32, i32, i32, i32,
                                                 C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
     lib.vibe_moe_layer_forward.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
@@ -137,7 +141,7 @@ def load() -> C.CDLL:
     lib.vibe_placement_swap_refine.argtypes = [C.POINTER(i32), dp, i32, i32, dp, C.POINTER(_LatencyModel), i32,
                                                C.c_double, i32, C.POINTER(i32), C.POINTER(i32)]
     for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_grouped_ffn_scatter",
-                 "vibe_combine_scattered",
+                 "vibe_combine_scattered", "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
                  "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
                  "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
@@ -287,6 +291,54 @@ def combine_scattered(Yw: torch.Tensor, assign_to_row: torch.Tensor, T: int, k: 
     _ok(lib.vibe_combine_scattered(Yw.data_ptr(), assign_to_row.data_ptr(), T, k, d, out.data_ptr(),
                                    _stream(stream)), "vibe_combine_scattered")
     return out
+
+
+# ------------------------------------------------------------------------------------ f2: FP8
+def fp8_quantize_rows(X: torch.Tensor, stream=None):
+    """bf16 [R,d] -> (Xq uint8 e4m3 codes [R,d], row_scale f32 [R])"""
+    lib = load()
+    _check(X, torch.bfloat16, "X")
+    R, d = X.shape
+    Xq = torch.empty((R, d), dtype=torch.uint8, device=X.device)
+    rs = torch.empty((R,), dtype=torch.float32, device=X.device)
+    _ok(lib.vibe_fp8_quantize_rows(X.data_ptr(), R, d, Xq.data_ptr(), rs.data_ptr(), _stream(stream)),
+        "vibe_fp8_quantize_rows")
+    return Xq, rs
+
+
+def fp8_pack_weights(W: torch.Tensor, stream=None):
+    """bf16 [E,K,N] -> (Wq uint8 e4m3 codes [E,N,K], scale f32 [E])"""
+    lib = load()
+    _check(W, torch.bfloat16, "W")
+    E, K, N = W.shape
+    Wq = torch.empty((E, N, K), dtype=torch.uint8, device=W.device)
+    sc = torch.empty((E,), dtype=torch.float32, device=W.device)
+    _ok(lib.vibe_fp8_pack_weights(W.data_ptr(), E, K, N, Wq.data_ptr(), sc.data_ptr(), _stream(stream)),
+        "vibe_fp8_pack_weights")
+    return Wq, sc
+
+
+def grouped_ffn_fp8(Xq, row_scale, offsets, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq=None, Y=None, stream=None):
+    """-> (Y bf16 [R_cap,d], Hq uint8 [R_cap,f])"""
+    lib = load()
+    for t, n in ((Xq, "Xq"), (W1q, "W1q"), (W3q, "W3q"), (W2q, "W2q")):
+        _check(t, torch.uint8, n)
+    for t, n in ((row_scale, "row_scale"), (s1, "s1"), (s3, "s3"), (s2, "s2"), (h_scale, "h_scale")):
+        _check(t, torch.float32, n)
+    _check(offsets, torch.int32, "offsets")
+    Rcap, d = Xq.shape
+    E_loc, f, d1 = W1q.shape
+    if d1 != d or tuple(W3q.shape) != (E_loc, f, d) or tuple(W2q.shape) != (E_loc, d, f):
+        raise VibeError("packed weight shapes must be W1q,W3q [E_loc,f,d], W2q [E_loc,d,f]")
+    if Hq is None:
+        Hq = torch.empty((Rcap, f), dtype=torch.uint8, device=Xq.device)
+    if Y is None:
+        Y = torch.empty((Rcap, d), dtype=torch.bfloat16, device=Xq.device)
+    _ok(lib.vibe_grouped_ffn_fp8(Xq.data_ptr(), row_scale.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f,
+                                 W1q.data_ptr(), s1.data_ptr(), W3q.data_ptr(), s3.data_ptr(), W2q.data_ptr(),
+                                 s2.data_ptr(), h_scale.data_ptr(), Hq.data_ptr(), Y.data_ptr(), _stream(stream)),
+        "vibe_grouped_ffn_fp8")
+    return Y, Hq
 
 
 # ------------------------------------------------------------------------------------ a5

@@ -1,0 +1,543 @@
+// ffn_fp8.cu -- S8(f) f2: the grouped SwiGLU expert FFN with FP8 (e4m3) operands
+// (vibe_grouped_ffn_fp8).  "Precision: FP8" for both evaluated models (Table 2a);
+// recipe = DESIGN.md readings Q1-Q4.
+//
+// Same machine as ffn.cu (swap-AB, 74 CTA pairs, cta_group::2 MMAs of M = 256, warp-uniform TMA /
+// MMA loops, equal token tiles, rotated tile assignment, 2 TMEM accumulator stages) with
+//   * tcgen05.mma kind::f8f6f4: K = 32 per instruction, 128 one-byte elements per 128-byte smem row,
+//     so a K step is 128 deep and moves the same 32 KB per CTA as the bf16 kernel's 64-deep step
+//   * weights pre-quantised AND pre-transposed to [E_loc, N, K] (K contiguous) by vibe_fp8_pack_weights:
+//     both operands K-major, plain SW128 descriptors
+//   * scales on the accumulators in the epilogue: GEMM-1  g = sx[row] s1[e] acc_g, u = sx[row] s3[e] acc_u,
+//     h = silu(g) u, Hq = e4m3(h / sh[e]);  GEMM-2  y = sh[e] s2[e] acc -> bf16
+#include <mutex>
+#include <unordered_map>
+#include <string>
+#include <cstring>
+
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace vibe {
+namespace {
+
+constexpr int BK = 128;                 // K per smem stage (one 128-byte swizzle atom of e4m3)
+constexpr int TN = 256;                 // tokens per tile = max UMMA N
+constexpr int UMMA_K = 32;
+constexpr int STAGES = 6;
+constexpr int ATOM_BYTES = 64 * BK;             // 8 KB : 64 features x 128 K (K-major, SW128)
+constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumulator lanes
+constexpr int B_BYTES = (TN / 2) * BK;          // 16 KB: this CTA's half of the token tile
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
+constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
+constexpr int SX_BYTES = 4 * TN * 4;            // GEMM-1: the tile's row scales, one 1 KB slice per epilogue warp
+// warps: 0 = TMA producer, 1 = MMA issuer, 2.. = epilogue.  GEMM-1 has 4 epilogue warps (its SwiGLU
+// epilogue needs ~200 registers per thread); the down projection has 8 -- two per TMEM lane quarter,
+// alternating 32-column blocks -- because with a short K loop (f = 768: 12 K steps per tile) one warp
+// per quarter could not drain a 256-column accumulator as fast as the tensor pipe fills the next
+// (ncu at the C2 shape: tensor pipe 33 % active with 4 warps).
+__host__ __device__ constexpr int num_threads(int mode) { return mode == 0 ? 192 : 320; }
+constexpr int MAX_SLOTS = 512;
+constexpr int TMEM_COLS = 512;
+
+struct SmemTail {
+  uint64_t full[STAGES];          // leader CTA: both CTAs' TMA bytes of a stage have landed
+  uint64_t empty[STAGES];         // each CTA: the MMAs reading the stage have retired
+  uint64_t tfull[2];              // each CTA: accumulator stage complete
+  uint64_t tempty[2];             // leader CTA: all 8 epilogue warps of the pair drained it
+  uint32_t tmem_base;
+  int32_t total_t_tiles;
+  int32_t off[MAX_SLOTS + 1];     // segment starts (rows)
+  int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
+  int32_t tsz[MAX_SLOTS];         // rows per token tile of the slot (multiple of 16, <= TN)
+};
+constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + SX_BYTES + sizeof(SmemTail);
+static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB dynamic shared memory of sm_100");
+
+struct TileCursor {
+  int e = 0;
+  // tile id -> (slot e, feature block, token tile).  Tile ids are monotone per CTA, so e only advances.
+  __device__ __forceinline__ void decode(const SmemTail* t, int tile, int NB, int& f_blk, int& t_blk) {
+    while (tile >= t->cum[e + 1] * NB) ++e;
+    const int local = tile - t->cum[e] * NB;
+    const int tt = t->cum[e + 1] - t->cum[e];
+    f_blk = local / tt;
+    t_blk = local - f_blk * tt;
+  }
+};
+
+// Tile of CTA pair `pair` in round `rnd`: round r hands out tiles [r*P, (r+1)*P) ROTATED by r.
+// Tile ids stay increasing per pair, every tile is taken exactly once, and a pair does not keep
+// the same position inside a repeating cost pattern (with the plain stride P = 74, a layer whose
+// experts all have a 256-row and a 128-row token tile gave half the pairs only the large tiles).
+__device__ __forceinline__ int tile_of(int rnd, int pair, int P) { return rnd * P + (pair + rnd) % P; }
+
+__device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ float swiglu(float g, float u) { return __fdividef(g, 1.0f + __expf(-g)) * u; }
+
+// Store a 32-lane x 32-column block held one lane (= feature) per thread, v[i] = column
+// (= token) i, into row-major out[token][feature].  Every lane first packs its OWN two tokens
+// (i, i+1) of its feature into one bf16x2 word; lanes 2j / 2j+1 swap that word with one shuffle
+// and a byte permute picks {token i: features f, f+1} in the even lane and {token i+1: f, f+1}
+// in the odd lane -- per token pair: 1 cvt.bf16x2 + 1 shfl + 1 prmt + 1 store (the first version
+// shuffled fp32 values and selected operands with SELs: 365 instructions per block against ~120
+// now, and the down projection at K = 768 was bound by exactly this epilogue).
+__device__ __forceinline__ void store_block_T(const float (&v)[32], __nv_bfloat16* __restrict__ out, size_t ld,
+                                              int row0, int n_rows, int feat, bool feat_ok, int lane) {
+  const int odd = lane & 1;
+  const uint32_t sel = odd ? 0x3276u : 0x5410u;
+  __nv_bfloat16* p = out + (size_t)(row0 + odd) * ld + (feat - odd);
+  const size_t step = 2 * ld;
+  if (n_rows >= 32) {
+#pragma unroll
+    for (int i = 0; i < 32; i += 2) {
+      const uint32_t own = pack2_bf16(v[i], v[i + 1]);
+      const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+      const uint32_t pk = __byte_perm(own, got, sel);
+      if (feat_ok) *reinterpret_cast<uint32_t*>(p) = pk;
+      p += step;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 32; i += 2) {
+      const uint32_t own = pack2_bf16(v[i], v[i + 1]);
+      const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+      const uint32_t pk = __byte_perm(own, got, sel);
+      if (feat_ok && i + odd < n_rows) *reinterpret_cast<uint32_t*>(p) = pk;
+      p += step;
+    }
+  }
+}
+
+// The same transposed store for an e4m3 output (GEMM-1 writes Hq): every lane packs its own two tokens
+// of its feature into an e4m3x2 halfword; one shuffle + byte permute give {token: features f, f+1}.
+__device__ __forceinline__ void store_block_T_e4m3(const float (&v)[32], uint8_t* __restrict__ out, size_t ld, int row0,
+                                                   int n_rows, int feat, bool feat_ok, int lane) {
+  const int odd = lane & 1;
+  const uint32_t sel = odd ? 0x0015u : 0x0040u;   // even: (own.b0, got.b0) = token i;  odd: (got.b1, own.b1) = token i+1
+  uint8_t* p = out + (size_t)(row0 + odd) * ld + (feat - odd);
+  const size_t step = 2 * ld;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    const uint32_t own = ptx::pack2_e4m3(v[i], v[i + 1]);
+    const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+    const uint32_t pk = __byte_perm(own, got, sel);
+    if (feat_ok && i + odd < n_rows) *reinterpret_cast<uint16_t*>(p) = (uint16_t)pk;
+    p += step;
+  }
+}
+
+// kMode: 0 = gate|up + SwiGLU (GEMM-1, writes Hq e4m3), 1 = down (GEMM-2, writes Y bf16).
+template <int kMode>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 1)
+ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
+                 const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
+                 int n_total, int k_total, void* __restrict__ out_v, int ld_out,
+                 const float* __restrict__ row_scale /*GEMM-1: sx [R_cap]*/, const float* __restrict__ sw0 /*[E_loc]*/,
+                 const float* __restrict__ sw1 /*[E_loc] (GEMM-1: W3)*/, const float* __restrict__ h_scale /*[E_loc]*/) {
+  constexpr bool kGateUp = (kMode == 0);
+  constexpr int FB = kGateUp ? 128 : 256;   // output features per pair tile
+  constexpr int FC = FB / 2;                // ... per CTA
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  float* xchg = reinterpret_cast<float*>(smem + (size_t)STAGES * STAGE_BYTES);
+  float* sx_all = reinterpret_cast<float*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES);
+  SmemTail* tail = reinterpret_cast<SmemTail*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + SX_BYTES);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();      // 0 = leader (issues the MMAs)
+  const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
+  const int NB = (n_total + FB - 1) / FB;
+  const int KB = k_total / BK;
+
+  // ------------------------------------------------------------------ setup
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tensormap(&tmAct);
+    ptx::prefetch_tensormap(&tmW0);
+    if (kGateUp) ptx::prefetch_tensormap(&tmW1);
+    for (int s = 0; s < STAGES; ++s) {
+      ptx::mbar_init(ptx::smem_u32(&tail->full[s]), 1);
+      ptx::mbar_init(ptx::smem_u32(&tail->empty[s]), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      ptx::mbar_init(ptx::smem_u32(&tail->tfull[a]), 1);
+      ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 2 * (num_threads(kMode) / 32 - 2));   // epilogue warps of the pair
+    }
+    ptx::fence_barrier_init();
+  } else if (warp == 1) {
+    ptx::tmem_alloc_2sm(ptx::smem_u32(&tail->tmem_base), TMEM_COLS);
+    ptx::tmem_relinquish_2sm();
+  } else if (warp == 2) {
+    // segment starts + exclusive scan of token tiles per slot (warp-shuffle scan, 32 slots a step)
+    int carry = 0;
+    for (int base = 0; base < E_loc; base += 32) {
+      const int e = base + lane;
+      int lo = 0, hi = 0;
+      if (e < E_loc) {
+        lo = offsets[e];
+        hi = offsets[e + 1];
+        tail->off[e] = lo;
+      }
+      // An expert's rows are cut into nt EQUAL token tiles (not 256, 256, ..., remainder): the pairs
+      // that share its weight tile (same feature block, other token tiles) and its activation tile
+      // (same token tile, other feature blocks) then run K steps of the same length and stay in
+      // step, which is what lets L2 serve the second reader.  With a short last tile the readers
+      // drift apart by more than L2 holds and DRAM traffic doubles (measured, profiles/).
+      const int nt = (hi - lo + TN - 1) / TN;
+      if (e < E_loc) tail->tsz[e] = nt > 0 ? ((((hi - lo + nt - 1) / nt) + 15) & ~15) : TN;
+      int inc = nt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int n = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += n;
+      }
+      if (e < E_loc) tail->cum[e] = carry + inc - nt;
+      carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) {
+      tail->cum[E_loc] = carry;
+      tail->off[E_loc] = offsets[E_loc];
+      tail->total_t_tiles = carry;
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::cluster_sync_all();      // the peer's barriers are initialised before anything signals them
+  ptx::tc_fence_after();
+
+  const uint32_t tmem_base = tail->tmem_base;
+  const int total_tiles = tail->total_t_tiles * NB;
+
+  if (warp == 0) {
+    // ================================================================ TMA producer (both CTAs)
+    // The WHOLE warp walks the tile list (warp-uniform control flow and operands); one elected
+    // lane issues the expect_tx and the TMA instructions.
+    {
+      // Both operands are re-read through L2: an activation tile by every feature block of its
+      // expert, a weight tile by the pairs working on the other token tiles of the same expert.
+      // Those pairs are NOT in lock-step (tile costs differ with the ragged N), so a weight line
+      // must survive a few microseconds: evict_first on the weights doubled the DRAM reads
+      // (measured, profiles/), evict_last keeps them at the algorithmic bytes.
+      const uint64_t pol_act = ptx::policy_evict_last();
+      const uint64_t pol_w = ptx::policy_evict_last();
+      const uint32_t smem_base = ptx::smem_u32(smem);
+      const uint32_t full0 = ptx::mapa_u32(ptx::smem_u32(&tail->full[0]), 0);   // the leader's barriers
+      TileCursor cur;
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, tile = tile_of(rnd, pair, num_pairs)) {
+        int f_blk, t_blk;
+        cur.decode(tail, tile, NB, f_blk, t_blk);
+        const int e = cur.e;
+        const int tsz = tail->tsz[e];
+        const int row0 = tail->off[e] + t_blk * tsz;
+        const int n_rows = min(tsz, tail->off[e + 1] - row0);
+        const int half = ((n_rows + 15) >> 4) << 3;          // UMMA N / 2: this CTA's share of the columns
+        const int row_b = row0 + (int)rank * half;
+        const int n0 = f_blk * FB + (int)rank * FC;
+        for (int kb = 0; kb < KB; ++kb) {
+          ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
+          if (ptx::elect_one()) {
+            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), 2 * STAGE_BYTES);
+            const uint32_t full = full0 + (uint32_t)stage * 8u;
+            const uint32_t a_s = smem_base + (uint32_t)stage * STAGE_BYTES;
+            const uint32_t b_s = a_s + A_BYTES;
+            const int k0 = kb * BK;
+            if (kGateUp) {
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, k0, n0, e, pol_w);                 // gate -> lanes 0..63
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, k0, n0, e, pol_w);    // up   -> lanes 64..127
+            } else {
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, k0, n0, e, pol_w);
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, k0, n0 + 64, e, pol_w);
+            }
+            ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================ UMMA issuer (leader CTA)
+    // The whole warp runs the loop; one elected lane issues the MMAs and the commits (always the
+    // same lane: tcgen05.commit tracks the MMAs of the issuing thread).
+    if (rank == 0) {
+      constexpr uint32_t idesc0 = ptx::make_idesc_e4m3_f32(256, 0);
+      // descriptor = constant high word | low word (start address >> 4 in bits [0,14), LBO in [16,30))
+      constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+      const uint32_t smem_base = ptx::smem_u32(smem);
+      const uint32_t a_lo0 = ((smem_base >> 4) & 0x3fffu) | ((16u >> 4) << 16);
+      const uint32_t b_lo0 = (((smem_base + A_BYTES) >> 4) & 0x3fffu) | ((16u >> 4) << 16);
+      TileCursor cur;
+      int stage = 0;
+      uint32_t phase = 0;
+      int it = 0;
+      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
+        int f_blk, t_blk;
+        cur.decode(tail, tile, NB, f_blk, t_blk);
+        const int e = cur.e;
+        const int tsz = tail->tsz[e];
+        const int n_rows = min(tsz, tail->off[e + 1] - (tail->off[e] + t_blk * tsz));
+        const uint32_t n_mma = (uint32_t)((n_rows + 15) >> 4) << 4;
+        const uint32_t idesc = idesc0 | ((n_mma >> 3) << 17);
+        const int acc = it & 1;
+        const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
+        ptx::mbar_wait(ptx::smem_u32(&tail->tempty[acc]), acc_phase ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (uint32_t)acc * TN;
+        for (int kb = 0; kb < KB; ++kb) {
+          ptx::mbar_wait(ptx::smem_u32(&tail->full[stage]), phase);
+          ptx::tc_fence_after();
+          if (ptx::elect_one()) {
+            // A and B: K-major SW128 -> 32 one-byte elements = 32 bytes inside the 128-byte row (+2 in units of 16 B)
+            const uint32_t a_lo = a_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
+            const uint32_t b_lo = b_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
+#pragma unroll
+            for (int k = 0; k < BK / UMMA_K; ++k) {
+              const uint64_t da = ((uint64_t)DESC_HI << 32) | (uint64_t)(a_lo + (uint32_t)k * (UMMA_K / 16));
+              const uint64_t db = ((uint64_t)DESC_HI << 32) | (uint64_t)(b_lo + (uint32_t)k * (UMMA_K / 16));
+              ptx::umma_f8_2sm(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
+            }
+            ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
+            if (kb == KB - 1)
+              ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->tfull[acc]), 3);   // accumulator ready in both CTAs
+          }
+          __syncwarp();
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else {
+    // ================================================================ epilogue (warps 2..5, both CTAs)
+    const int q = warp & 3;  // TMEM lane quarter this warp may access
+    const int blk_par = (warp - 2) >> 2;   // down projection: which 32-column blocks (even / odd) are mine
+    TileCursor cur;
+    int it = 0;
+    for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
+      int f_blk, t_blk;
+      cur.decode(tail, tile, NB, f_blk, t_blk);
+      const int e = cur.e;
+      const int tsz = tail->tsz[e];
+      const int row0 = tail->off[e] + t_blk * tsz;
+      const int n_rows = min(tsz, tail->off[e + 1] - row0);
+      const int acc = it & 1;
+      const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
+      // GEMM-1: the tile's row scales sx go to this warp's slice while the MMAs of the tile still run
+      float* sx = sx_all + (warp - 2) * TN;
+      if (kGateUp) {
+        __syncwarp();                       // the previous tile's reads of the slice are done
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) {
+          const int c = b * 32 + lane;
+          sx[c] = (c < n_rows) ? __ldg(row_scale + row0 + c) : 0.0f;
+        }
+        __syncwarp();
+      }
+      const float se0 = __ldg(sw0 + e);
+      const float se1 = kGateUp ? __ldg(sw1 + e) : 0.0f;
+      const float she = __ldg(h_scale + e);
+      ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
+      ptx::tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
+      if (kGateUp) {
+        // lanes 0..63 gate (q = 0,1), lanes 64..127 up (q = 2,3) of the same 64 features.
+        // Per 64 columns: the gate warp finishes columns 0..31 (needs the partner's up block),
+        // the up warp finishes columns 32..63 (needs the partner's gate block).
+        const bool is_up = q >= 2;
+        const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
+        const bool feat_ok = feat < n_total;
+        float* mine = xchg + ((q & 1) * 2 + (is_up ? 1 : 0)) * 1024;      // block I publish  [col][lane]
+        float* theirs = xchg + ((q & 1) * 2 + (is_up ? 0 : 1)) * 1024;    // block my partner publishes
+        const uint32_t bar_id = 1 + (q & 1);
+        for (int c0 = 0; c0 < n_rows; c0 += 64) {
+          uint32_t a[32], b[32];
+          ptx::tmem_ld_32x32(taddr + c0, a);
+          ptx::tmem_ld_32x32(taddr + c0 + 32, b);
+          ptx::tmem_ld_wait();
+          // publish the block the partner finishes: gate warp -> its gate of cols 32..63; up warp -> its up of cols 0..31
+#pragma unroll
+          for (int i = 0; i < 32; ++i) mine[i * 32 + lane] = __uint_as_float(is_up ? a[i] : b[i]);
+          ptx::named_bar_sync(bar_id, 64);
+          float h[32];
+          const int cbase = c0 + (is_up ? 32 : 0);
+          const float inv_sh = 1.0f / she;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float o = theirs[i * 32 + lane];
+            const float sxi = sx[cbase + i];
+            const float g = (is_up ? o : __uint_as_float(a[i])) * (sxi * se0);
+            const float u = (is_up ? __uint_as_float(b[i]) : o) * (sxi * se1);
+            h[i] = swiglu(g, u) * inv_sh;
+          }
+          ptx::named_bar_sync(bar_id, 64);     // both blocks consumed before the next publish
+          store_block_T_e4m3(h, reinterpret_cast<uint8_t*>(out_v), (size_t)ld_out, row0 + cbase, n_rows - cbase, feat,
+                             feat_ok, lane);
+        }
+      } else {
+        const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
+        const bool feat_ok = feat < n_total;
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) {
+          const int c0 = b * 32;
+          if (c0 >= n_rows) break;
+          if ((b & 1) != blk_par) continue;
+          uint32_t a[32];
+          ptx::tmem_ld_32x32(taddr + c0, a);
+          ptx::tmem_ld_wait();
+          float v[32];
+#pragma unroll
+          for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]) * (she * se0);
+          store_block_T(v, reinterpret_cast<__nv_bfloat16*>(out_v), (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok,
+                        lane);
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa_u32(ptx::smem_u32(&tail->tempty[acc]), 0));
+    }
+  }
+
+  // ------------------------------------------------------------------ teardown
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::cluster_sync_all();      // neither CTA frees TMEM / exits while the peer still uses the pair
+  if (warp == 1) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc_2sm(tmem_base, TMEM_COLS);
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// TMA tensor maps (host).  cuTensorMapEncodeTiled is a driver entry point fetched through
+// the runtime, so libvibe.so does not link libcuda.  Maps are cached for the process
+// lifetime, keyed by (pointer, shape): weights and workspaces are long-lived in serving.
+// ---------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  });
+  return fn;
+}
+
+struct MapKey {
+  const void* ptr;
+  uint64_t d0, d1, d2;
+  uint32_t b0, b1;
+  bool operator==(const MapKey& o) const {
+    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1;
+  }
+};
+struct MapKeyHash {
+  size_t operator()(const MapKey& k) const {
+    size_t h = reinterpret_cast<size_t>(k.ptr);
+    h = h * 1315423911u ^ k.d0;
+    h = h * 1315423911u ^ k.d1;
+    h = h * 1315423911u ^ k.d2;
+    h = h * 1315423911u ^ ((uint64_t)k.b0 << 32 | k.b1);
+    return h;
+  }
+};
+std::mutex g_map_mu;
+std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
+
+// rank 2: dims (d0 inner, d1); rank 3: dims (d0 inner, d1, d2).  One-byte elements, 128-byte swizzle.
+vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t box0, uint32_t box1,
+                           CUtensorMap* out) {
+  MapKey key{ptr, d0, d1, d2, box0, box1};
+  {
+    std::lock_guard<std::mutex> lk(g_map_mu);
+    auto it = g_maps.find(key);
+    if (it != g_maps.end()) {
+      *out = it->second;
+      return VIBE_OK;
+    }
+  }
+  EncodeTiledFn enc = get_encode_fn();
+  VIBE_REQUIRE(enc != nullptr, VIBE_ERR_CUDA, "cuTensorMapEncodeTiled entry point unavailable (no CUDA driver?)");
+  const bool r3 = d2 > 0;
+  cuuint64_t dims[3] = {d0, d1, r3 ? d2 : 1};
+  cuuint64_t strides[2] = {d0, d0 * d1};
+  cuuint32_t box[3] = {box0, box1, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUtensorMap m;
+  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_UINT8, r3 ? 3 : 2, const_cast<void*>(ptr), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  VIBE_REQUIRE(r == CUDA_SUCCESS, VIBE_ERR_CUDA,
+               "cuTensorMapEncodeTiled failed (CUresult %d) ptr=%p dims=(%llu,%llu,%llu) box=(%u,%u)", (int)r, ptr,
+               (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2, box0, box1);
+  {
+    std::lock_guard<std::mutex> lk(g_map_mu);
+    if (g_maps.size() > 4096) g_maps.clear();
+    g_maps[key] = m;
+  }
+  *out = m;
+  return VIBE_OK;
+}
+
+}  // namespace
+
+vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const int32_t* offsets, int E_loc, int R_cap,
+                                 int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
+                                 const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
+                                 cudaStream_t st) {
+  CUtensorMap tmX, tmH, tmW1, tmW3, tmW2;
+  vibe_status s;
+  // activations [R_cap, K] and packed weights [E_loc, N, K]: K innermost, boxes of 128 K x (128 | 64) rows
+  if ((s = get_tensor_map(Xq, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(Hq, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(W1q, d, f, E_loc, BK, 64, &tmW1)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(W3q, d, f, E_loc, BK, 64, &tmW3)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(W2q, f, d, E_loc, BK, 64, &tmW2)) != VIBE_OK) return s;
+  static std::once_flag once;
+  static cudaError_t attr_err = cudaSuccess;
+  std::call_once(once, [] {
+    attr_err = cudaFuncSetAttribute(ffn8_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+    if (attr_err == cudaSuccess)
+      attr_err = cudaFuncSetAttribute(ffn8_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
+  });
+  VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
+               SMEM_BYTES, cudaGetErrorString(attr_err));
+  const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
+  ffn8_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d, Hq, f, row_scale,
+                                                                s1, s3, h_scale);
+  VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<gate_up>");
+  ffn8_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f, Y, d, nullptr, s2,
+                                                                nullptr, h_scale);
+  VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<down>");
+  return VIBE_OK;
+}
+
+}  // namespace vibe
+
+extern "C" vibe_status vibe_grouped_ffn_fp8(const void* Xq, const float* row_scale, const int32_t* offsets,
+                                            int32_t E_loc, int32_t R_cap, int32_t d, int32_t f, const void* W1q,
+                                            const float* s1, const void* W3q, const float* s3, const void* W2q,
+                                            const float* s2, const float* h_scale, void* Hq_ws, void* Y,
+                                            void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(E_loc >= 1 && R_cap >= 1 && d >= 1 && f >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_grouped_ffn_fp8: bad sizes E_loc=%d R_cap=%d d=%d f=%d", E_loc, R_cap, d, f);
+  VIBE_REQUIRE(Xq && row_scale && offsets && W1q && s1 && W3q && s3 && W2q && s2 && h_scale && Hq_ws && Y,
+               VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_fp8: NULL argument");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0, VIBE_ERR_UNSUPPORTED,
+               "vibe_grouped_ffn_fp8: d and f must be multiples of 128 (d=%d f=%d)", d, f);
+  VIBE_REQUIRE(E_loc <= MAX_SLOTS, VIBE_ERR_UNSUPPORTED, "vibe_grouped_ffn_fp8: E_loc > %d not implemented", MAX_SLOTS);
+  VIBE_REQUIRE(aligned16(Xq) && aligned16(W1q) && aligned16(W3q) && aligned16(W2q) && aligned16(Hq_ws) && aligned16(Y),
+               VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_fp8: all tensors must be 16-byte aligned");
+  return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq_ws, Y,
+                              reinterpret_cast<cudaStream_t>(stream));
+}

@@ -486,3 +486,57 @@ def test_ffn_scatter_and_scattered_combine(which):
     mo = O.ffn_error_metrics(go, ref_out)
     bound = 1e-2 * mo["rms_ref"] + 2.0 ** -8 * (ref_abs + np.abs(ref_out))
     assert mo["mean_rel_err"] <= 5e-3 and np.all(np.abs(go - ref_out) <= bound), mo
+
+
+# ================================================================== f2: FP8 (e4m3) quantisers and grouped FFN
+def test_fp8_quantisers_bit_exact():
+    """Codes and scales are integer / bit-level work: bit-exact against the oracle (both sides form the scale and
+    the quotient in binary32 and round once to e4m3)."""
+    rng = I._rng(21, 21)
+    X = I.make_X(300, 512, 7)
+    X[17] = 0                                                    # an all-zero row keeps scale 1
+    X[5, :] = I.f32_to_bf16_bits((rng.standard_normal(512) * 1e-3).astype(np.float32))
+    xq_o, rs_o = O.fp8_quantize_rows(X)
+    xq, rs = B.fp8_quantize_rows(dev_bf16(X))
+    torch.cuda.synchronize()
+    assert np.array_equal(rs.cpu().numpy().view(np.uint32), rs_o.view(np.uint32)), "row scales"
+    assert np.array_equal(xq.cpu().numpy(), xq_o), "activation codes"
+    E, K, N = 3, 160, 96
+    W = np.stack([I.make_expert_weight(1, e, K, N, 0.05 * (e + 1), 8) for e in range(E)])
+    W[1] = 0
+    wq_o, sc_o = O.fp8_pack_weights(W)
+    wq, sc = B.fp8_pack_weights(dev_bf16(W))
+    torch.cuda.synchronize()
+    assert np.array_equal(sc.cpu().numpy().view(np.uint32), sc_o.view(np.uint32)), "expert scales"
+    assert np.array_equal(wq.cpu().numpy(), wq_o), "weight codes / [E,N,K] layout"
+
+
+@pytest.mark.parametrize("T,E,k,d,f", [(64, 8, 2, 256, 512), (700, 4, 2, 384, 256), (300, 16, 4, 128, 128),
+                                       (1500, 2, 1, 512, 640)])
+def test_ffn_fp8_against_oracle(T, E, k, d, f):
+    """vibe_grouped_ffn_fp8 against the oracle's FP8 FFN on the SAME codes and scales.  Hq is an integer code
+    decided by an fp32 value on the GPU and an f64 value in the oracle: codes may differ by one step where the
+    value sits on a rounding boundary (bounded fraction); Y meets the north-star float bars."""
+    cfg = I.scaled(I.C0, T=T, E=E, E_loc=E, k=k, d=d, f=f)
+    L, ids, w, emap, off, r2a, a2r, Xp, R = ffn_case(cfg, 3)
+    W1q, s1 = O.fp8_pack_weights(L["W1"]); W3q, s3 = O.fp8_pack_weights(L["W3"]); W2q, s2 = O.fp8_pack_weights(L["W2"])
+    Xq, rs = O.fp8_quantize_rows(Xp)
+    _, H_bf = O.grouped_ffn(Xp, off, r2a, L["W1"], L["W3"], L["W2"])
+    hs = np.array([max(np.abs(H_bf[off[e]:off[e + 1]]).max(), 1e-6) / 448.0 if off[e + 1] > off[e] else 1.0
+                   for e in range(E)], np.float32)
+    Y_o, Hq_o = O.grouped_ffn_fp8(Xq, rs, off, r2a, W1q, s1, W3q, s3, W2q, s2, hs)
+    Rcap = max(1, B.rows_cap(T, k, E, 1))
+    Xq_d = torch.zeros((Rcap, d), dtype=torch.uint8, device="cuda"); Xq_d[:R] = dev(Xq)
+    rs_d = torch.ones((Rcap,), dtype=torch.float32, device="cuda"); rs_d[:R] = dev(rs)
+    Y, Hq = B.grouped_ffn_fp8(Xq_d, rs_d, dev(off), dev(W1q), dev(s1), dev(W3q), dev(s3), dev(W2q), dev(s2), dev(hs))
+    torch.cuda.synchronize()
+    t8 = O.e4m3_decode_table()
+    hq = Hq.cpu().numpy()[:R]
+    diff = hq != Hq_o
+    assert diff.mean() <= 0.02, f"{diff.mean():.4f} of the Hq codes differ"
+    # where they differ it is by one code step (adjacent e4m3 values, or +-0)
+    a, b = t8[hq[diff]], t8[Hq_o[diff]]
+    step = np.maximum(np.abs(a), np.abs(b)) * 2.0 ** -3 + 2.0 ** -9
+    assert np.all(np.abs(a - b) <= step * 1.0001)
+    m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_o)
+    assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
