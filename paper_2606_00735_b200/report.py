@@ -1,6 +1,6 @@
 """Per-kernel measurements on one B200 beyond the single bench.py line.
 
-    python -m paper_2606_00735_b200.report [--sections stages,ffn,fused,layer,profile,placement,variability,rack,recalibration]
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,fp8,fused,layer,profile,placement,variability,rack,recalibration]
                                            [--out gpurun_out/report.json] [--quick]
 
 Sections (all through the C-ABI binding; seeded synthetic inputs):
@@ -11,6 +11,7 @@ Sections (all through the C-ABI binding; seeded synthetic inputs, DESIGN.md sect
   ffn        grouped FFN on BALANCED routing (every expert n rows), n = 128..4096, for the
              C1/C2/C3 shapes: TFLOP/s and fraction of the measured bf16 peaks -- the
              ">= 512 tokens per expert" target of BASELINE.json is read off this table.
+  fp8        vibe_grouped_ffn_fp8 (e4m3 operands) next to the bf16 kernel, balanced routing.
   fused      vibe_grouped_ffn + vibe_combine versus the fused gate-weighted scatter path
              (vibe_grouped_ffn_scatter + vibe_combine_scattered) on the routed C1 / C2 batches.
   layer      the whole layer through vibe_moe_layer_forward, eager launches versus one CUDA graph.
@@ -239,6 +240,48 @@ def section_layer(peaks, quick):
         out.append({"config": cfg.name, "eager_us": round(eager, 1), "graph_us": round(graph, 1),
                     "tokens_per_s_eager": round(T / eager * 1e6), "tokens_per_s_graph": round(T / graph * 1e6)})
         del W1, W3, W2, Xs, lgs, arena
+        torch.cuda.empty_cache()
+    return out
+
+
+def section_ffn_fp8(peaks, quick):
+    """f2: vibe_grouped_ffn_fp8 on BALANCED routing (every expert n rows) for the C1/C2/C3 shapes, next to the
+    bf16 kernel on the same box in the same run.  FP8 tensor peak = 2 x the measured bf16 peaks (the guide's
+    nominal ratio, as the task's roofline rule prescribes for a dtype without its own measured peak)."""
+    out = []
+    for cfg in (I.C1, I.C2, I.C3):
+        E, d, f = cfg.E_loc, cfg.d, cfg.f
+        W1, W3, W2 = _weights(E, d, f)
+        W1q, s1 = B.fp8_pack_weights(W1)
+        W3q, s3 = B.fp8_pack_weights(W3)
+        W2q, s2 = B.fp8_pack_weights(W2)
+        hs = torch.full((E,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+        for n in ((512, 2048) if quick else (128, 512, 1024, 2048, 4096)):
+            R = E * n
+            Xp = torch.randn((R, d), device="cuda").to(torch.bfloat16)
+            Xq, rs = B.fp8_quantize_rows(Xp)
+            off = (torch.arange(E + 1, device="cuda", dtype=torch.int32) * n).contiguous()
+            Hq = torch.empty((R, f), dtype=torch.uint8, device="cuda")
+            H = torch.empty((R, f), dtype=torch.bfloat16, device="cuda")
+            Y = torch.empty((R, d), dtype=torch.bfloat16, device="cuda")
+            f8 = lambda i: B.grouped_ffn_fp8(Xq, rs, off, W1q, s1, W3q, s3, W2q, s2, hs, Hq=Hq, Y=Y)
+            bf = lambda i: B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y)
+            t0 = time.time()
+            while time.time() - t0 < (0.2 if quick else 1.0):
+                f8(0)
+                torch.cuda.synchronize()
+            iters = 20 if quick else 60
+            t8 = _time(f8, iters)
+            tb = _time(bf, iters)
+            tq = _time(lambda i: B.fp8_quantize_rows(Xp), iters)
+            flops = 6.0 * R * d * f
+            out.append({"shape": cfg.name, "tokens_per_expert": n, "fp8_us": round(t8, 1), "bf16_us": round(tb, 1),
+                        "quantize_rows_us": round(tq, 1), "fp8_TFLOP/s": round(flops / t8 / 1e6, 1),
+                        "bf16_TFLOP/s": round(flops / tb / 1e6, 1), "speedup": round(tb / t8, 3),
+                        "fp8_frac_of_2x_bf16_sustained": round(flops / t8 / 1e6 / (2 * peaks["bf16_tflops_sustained"]), 4),
+                        "fp8_frac_of_2x_bf16_burst": round(flops / t8 / 1e6 / (2 * peaks["bf16_tflops"]), 4)})
+            del Xp, Xq, Hq, H, Y
+        del W1, W3, W2, W1q, W3q, W2q
         torch.cuda.empty_cache()
     return out
 
@@ -514,6 +557,13 @@ def write_markdown(r, path, command):
             med=lambda f: round(st.median(f(y) for y in v),2)
             gt=[y['gain_latency_vs_token'] for y in v]
             o.append(f"| {k_[0]} | {k_[1]} | {k_[2]} | {k_[3]} | {med(lambda y:y['contiguous']['score_us'])} | {med(lambda y:y['token_balanced']['score_us'])} | {med(lambda y:y['latency_balanced']['score_us'])} | {round(st.median(gt),4)} ({min(gt)}..{max(gt)}) | {med(lambda y:y['gain_latency_vs_contiguous'])} |")
+    if "ffn_fp8" in r:
+        o.append("\n## ffn_fp8: vibe_grouped_ffn_fp8 (e4m3 x e4m3, fp32 accumulate) vs vibe_grouped_ffn (bf16), balanced, same run\n")
+        o.append("| shape | tokens/expert | fp8 us | bf16 us | speedup | fp8 TFLOP/s | bf16 TFLOP/s | fp8 / (2 x bf16 sustained) | fp8 / (2 x bf16 burst) | quantize rows us |")
+        o.append("|---|---|---|---|---|---|---|---|---|---|")
+        for x in r["ffn_fp8"]:
+            o.append(f"| {x['shape']} | {x['tokens_per_expert']} | {x['fp8_us']} | {x['bf16_us']} | {x['speedup']} | {x['fp8_TFLOP/s']} | "
+                     f"{x['bf16_TFLOP/s']} | {x['fp8_frac_of_2x_bf16_sustained']} | {x['fp8_frac_of_2x_bf16_burst']} | {x['quantize_rows_us']} |")
     if "layer" in r:
         o.append("\n## layer: vibe_moe_layer_forward (route + permute + grouped FFN + combine), zipf-routed batches, 4 rotating input sets\n")
         o.append("| config | eager us | CUDA graph us | tokens/s eager | tokens/s graph |\n|---|---|---|---|---|")
@@ -549,7 +599,7 @@ def write_markdown(r, path, command):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--sections", default="stages,ffn,fused,layer,profile,placement,variability,rack,recalibration")
+    ap.add_argument("--sections", default="stages,ffn,fp8,fused,layer,profile,placement,variability,rack,recalibration")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--md", default="", help="also write the report as markdown tables (needs all sections)")
@@ -574,6 +624,10 @@ def main():
     if "fused" in want:
         rep["fused_scatter"] = section_fused(peaks, args.quick)
         for r in rep["fused_scatter"]:
+            print(r, flush=True)
+    if "fp8" in want:
+        rep["ffn_fp8"] = section_ffn_fp8(peaks, args.quick)
+        for r in rep["ffn_fp8"]:
             print(r, flush=True)
     if "layer" in want:
         rep["layer"] = section_layer(peaks, args.quick)
