@@ -241,13 +241,25 @@ VIBE_API vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg /*hos
                                                  void* out_h /*host*/, int32_t* counts_h /*host*/, void* arena,
                                                  size_t arena_bytes, void* stream);
 
+/* The whole layer with the FP8 FFN (f2): route -> e4m3 quantisation of the T token rows -> permute (one-byte
+ * rows) -> row-scale gather -> vibe_grouped_ffn_fp8 -> combine.  Packed weights / scales as in
+ * vibe_grouped_ffn_fp8; arena: vibe_workspace_bytes(VIBE_WS_LAYER_FP8, ...) bytes, 256-byte aligned.
+ * out [T,d] bf16, counts [E] i32 (device).  d % 128 == 0, f % 128 == 0. */
+VIBE_API vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg /*host*/, const float* logits,
+                                                const void* X, const int32_t* expert_map, int32_t T, int32_t d,
+                                                int32_t f, int32_t E_loc, const void* W1q, const float* s1,
+                                                const void* W3q, const float* s3, const void* W2q, const float* s2,
+                                                const float* h_scale, void* out, int32_t* counts, void* arena,
+                                                size_t arena_bytes, void* stream);
+
 /* Workspace sizing.  `which` selects the consumer. */
 enum {
   VIBE_WS_PERMUTE = 0,
   VIBE_WS_FFN = 1,
   VIBE_WS_PROFILE = 2, /* T = max tokens per expert of the sweep */
   VIBE_WS_LAYER = 3,
-  VIBE_WS_LAYER_HOST = 4
+  VIBE_WS_LAYER_HOST = 4,
+  VIBE_WS_LAYER_FP8 = 5
 };
 VIBE_API size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int32_t E, int32_t E_loc, int32_t d,
                                      int32_t f, int32_t align);

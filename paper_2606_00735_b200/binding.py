@@ -26,7 +26,7 @@ LIB_PATH = os.path.join(_PKG, "libvibe.so")
 VIBE_OK = 0
 SCORE_SOFTMAX = 0
 SCORE_SIGMOID = 1
-WS_PERMUTE, WS_FFN, WS_PROFILE, WS_LAYER, WS_LAYER_HOST = 0, 1, 2, 3, 4
+WS_PERMUTE, WS_FFN, WS_PROFILE, WS_LAYER, WS_LAYER_HOST, WS_LAYER_FP8 = 0, 1, 2, 3, 4, 5
 MODEL_A, MODEL_B = 0, 1
 
 # every symbol include/vibe.h declares (tests check that the .so exports exactly these)
@@ -36,7 +36,7 @@ EXPORTED_SYMBOLS = (
     "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
-    "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
+    "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -112,6 +112,8 @@ def load() -> C.CDLL:
                                            vp, vp, vp, sz, vp]
     lib.vibe_moe_layer_forward_host.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
                                                 vp, vp, vp, sz, vp]
+    lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
+                                               vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_workspace_bytes.argtypes = [i32] * 8
     lib.vibe_workspace_bytes.restype = sz
     lib.vibe_rows_cap.argtypes = [i32] * 4
@@ -141,7 +143,7 @@ def load() -> C.CDLL:
     lib.vibe_placement_swap_refine.argtypes = [C.POINTER(i32), dp, i32, i32, dp, C.POINTER(_LatencyModel), i32,
                                                C.c_double, i32, C.POINTER(i32), C.POINTER(i32)]
     for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_grouped_ffn_scatter",
-                 "vibe_combine_scattered", "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
+                 "vibe_combine_scattered", "vibe_moe_layer_forward_fp8", "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
                  "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
                  "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
@@ -409,6 +411,32 @@ def moe_layer_forward(cfg: RouteConfig, logits, X, expert_map, W1, W3, W2, out=N
                                    topk_ids.data_ptr() if topk_ids is not None else None,
                                    topk_w.data_ptr() if topk_w is not None else None, arena.data_ptr(),
                                    arena.numel(), _stream(stream)), "vibe_moe_layer_forward")
+    return out, counts
+
+
+def moe_layer_forward_fp8(cfg: RouteConfig, logits, X, expert_map, W1q, s1, W3q, s3, W2q, s2, h_scale, out=None,
+                          counts=None, arena=None, stream=None):
+    """The whole layer with the FP8 FFN (weights packed by fp8_pack_weights)."""
+    lib = load()
+    _check(logits, torch.float32, "logits")
+    _check(X, torch.bfloat16, "X")
+    T, d = X.shape
+    E_loc, f, _ = W1q.shape
+    dev = X.device
+    if out is None:
+        out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+    if counts is None:
+        counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
+    need = workspace_bytes(WS_LAYER_FP8, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
+    if arena is None:
+        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+    c = cfg._c()
+    _ok(lib.vibe_moe_layer_forward_fp8(C.byref(c), logits.data_ptr(), X.data_ptr(),
+                                       expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
+                                       W1q.data_ptr(), s1.data_ptr(), W3q.data_ptr(), s3.data_ptr(), W2q.data_ptr(),
+                                       s2.data_ptr(), h_scale.data_ptr(), out.data_ptr(), counts.data_ptr(),
+                                       arena.data_ptr(), arena.numel(), _stream(stream)),
+        "vibe_moe_layer_forward_fp8")
     return out, counts
 
 

@@ -54,6 +54,33 @@ LayerArena layer_arena(int T, int k, int E_loc, int d, int f) {
   return a;
 }
 
+LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f) {
+  LayerArenaFp8 a{};
+  const size_t A = (size_t)T * k;
+  a.R_cap = vibe_rows_cap(T, k, E_loc, 1);
+  if (a.R_cap < 1) a.R_cap = 1;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o += round_up(bytes ? bytes : 16, 256);
+    return at;
+  };
+  a.ids = take(A * 4);
+  a.w = take(A * 4);
+  a.offsets = take((size_t)(E_loc + 1) * 4);
+  a.r2a = take((size_t)a.R_cap * 4);
+  a.a2r = take(A * 4);
+  a.Xq = take((size_t)T * d);
+  a.tok_scale = take((size_t)T * 4);
+  a.Xpq = take((size_t)a.R_cap * d);
+  a.row_scale = take((size_t)a.R_cap * 4);
+  a.Hq = take((size_t)a.R_cap * f);
+  a.Y = take((size_t)a.R_cap * d * 2);
+  a.perm_ws = take(permute_ws_bytes(T, k, E_loc));
+  a.total = o;
+  return a;
+}
+
 }  // namespace vibe
 
 extern "C" const char* vibe_status_string(vibe_status s) {
@@ -83,6 +110,7 @@ extern "C" size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int3
       return round_up(R * d * 2, 256) * 2 + round_up(R * f * 2, 256) + round_up((size_t)(E_loc + 1) * 4, 256);
     }
     case VIBE_WS_LAYER: return layer_arena(T, k, E_loc, d, f).total;
+    case VIBE_WS_LAYER_FP8: return layer_arena_fp8(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_HOST:
       return layer_arena(T, k, E_loc, d, f).total + round_up((size_t)T * E * 4, 256) +
              round_up((size_t)T * d * 2, 256) * 2 + round_up((size_t)E * 4, 256);

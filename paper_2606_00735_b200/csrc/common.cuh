@@ -59,6 +59,14 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
 vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                               const void* W1, const void* W3, const void* W2, void* H_ws, void* Y);
 
+vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_assign, const int32_t* offsets, int E_loc,
+                                  int k, int R_cap, float* row_scale, cudaStream_t st);
+struct LayerArenaFp8 {
+  size_t ids, w, offsets, r2a, a2r, Xq, tok_scale, Xpq, row_scale, Hq, Y, perm_ws, total;
+  int64_t R_cap;
+};
+LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f);
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

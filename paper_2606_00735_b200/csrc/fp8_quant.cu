@@ -89,7 +89,34 @@ __global__ void fp8_finish_scales_kernel(float* __restrict__ scale, int E) {
   if (e < E) scale[e] = scale_of(scale[e]);
 }
 
+// row_scale[r] = scale of the token behind permuted row r (1 for padding rows and rows past the last segment)
+__global__ void __launch_bounds__(256) fp8_gather_row_scales_kernel(const float* __restrict__ tok_scale,
+                                                                    const int32_t* __restrict__ row_to_assign,
+                                                                    const int32_t* __restrict__ offsets, int E_loc, int k,
+                                                                    int R_cap, float* __restrict__ row_scale) {
+  const int R = __ldg(offsets + E_loc);
+  for (int r = blockIdx.x * 256 + threadIdx.x; r < R_cap; r += gridDim.x * 256) {
+    float s = 1.0f;
+    if (r < R) {
+      const int i = __ldg(row_to_assign + r);
+      if (i >= 0) s = __ldg(tok_scale + i / k);
+    }
+    row_scale[r] = s;
+  }
+}
+
 }  // namespace
+
+vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_assign, const int32_t* offsets, int E_loc,
+                                  int k, int R_cap, float* row_scale, cudaStream_t st) {
+  int blocks = (R_cap + 255) / 256;
+  if (blocks > num_sms() * 8) blocks = num_sms() * 8;
+  if (blocks < 1) blocks = 1;
+  fp8_gather_row_scales_kernel<<<blocks, 256, 0, st>>>(tok_scale, row_to_assign, offsets, E_loc, k, R_cap, row_scale);
+  VIBE_LAUNCH_CHECK("fp8_gather_row_scales_kernel");
+  return VIBE_OK;
+}
+
 }  // namespace vibe
 
 extern "C" vibe_status vibe_fp8_quantize_rows(const void* X, int32_t R, int32_t d, void* Xq, float* row_scale,
