@@ -237,9 +237,27 @@ def section_layer(peaks, quick):
         torch.cuda.synchronize()
         eager = e0.elapsed_time(e1) * 1e3 / iters
         graph = _time(layer, iters, period=nsets)
-        out.append({"config": cfg.name, "eager_us": round(eager, 1), "graph_us": round(graph, 1),
-                    "tokens_per_s_eager": round(T / eager * 1e6), "tokens_per_s_graph": round(T / graph * 1e6)})
-        del W1, W3, W2, Xs, lgs, arena
+        row = {"config": cfg.name, "eager_us": round(eager, 1), "graph_us": round(graph, 1),
+               "tokens_per_s_eager": round(T / eager * 1e6), "tokens_per_s_graph": round(T / graph * 1e6)}
+        # the same layer with the FP8 FFN (weights packed once, outside the timed region)
+        W1q, s1 = B.fp8_pack_weights(W1)
+        W3q, s3 = B.fp8_pack_weights(W3)
+        W2q, s2 = B.fp8_pack_weights(W2)
+        hs = torch.full((E_loc,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+        arena8 = torch.empty((B.workspace_bytes(B.WS_LAYER_FP8, T, k, E, E_loc, d, f),), dtype=torch.uint8, device="cuda")
+
+        def layer8(i):
+            B.moe_layer_forward_fp8(rc, lgs[i % nsets], Xs[i % nsets], emap, W1q, s1, W3q, s3, W2q, s2, hs, out=o,
+                                    counts=cnt, arena=arena8)
+
+        for i in range(8):
+            layer8(i)
+        torch.cuda.synchronize()
+        g8 = _time(layer8, iters, period=nsets)
+        row.update({"fp8_graph_us": round(g8, 1), "fp8_tokens_per_s_graph": round(T / g8 * 1e6),
+                    "fp8_speedup": round(graph / g8, 3)})
+        out.append(row)
+        del W1, W3, W2, Xs, lgs, arena, W1q, W3q, W2q, arena8
         torch.cuda.empty_cache()
     return out
 
@@ -566,9 +584,10 @@ def write_markdown(r, path, command):
                      f"{x['bf16_TFLOP/s']} | {x['fp8_frac_of_2x_bf16_sustained']} | {x['fp8_frac_of_2x_bf16_burst']} | {x['quantize_rows_us']} |")
     if "layer" in r:
         o.append("\n## layer: vibe_moe_layer_forward (route + permute + grouped FFN + combine), zipf-routed batches, 4 rotating input sets\n")
-        o.append("| config | eager us | CUDA graph us | tokens/s eager | tokens/s graph |\n|---|---|---|---|---|")
+        o.append("| config | bf16 eager us | bf16 CUDA graph us | tokens/s eager | tokens/s graph | FP8 layer (vibe_moe_layer_forward_fp8) graph us | FP8 tokens/s | FP8 / bf16 |\n|---|---|---|---|---|---|---|---|")
         for x in r["layer"]:
-            o.append(f"| {x['config']} | {x['eager_us']} | {x['graph_us']} | {x['tokens_per_s_eager']} | {x['tokens_per_s_graph']} |")
+            o.append(f"| {x['config']} | {x['eager_us']} | {x['graph_us']} | {x['tokens_per_s_eager']} | {x['tokens_per_s_graph']} | "
+                     f"{x.get('fp8_graph_us')} | {x.get('fp8_tokens_per_s_graph')} | {x.get('fp8_speedup')} |")
     if "variability" in r:
         v = r["variability"]
         o.append("\n## variability: " + str(v["executions"]) + " consecutive executions, " + v["shape"] +
