@@ -217,6 +217,17 @@ VIBE_API vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int32
                                                  float* latency_us /*host*/, float* samples_us /*host|NULL*/,
                                                  void* ws, size_t ws_bytes, void* stream);
 
+/* a6 in the paper's precision (f2): the same profile of vibe_grouped_ffn_fp8 (packed weights and scales as there).
+ * ws: vibe_workspace_bytes(VIBE_WS_PROFILE, T = max tokens_per_expert, ...) rounded up to 256, plus
+ * 4 * E_loc * max(tokens_per_expert) rounded up to 256 bytes. */
+VIBE_API vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
+                                                     const float* s1, const void* W3q, const float* s3,
+                                                     const void* W2q, const float* s2, const float* h_scale,
+                                                     const int32_t* tokens_per_expert /*host*/, int32_t n_points,
+                                                     int32_t mode, int32_t warmup, int32_t iters,
+                                                     float* latency_us /*host*/, float* samples_us /*host|NULL*/,
+                                                     void* ws, size_t ws_bytes, void* stream);
+
 /* ------------------------------------------------------------------------------------
  * The whole layer (a1..a5) as one call: enqueues route -> permute -> grouped FFN ->
  * combine on `stream` using one caller-provided device arena.

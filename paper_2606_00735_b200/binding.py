@@ -37,6 +37,7 @@ EXPORTED_SYMBOLS = (
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
+    "vibe_profile_expert_latency_fp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -108,6 +109,8 @@ def load() -> C.CDLL:
     lib.vibe_grouped_ffn_fp8.argtypes = [vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vibe_profile_expert_latency.argtypes = [i32, i32, i32, vp, vp, vp, C.POINTER(i32), i32, i32, i32, i32,
                                                 C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
+    lib.vibe_profile_expert_latency_fp8.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, C.POINTER(i32), i32, i32, i32,
+                                                    i32, C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
     lib.vibe_moe_layer_forward.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                            vp, vp, vp, sz, vp]
     lib.vibe_moe_layer_forward_host.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
@@ -144,7 +147,7 @@ def load() -> C.CDLL:
                                                C.c_double, i32, C.POINTER(i32), C.POINTER(i32)]
     for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_grouped_ffn_scatter",
                  "vibe_combine_scattered", "vibe_moe_layer_forward_fp8", "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
-                 "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
+                 "vibe_profile_expert_latency", "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
                  "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
                  "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine"):
@@ -386,6 +389,25 @@ def profile_expert_latency(W1: torch.Tensor, W3: torch.Tensor, W2: torch.Tensor,
     if return_samples:
         return lat_np, np.array(samples[:], dtype=np.float64).reshape(npts, iters)
     return lat_np
+
+
+def profile_expert_latency_fp8(W1q, s1, W3q, s3, W2q, s2, h_scale, tokens_per_expert: Sequence[int] = DEFAULT_SWEEP,
+                               mode: int = 0, warmup: int = 10, iters: int = 100, stream=None):
+    """vibe_profile_expert_latency for the FP8 FFN (median latency [us] per sweep point)."""
+    lib = load()
+    E_loc, f, d = W1q.shape
+    toks = (C.c_int32 * len(tokens_per_expert))(*[int(x) for x in tokens_per_expert])
+    npts = len(tokens_per_expert)
+    lat = (C.c_float * npts)()
+    nmax = max(tokens_per_expert)
+    need = (workspace_bytes(WS_PROFILE, nmax, 1, E_loc, E_loc, d, f, 1) + 255) // 256 * 256 + \
+        (4 * E_loc * max(nmax, 1) + 255) // 256 * 256
+    ws = torch.empty((need,), dtype=torch.uint8, device=W1q.device)
+    _ok(lib.vibe_profile_expert_latency_fp8(E_loc, d, f, W1q.data_ptr(), s1.data_ptr(), W3q.data_ptr(), s3.data_ptr(),
+                                            W2q.data_ptr(), s2.data_ptr(), h_scale.data_ptr(), toks, npts, mode, warmup,
+                                            iters, lat, None, ws.data_ptr(), ws.numel(), _stream(stream)),
+        "vibe_profile_expert_latency_fp8")
+    return np.array(lat[:], dtype=np.float64)
 
 
 # ------------------------------------------------------------------------------------ layer

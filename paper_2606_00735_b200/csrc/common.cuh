@@ -56,6 +56,10 @@ size_t permute_ws_bytes(int T, int k, int E_loc);
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y, cudaStream_t st,
                              const int32_t* row_to_assign = nullptr, const float* topk_w = nullptr);
+vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const int32_t* offsets, int E_loc, int R_cap,
+                                 int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
+                                 const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
+                                 cudaStream_t st);
 vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                               const void* W1, const void* W3, const void* W2, void* H_ws, void* Y);
 

@@ -19,6 +19,61 @@ __global__ void fill_pattern_kernel(__nv_bfloat16* p, size_t n) {
     p[i] = __float2bfloat16_rn(((int)(h & 0xffff) - 32768) * (1.0f / 32768.0f));
   }
 }
+__global__ void fill_ones_kernel(float* p, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 1.0f;
+}
+}  // namespace
+}  // namespace vibe
+
+namespace vibe {
+namespace {
+// the sweep itself: per point upload the offsets, `warmup` untimed + `iters` timed calls of run(), median
+template <class Run>
+vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_points, int mode, int warmup, int iters,
+                          float* latency_us, float* samples_us, int32_t* offsets, cudaStream_t st, Run run) {
+  std::vector<cudaEvent_t> ev(2 * (size_t)iters);
+  for (auto& e : ev) VIBE_CUDA(cudaEventCreate(&e));
+  std::vector<int32_t> off(E_loc + 1);
+  std::vector<float> t(iters);
+  vibe_status rc = VIBE_OK;
+  for (int p = 0; p < n_points && rc == VIBE_OK; ++p) {
+    const int n = tokens_per_expert[p];
+    off[0] = 0;
+    for (int e = 0; e < E_loc; ++e) off[e + 1] = off[e] + ((mode == 0 || e == 0) ? n : 0);
+    cudaError_t ce = cudaMemcpyAsync(offsets, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) {
+      set_error("vibe_profile_expert_latency: offsets upload failed: %s", cudaGetErrorString(ce));
+      rc = VIBE_ERR_CUDA;
+      break;
+    }
+    for (int i = 0; i < warmup && rc == VIBE_OK; ++i)
+      rc = run();
+    for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
+      cudaEventRecord(ev[2 * i], st);
+      rc = run();
+      cudaEventRecord(ev[2 * i + 1], st);
+    }
+    if (rc != VIBE_OK) break;
+    ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) {
+      set_error("vibe_profile_expert_latency: kernel failed: %s", cudaGetErrorString(ce));
+      rc = VIBE_ERR_CUDA;
+      break;
+    }
+    for (int i = 0; i < iters; ++i) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]);
+      t[i] = ms * 1000.0f;
+      if (samples_us) samples_us[(size_t)p * iters + i] = t[i];
+    }
+    std::sort(t.begin(), t.end());
+    const float med = (iters & 1) ? t[iters / 2] : 0.5f * (t[iters / 2 - 1] + t[iters / 2]);
+    latency_us[p] = (mode == 0) ? med / (float)E_loc : med;
+  }
+  for (auto& e : ev) cudaEventDestroy(e);
+  return rc;
+}
 }  // namespace
 }  // namespace vibe
 
@@ -57,46 +112,53 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
   fill_pattern_kernel<<<num_sms() * 4, 256, 0, st>>>(reinterpret_cast<__nv_bfloat16*>(Xp), (size_t)R_cap * d);
   VIBE_LAUNCH_CHECK("fill_pattern_kernel");
 
-  std::vector<cudaEvent_t> ev(2 * (size_t)iters);
-  for (auto& e : ev) VIBE_CUDA(cudaEventCreate(&e));
-  std::vector<int32_t> off(E_loc + 1);
-  std::vector<float> t(iters);
-  vibe_status rc = VIBE_OK;
-  for (int p = 0; p < n_points && rc == VIBE_OK; ++p) {
-    const int n = tokens_per_expert[p];
-    off[0] = 0;
-    for (int e = 0; e < E_loc; ++e) off[e + 1] = off[e] + ((mode == 0 || e == 0) ? n : 0);
-    cudaError_t ce = cudaMemcpyAsync(offsets, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-    if (ce != cudaSuccess) {
-      set_error("vibe_profile_expert_latency: offsets upload failed: %s", cudaGetErrorString(ce));
-      rc = VIBE_ERR_CUDA;
-      break;
-    }
-    for (int i = 0; i < warmup && rc == VIBE_OK; ++i)
-      rc = grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st);
-    for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
-      cudaEventRecord(ev[2 * i], st);
-      rc = grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st);
-      cudaEventRecord(ev[2 * i + 1], st);
-    }
-    if (rc != VIBE_OK) break;
-    ce = cudaStreamSynchronize(st);
-    if (ce != cudaSuccess) {
-      set_error("vibe_profile_expert_latency: kernel failed: %s", cudaGetErrorString(ce));
-      rc = VIBE_ERR_CUDA;
-      break;
-    }
-    for (int i = 0; i < iters; ++i) {
-      float ms = 0.f;
-      cudaEventElapsedTime(&ms, ev[2 * i], ev[2 * i + 1]);
-      t[i] = ms * 1000.0f;
-      if (samples_us) samples_us[(size_t)p * iters + i] = t[i];
-    }
-    std::sort(t.begin(), t.end());
-    const float med = (iters & 1) ? t[iters / 2] : 0.5f * (t[iters / 2 - 1] + t[iters / 2]);
-    latency_us[p] = (mode == 0) ? med / (float)E_loc : med;
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st,
+                       [&]() { return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st); });
+}
+
+extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
+                                                       const float* s1, const void* W3q, const float* s3,
+                                                       const void* W2q, const float* s2, const float* h_scale,
+                                                       const int32_t* tokens_per_expert, int32_t n_points,
+                                                       int32_t mode, int32_t warmup, int32_t iters, float* latency_us,
+                                                       float* samples_us, void* ws, size_t ws_bytes, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(tokens_per_expert && latency_us && n_points >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_fp8: need tokens_per_expert, latency_us, n_points >= 1");
+  VIBE_REQUIRE(mode == 0 || mode == 1, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency_fp8: mode must be 0 or 1");
+  VIBE_REQUIRE(warmup >= 0 && iters >= 1 && iters <= 100000, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_fp8: need warmup >= 0, 1 <= iters <= 100000");
+  VIBE_REQUIRE(W1q && s1 && W3q && s3 && W2q && s2 && h_scale, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_fp8: NULL weights / scales");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0 && E_loc >= 1, VIBE_ERR_UNSUPPORTED,
+               "vibe_profile_expert_latency_fp8: d and f must be multiples of 128");
+  int n_max = 0;
+  for (int p = 0; p < n_points; ++p) {
+    VIBE_REQUIRE(tokens_per_expert[p] >= 0, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency_fp8: negative token count");
+    n_max = std::max(n_max, tokens_per_expert[p]);
   }
-  for (auto& e : ev) cudaEventDestroy(e);
-  return rc;
+  VIBE_REQUIRE((int64_t)E_loc * std::max(n_max, 1) < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_fp8: E_loc * max tokens >= 2^31");
+  const int R_cap = E_loc * std::max(n_max, 1);
+  const size_t base_need = round_up(vibe_workspace_bytes(VIBE_WS_PROFILE, n_max, 1, E_loc, E_loc, d, f, 1), 256);
+  const size_t need = base_need + round_up((size_t)R_cap * 4, 256);
+  VIBE_REQUIRE(ws != nullptr && ws_bytes >= need && (reinterpret_cast<uintptr_t>(ws) & 255u) == 0, VIBE_ERR_WORKSPACE,
+               "vibe_profile_expert_latency_fp8: workspace needs %zu bytes, 256-byte aligned (got %zu)", need, ws_bytes);
+  // the bf16 profile's workspace layout with one-byte activations (Xq | Y | Hq | offsets), row scales appended
+  char* base = reinterpret_cast<char*>(ws);
+  void* Xq = base;
+  void* Y = base + round_up((size_t)R_cap * d * 2, 256);
+  char* Hreg = base + 2 * round_up((size_t)R_cap * d * 2, 256);
+  void* Hq = Hreg;
+  int32_t* offsets = reinterpret_cast<int32_t*>(Hreg + round_up((size_t)R_cap * f * 2, 256));
+  float* row_scale = reinterpret_cast<float*>(base + base_need);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  // arbitrary finite codes (0x38 = 1.0) and unit row scales: latency does not depend on the values
+  VIBE_CUDA(cudaMemsetAsync(Xq, 0x38, (size_t)R_cap * d, st));
+  fill_ones_kernel<<<num_sms() * 2, 256, 0, st>>>(row_scale, (size_t)R_cap);
+  VIBE_LAUNCH_CHECK("fill_ones_kernel");
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st, [&]() {
+    return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, st);
+  });
 }

@@ -364,6 +364,17 @@ def section_profile(peaks, quick):
                              "p10_us": round(float(np.percentile(samples[j], 10)), 3),
                              "p90_us": round(float(np.percentile(samples[j], 90)), 3),
                              "weight_stream_floor_us": round(floor_us, 3) if mode == 0 else None})
+        # the same sweep for the FP8 FFN (mode 0): the per-GPU performance model in the paper's precision
+        W1q, s1 = B.fp8_pack_weights(W1)
+        W3q, s3 = B.fp8_pack_weights(W3)
+        W2q, s2 = B.fp8_pack_weights(W2)
+        hs = torch.full((E,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+        lat8 = B.profile_expert_latency_fp8(W1q, s1, W3q, s3, W2q, s2, hs, B.DEFAULT_SWEEP[::-1], mode=0,
+                                            warmup=10 if quick else 30, iters=20 if quick else 100)[::-1]
+        m0 = [r for r in rows if r["mode"] == 0]
+        for j, r in enumerate(m0):
+            r["fp8_latency_us"] = round(float(lat8[j]), 3)
+        del W1q, W3q, W2q
         out[cfg.name] = {"E_loc": E, "d": d, "f": f, "rows": rows}
         del W1, W3, W2
         torch.cuda.empty_cache()
@@ -557,12 +568,12 @@ def write_markdown(r, path, command):
         o.append("\n## profile: per-expert latency l(n) [us], median of 100 calls per point (p10..p90), modes 0 (all experts n rows; time / E_loc) and 1 (one expert n rows)\n")
         for name,p in r['profile'].items():
             o.append(f"### {name}: E_loc={p['E_loc']} d={p['d']} f={p['f']}\n")
-            o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 |\n|---|---|---|---|---|---|---|---|")
+            o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 | FP8 mode 0 us |\n|---|---|---|---|---|---|---|---|---|")
             m0={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==0}
             m1={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==1}
             for n in sorted(m0):
                 a,b=m0[n],m1[n]
-                o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} |")
+                o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} | {a.get('fp8_latency_us')} |")
             o.append("")
     if "placement_stress" in r:
         o.append("## placement_stress (BASELINE.json configs[4]): 256 experts -> 8 virtual GPUs, sigma ~ U[0.78,1.0] (8 seeds), measured C3-shape profile\n")

@@ -577,3 +577,18 @@ def test_layer_forward_fp8_against_oracle(which):
     assert m["mean_rel_err"] <= 2 * FFN_MEAN, m
     bound = 2e-2 * m["rms_ref"] + BF16_U * ref_abs + BF16_U * np.abs(ref)
     assert np.all(np.abs(got - ref) <= bound), (np.max(np.abs(got - ref) / bound), m)
+
+
+def test_profile_expert_latency_fp8_sanity():
+    """a6 for the FP8 FFN: positive, finite, growing with n, and faster than the bf16 profile at large n."""
+    cfg = I.scaled(I.C2, E=16, E_loc=16)
+    Wb = [dev_bf16(x) for x in I.make_weights(cfg.E_loc, cfg.d, cfg.f, 0)]
+    (W1q, s1), (W3q, s3), (W2q, s2) = (B.fp8_pack_weights(w) for w in Wb)
+    hs = torch.full((cfg.E_loc,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+    sweep = [1, 128, 2048]
+    lat8 = B.profile_expert_latency_fp8(W1q, s1, W3q, s3, W2q, s2, hs, sweep, mode=0, warmup=3, iters=15)
+    latb = B.profile_expert_latency(Wb[0], Wb[1], Wb[2], sweep, mode=0, warmup=3, iters=15)
+    assert lat8.shape == (3,) and np.all(lat8 > 0) and np.all(np.isfinite(lat8))
+    assert lat8[2] > lat8[0] and lat8[2] < latb[2]
+    flops = 6.0 * 2048 * cfg.d * cfg.f
+    assert lat8[2] * 1e-6 >= flops / 4.5e15          # cannot beat the nominal dense fp8 peak
