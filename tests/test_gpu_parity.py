@@ -289,6 +289,8 @@ def test_ffn_tiles_and_tails(T, E, k, d, f, align):
     ([1, 15, 16, 17, 0, 31, 33, 255], 128, 256),          # every N granule edge of the swap-AB tile (N = roundup(n,16))
     ([256, 257, 511, 513, 0, 0, 2, 768], 256, 128),       # full token tiles + 1-row / 255-row tails, empty slots
     ([3] * 70 + [0] * 30 + [40] * 28, 64, 192),           # 128 slots: the slot scan spans several 32-lane steps
+    ([4100, 790, 1000, 0, 385], 128, 1024),               # equal token tiles (17 x 256 with 4 rows in the last, 4 x 208,
+                                                          # 4 x 256, 2 x 208) and 216 / 54 tiles: several rotated rounds
 ])
 def test_ffn_ragged_token_tiles(rows, d, f):
     """Segment lengths chosen around the UMMA-N granule (16), the CTA-pair split (N/2) and the
@@ -592,3 +594,25 @@ def test_profile_expert_latency_fp8_sanity():
     assert lat8[2] > lat8[0] and lat8[2] < latb[2]
     flops = 6.0 * 2048 * cfg.d * cfg.f
     assert lat8[2] * 1e-6 >= flops / 4.5e15          # cannot beat the nominal dense fp8 peak
+
+
+@pytest.mark.parametrize("rows,d,f", [([1, 15, 16, 17, 0, 31, 33, 255], 128, 256), ([4100, 790, 0, 385], 128, 512)])
+def test_ffn_fp8_ragged_token_tiles(rows, d, f):
+    """The FP8 kernel shares the tile logic of the bf16 kernel but not its epilogues: the same ragged segments."""
+    E = len(rows)
+    off = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    R = int(off[-1])
+    Xp = I.make_X(R, d, 79)
+    W1, W3, W2 = I.make_weights(E, d, f, 80)
+    r2a = np.arange(R, dtype=np.int32)
+    W1q, s1 = O.fp8_pack_weights(W1); W3q, s3 = O.fp8_pack_weights(W3); W2q, s2 = O.fp8_pack_weights(W2)
+    Xq, rs = O.fp8_quantize_rows(Xp)
+    hs = np.full(E, 6.0 / 448.0, np.float32)
+    Y_o, Hq_o = O.grouped_ffn_fp8(Xq, rs, off, r2a, W1q, s1, W3q, s3, W2q, s2, hs)
+    Xq_d = torch.full((R + 300, d), 0x7E, dtype=torch.uint8, device="cuda"); Xq_d[:R] = dev(Xq)      # 448s past the end
+    rs_d = torch.full((R + 300,), 1e30, dtype=torch.float32, device="cuda"); rs_d[:R] = dev(rs)
+    Y, Hq = B.grouped_ffn_fp8(Xq_d, rs_d, dev(off), dev(W1q), dev(s1), dev(W3q), dev(s3), dev(W2q), dev(s2), dev(hs))
+    torch.cuda.synchronize()
+    assert (Hq.cpu().numpy()[:R] != Hq_o).mean() <= 0.02
+    m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_o)
+    assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
