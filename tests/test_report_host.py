@@ -1,0 +1,32 @@
+"""CPU-only checks of the reporting helpers (no GPU work): the markdown writer accepts partial reports."""
+import os
+
+from paper_2606_00735_b200 import report
+
+
+def test_write_markdown_with_partial_and_full_sections(tmp_path):
+    rep = {"peaks": {"kind": "measured", "hbm_gbs": 6533.2, "bf16_tflops": 1665.5, "bf16_tflops_sustained": 1401.3},
+           "gpu": "NVIDIA B200"}
+    p = tmp_path / "a.md"
+    report.write_markdown(rep, str(p), "cmd")
+    assert "Peaks (measured" in p.read_text()
+    stage = {"us": 1.0, "GB/s": 2.0, "frac_hbm": 0.5}
+    rep.update({
+        "stages": [{"config": "C1", "T": 1, "E": 8, "E_loc": 8, "k": 2, "d": 64, "real_rows": 2, "route": stage,
+                    "permute": stage, "combine": stage}],
+        "ffn_balanced": [{"shape": "C1", "E_loc": 8, "d": 64, "f": 64, "tokens_per_expert": 512, "us_per_expert": 1.0,
+                          "TFLOP/s": 1.0, "frac_sustained": 0.1, "frac_burst": 0.1, "frac_of_per_expert_roofline": 0.1}],
+        "fused_scatter": [{"config": "C1", "ffn_plus_combine_us": 1.0, "fused_scatter_us": 1.0, "speedup": 1.0}],
+        "layer": [{"config": "C1", "eager_us": 1.0, "graph_us": 1.0, "tokens_per_s_eager": 1, "tokens_per_s_graph": 1}],
+        "profile": {"C2": {"E_loc": 2, "d": 64, "f": 64, "rows": [
+            {"mode": 0, "tokens_per_expert": 1, "latency_us": 1.0, "p10_us": 0.9, "p90_us": 1.1, "weight_stream_floor_us": 0.5},
+            {"mode": 1, "tokens_per_expert": 1, "latency_us": 2.0, "p10_us": 1.9, "p90_us": 2.1, "weight_stream_floor_us": None}]}},
+        "rack_projection": [{"G": 8, "experts_per_gpu": 32, "gain_latency_vs_token_median": 0.1,
+                             "gain_latency_vs_token_min": 0.0, "gain_latency_vs_token_max": 0.2,
+                             "gain_latency_vs_contiguous_median": 0.5, "latency_balanced_max_over_mean_median": 1.0}],
+    })
+    report.write_markdown(rep, str(p), "cmd")
+    text = p.read_text()
+    for needle in ("## stages", "## ffn_balanced", "## fused_scatter", "## layer", "## profile", "## rack_projection"):
+        assert needle in text
+    assert os.path.getsize(p) > 500
