@@ -310,6 +310,38 @@ def main():
     h2d = T * E * 4 + T * d * 2
     d2h = T * d * 2 + E * 4
 
+    # ---------------------------------------------------------------- the same layer with the FP8 (e4m3) FFN (S8(f) f2)
+    # extra information, not the headline: BASELINE.json's configs are bf16.  Weights are quantised once, outside
+    # the timed region (they are static in serving); the activations are quantised inside it.
+    fp8 = None
+    if d % 128 == 0 and f % 128 == 0:
+        W1q, s1q = B.fp8_pack_weights(W1)
+        W3q, s3q = B.fp8_pack_weights(W3)
+        W2q, s2q = B.fp8_pack_weights(W2)
+        hs8 = torch.full((E_loc,), 8.0 / 448.0, dtype=torch.float32, device=dev)
+        arena8 = torch.empty((B.workspace_bytes(B.WS_LAYER_FP8, T, k, E, E_loc, d, f),), dtype=torch.uint8, device=dev)
+        cnt8 = torch.empty((E,), dtype=torch.int32, device=dev)
+
+        def step8(i):
+            lg, Xd = sets_d[i % args.sets]
+            B.moe_layer_forward_fp8(rc, lg, Xd, emap, W1q, s1q, W3q, s3q, W2q, s2q, hs8, out=out, counts=cnt8,
+                                    arena=arena8, stream=stream)
+
+        n8 = max(20, args.steps // 2)
+        for i in range(max(3, args.warmup // 4)):
+            step8(i)
+        torch.cuda.synchronize()
+        a8, b8 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a8.record(stream)
+        for i in range(n8):
+            step8(i)
+        b8.record(stream)
+        torch.cuda.synchronize()
+        ms8 = a8.elapsed_time(b8) / n8
+        fp8 = {"layer_tokens_per_s": round(T / ms8 * 1e3), "ms_per_step": round(ms8, 4), "steps": n8,
+               "note": "vibe_moe_layer_forward_fp8 (e4m3 weights/activations, fp32 accumulate), one rank"}
+        del W1q, W3q, W2q, arena8
+
     # ---------------------------------------------------------------- roofline of the dominant kernel
     ffn_s = stage_ms[2] * 1e-3
     flops = 6.0 * R_real * d * f
@@ -397,6 +429,7 @@ def main():
             "cpu_baseline": cpu_baseline,
             "stages": stages,
             "ffn_tflops": round(achieved_tf, 2),
+            "fp8": fp8,
         }
         print(json.dumps(line), flush=True)
     group.close()
