@@ -219,3 +219,26 @@ def test_swap_refine_on_placement_stress_shape(lib):
     assert 2 * len(swaps) <= moved_full or len(swaps) == 0
     want, ws = O.placement_swap_refine(stale, new, G, scale, om, O.MODEL_B, 0.03)
     assert np.array_equal(fixed, want)
+
+
+def test_header_is_plain_c99(tmp_path):
+    """include/vibe.h is the boundary: it must compile as C (no C++-isms, no torch types) and link against the library."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "t.c"
+    src.write_text('#include "vibe.h"\n#include <stdio.h>\n'
+                   'int main(void) { vibe_route_cfg c; (void)c;\n'
+                   '  printf("%d %s %lld\\n", (int)vibe_version(), vibe_status_string(VIBE_ERR_WORKSPACE),\n'
+                   '         (long long)vibe_rows_cap(64, 2, 8, 1)); return 0; }\n')
+    exe = tmp_path / "t"
+    build_mod.build()
+    libdir = os.path.dirname(B.LIB_PATH)
+    r = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                        str(src), "-o", str(exe), "-L", libdir, "-lvibe", "-Wl,-rpath," + libdir],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0 and out.stdout.split() == ["100", "VIBE_ERR_WORKSPACE", "128"], (out.stdout, out.stderr)
