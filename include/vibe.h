@@ -110,7 +110,9 @@ VIBE_API vibe_status vibe_route_topk(const vibe_route_cfg* cfg /*host*/, const f
  * Outputs: Xp [R_cap,d] bf16, offsets [E_loc+1] i32, row_to_assign [R_cap] i32,
  * assign_to_row [A] i32, with R_cap >= vibe_rows_cap(T,k,E_loc,align).
  * counts: optional (may be NULL) -- the histogram produced by vibe_route_topk; advisory.
- * ws: vibe_workspace_bytes(VIBE_WS_PERMUTE, ...) bytes, 16-byte aligned.
+ * ws: vibe_workspace_bytes(VIBE_WS_PERMUTE, ...) bytes, 16-byte aligned; scratch of THIS call (a table of
+ *     per-CTA slot totals and the grid-barrier counters): calls that may run concurrently -- other streams,
+ *     graphs replayed side by side -- must be given different workspaces.
  * ---------------------------------------------------------------------------------- */
 VIBE_API vibe_status vibe_permute(const void* X, const int32_t* topk_ids, const int32_t* counts,
                                   const int32_t* expert_map, int32_t T, int32_t d, int32_t k, int32_t E,

@@ -38,12 +38,11 @@ constexpr int kMaxSlots = 1024;
 constexpr int kIdxThreads = 1024;
 constexpr int kIdxWarps = kIdxThreads / 32;
 constexpr int kBatch = 8;            // id loads in flight per lane
-constexpr int kBarSlots = 64;
 static_assert(kIdxWarps == 32, "the offsets scan keeps one warp partial per lane");
 
-// Grid-barrier state of K1, one slot per in-flight call (round-robin): {arrived, departed}.
-// Zero at module load; the last CTA to depart puts its slot back to zero.
-__device__ unsigned int g_bar[kBarSlots][2];
+// Grid-barrier state of K1: two counters {arrived, departed} at the end of the CALLER's workspace, zeroed by a
+// memset node in front of the launch -- calls that may run concurrently (other streams, replayed graphs) must
+// not share a workspace anyway (the table of CTA totals lives there), so they never share a barrier either.
 
 __device__ __forceinline__ int slot_of(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int i,
                                        int E, int E_loc) {
@@ -78,10 +77,7 @@ __device__ __forceinline__ void grid_barrier_once(unsigned* bar, unsigned G) {
     atomicAdd(&bar[0], 1u);
     while (ld_acquire_u32(&bar[0]) < G) __nanosleep(32);
     __threadfence();
-    if (atomicAdd(&bar[1], 1u) == G - 1) {   // everybody has seen arrived == G
-      bar[0] = 0;
-      bar[1] = 0;
-    }
+    atomicAdd(&bar[1], 1u);                  // (kept for debugging: departed == G when the kernel ends)
   }
   __syncthreads();
 }
@@ -89,7 +85,7 @@ __device__ __forceinline__ void grid_barrier_once(unsigned* bar, unsigned G) {
 // K1 ------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kIdxThreads, 1)
 perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ emap, int A, int E, int E_loc,
-                  int WCH, int align, int d, int bar_slot /* < 0: the grid is ONE cluster */,
+                  int WCH, int align, int d, unsigned int* bar /* NULL: the grid is ONE cluster */,
                   int32_t* __restrict__ tbl /*[G][E_loc]*/,
                   int32_t* __restrict__ offsets /*[E_loc+1]*/, int32_t* __restrict__ row_to_assign,
                   int32_t* __restrict__ assign_to_row, __nv_bfloat16* __restrict__ Xp) {
@@ -146,11 +142,11 @@ perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ e
     }
     tbl[(size_t)cta * E_loc + s] = run;
   }
-  if (bar_slot < 0) {
+  if (bar == nullptr) {
     __threadfence();
     ptx::cluster_sync_all();          // G <= 8: hardware cluster barrier (release / acquire at cluster scope)
   } else {
-    grid_barrier_once(g_bar[bar_slot], (unsigned)G);
+    grid_barrier_once(bar, (unsigned)G);
   }
   // ---- walk the table: rows before mine (base) and all rows (totals).  W slot columns x
   // NG row groups; group g takes rows g, g + NG, ... ----
@@ -320,8 +316,8 @@ __global__ void __launch_bounds__(256) perm_rows_by_row_kernel(const __nv_bfloat
 size_t permute_ws_bytes(int T, int k, int E_loc) {
   (void)T;
   (void)k;
-  // [G][E_loc] table of CTA slot totals, G <= number of SMs
-  return round_up((size_t)num_sms() * E_loc * sizeof(int32_t), 256);
+  // [G][E_loc] table of CTA slot totals, G <= number of SMs, + the grid-barrier counters
+  return round_up((size_t)num_sms() * E_loc * sizeof(int32_t), 256) + 256;
 }
 
 }  // namespace vibe
@@ -395,12 +391,14 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
     lc1.attrs = at;
     lc1.numAttrs = 1;
     VIBE_CUDA(cudaLaunchKernelEx(&lc1, perm_index_kernel, topk_ids, expert_map, (int)A, (int)E, (int)E_loc, WCH,
-                                 (int)align, (int)d, -1, tbl, offsets, row_to_assign, assign_to_row, Xpb));
+                                 (int)align, (int)d, (unsigned int*)nullptr, tbl, offsets, row_to_assign,
+                                 assign_to_row, Xpb));
   } else {
-    static std::atomic<unsigned> next_slot{0};
-    int bar_slot = (int)(next_slot.fetch_add(1, std::memory_order_relaxed) % kBarSlots);
+    unsigned int* bar = reinterpret_cast<unsigned int*>(reinterpret_cast<char*>(ws) +
+                                                        round_up((size_t)num_sms() * E_loc * sizeof(int32_t), 256));
+    VIBE_CUDA(cudaMemsetAsync(bar, 0, 2 * sizeof(unsigned int), st));
     int A_ = A, E_ = E, El_ = E_loc, al_ = align, d_ = d;
-    void* args[] = {(void*)&topk_ids, (void*)&expert_map, &A_, &E_, &El_, &WCH, &al_, &d_, &bar_slot, &tbl, &offsets,
+    void* args[] = {(void*)&topk_ids, (void*)&expert_map, &A_, &E_, &El_, &WCH, &al_, &d_, &bar, &tbl, &offsets,
                     &row_to_assign, &assign_to_row, &Xpb};
     VIBE_CUDA(cudaLaunchCooperativeKernel((const void*)perm_index_kernel, dim3(G), dim3(kIdxThreads), args, smem1,
                                           st));

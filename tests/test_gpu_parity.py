@@ -189,10 +189,10 @@ def test_permute_edge_cases():
     assert off.cpu().tolist() == [0] * 9
 
 
-def test_permute_full_grid_max_slots_and_barrier_slot_reuse():
+def test_permute_full_grid_max_slots_and_back_to_back_calls():
     """The cooperative index kernel at its limits: more assignments than 148 x 1024 threads (several
     batches per warp), the maximum number of slots (1024, 147 KB of shared memory), and 150 calls in a
-    row -- more than twice the 64 round-robin grid-barrier slots -- each checked bit for bit."""
+    row on one workspace (the grid-barrier counters are re-armed by every call) -- checked bit for bit."""
     rng = I._rng(11, 11)
     # A = 400 000 > 148 * 1024: every CTA of the grid works, warps own 96 assignments
     T, k, E = 50000, 8, 64
@@ -205,7 +205,7 @@ def test_permute_full_grid_max_slots_and_barrier_slot_reuse():
     res = rng.permutation(E)[:1024]
     emap[res] = rng.permutation(1024).astype(np.int32)
     check_permute(I.make_X(T, 64, 4), ids, emap, E, 1024, 16)
-    # barrier slots are recycled: 150 back-to-back calls on two alternating inputs
+    # 150 back-to-back calls on two alternating inputs
     Xa, Xb = I.make_X(700, 128, 5), I.make_X(900, 128, 6)
     ia = np.argsort(rng.random((700, 16)), axis=1)[:, :2].astype(np.int32)
     ib = np.argsort(rng.random((900, 16)), axis=1)[:, :3].astype(np.int32)
