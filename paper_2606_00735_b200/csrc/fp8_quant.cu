@@ -13,7 +13,8 @@ __device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u 
 __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
 __device__ __forceinline__ float scale_of(float amax) { return amax > 0.0f ? __fdiv_rn(amax, 448.0f) : 1.0f; }
 
-// one warp per row, 16-byte vectors; the row is read twice (the second read is an L1/L2 hit)
+// one warp per row, 16-byte vectors, 4 independent loads in flight per lane; the row is read twice (the second
+// read is an L1/L2 hit)
 __global__ void __launch_bounds__(256) fp8_quantize_rows_kernel(const __nv_bfloat16* __restrict__ X, int R, int d,
                                                                 uint8_t* __restrict__ Xq, float* __restrict__ row_scale) {
   const int lane = threadIdx.x & 31;
@@ -21,24 +22,34 @@ __global__ void __launch_bounds__(256) fp8_quantize_rows_kernel(const __nv_bfloa
   for (int r = blockIdx.x * 8 + (threadIdx.x >> 5); r < R; r += gridDim.x * 8) {
     const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)r * d);
     float amax = 0.0f;
-    for (int v = lane; v < vpr; v += 32) {
-      const uint4 q = src[v];
-      const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+    for (int v0 = lane; v0 < vpr; v0 += 128) {
+      uint4 q[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) amax = fmaxf(amax, fmaxf(fabsf(bf16_lo(w[i])), fabsf(bf16_hi(w[i]))));
+      for (int j = 0; j < 4; ++j) q[j] = (v0 + 32 * j < vpr) ? src[v0 + 32 * j] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const uint32_t w[4] = {q[j].x, q[j].y, q[j].z, q[j].w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) amax = fmaxf(amax, fmaxf(fabsf(bf16_lo(w[i])), fabsf(bf16_hi(w[i]))));
+      }
     }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
     const float s = scale_of(amax);
     if (lane == 0) row_scale[r] = s;
     uint2* dst = reinterpret_cast<uint2*>(Xq + (size_t)r * d);
-    for (int v = lane; v < vpr; v += 32) {
-      const uint4 q = src[v];
-      const uint32_t w[4] = {q.x, q.y, q.z, q.w};
-      uint32_t p[4];
+    for (int v0 = lane; v0 < vpr; v0 += 128) {
+      uint4 q[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) p[i] = ptx::pack2_e4m3(__fdiv_rn(bf16_lo(w[i]), s), __fdiv_rn(bf16_hi(w[i]), s));
-      dst[v] = make_uint2(p[0] | (p[1] << 16), p[2] | (p[3] << 16));
+      for (int j = 0; j < 4; ++j) q[j] = (v0 + 32 * j < vpr) ? src[v0 + 32 * j] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const uint32_t w[4] = {q[j].x, q[j].y, q[j].z, q[j].w};
+        uint32_t p[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) p[i] = ptx::pack2_e4m3(__fdiv_rn(bf16_lo(w[i]), s), __fdiv_rn(bf16_hi(w[i]), s));
+        if (v0 + 32 * j < vpr) dst[v0 + 32 * j] = make_uint2(p[0] | (p[1] << 16), p[2] | (p[3] << 16));
+      }
     }
   }
 }
@@ -110,7 +121,7 @@ __global__ void __launch_bounds__(256) fp8_gather_row_scales_kernel(const float*
 vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_assign, const int32_t* offsets, int E_loc,
                                   int k, int R_cap, float* row_scale, cudaStream_t st) {
   int blocks = (R_cap + 255) / 256;
-  if (blocks > num_sms() * 8) blocks = num_sms() * 8;
+  if (blocks > num_sms() * 16) blocks = num_sms() * 16;
   if (blocks < 1) blocks = 1;
   fp8_gather_row_scales_kernel<<<blocks, 256, 0, st>>>(tok_scale, row_to_assign, offsets, E_loc, k, R_cap, row_scale);
   VIBE_LAUNCH_CHECK("fp8_gather_row_scales_kernel");
@@ -129,7 +140,7 @@ extern "C" vibe_status vibe_fp8_quantize_rows(const void* X, int32_t R, int32_t 
   VIBE_REQUIRE(aligned16(X) && aligned16(Xq), VIBE_ERR_INVALID_ARG, "vibe_fp8_quantize_rows: X / Xq must be 16-byte aligned");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   int blocks = (R + 7) / 8;
-  if (blocks > num_sms() * 8) blocks = num_sms() * 8;
+  if (blocks > num_sms() * 16) blocks = num_sms() * 16;
   fp8_quantize_rows_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(X), R, d,
                                                    reinterpret_cast<uint8_t*>(Xq), row_scale);
   VIBE_LAUNCH_CHECK("fp8_quantize_rows_kernel");
