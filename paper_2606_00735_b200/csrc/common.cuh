@@ -65,6 +65,8 @@ vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc,
 
 vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_assign, const int32_t* offsets, int E_loc,
                                   int k, int R_cap, float* row_scale, cudaStream_t st);
+vibe_status fp8_quantize_resident_tokens(const void* X, int T, int d, void* Xq, float* tok_scale, const int32_t* ids,
+                                         const int32_t* emap, int k, int E, int E_loc, cudaStream_t st);
 struct LayerArenaFp8 {
   size_t ids, w, offsets, r2a, a2r, Xq, tok_scale, Xpq, row_scale, Hq, Y, perm_ws, total;
   int64_t R_cap;

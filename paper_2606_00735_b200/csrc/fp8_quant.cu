@@ -15,11 +15,27 @@ __device__ __forceinline__ float scale_of(float amax) { return amax > 0.0f ? __f
 
 // one warp per row, 16-byte vectors, 4 independent loads in flight per lane; the row is read twice (the second
 // read is an L1/L2 hit)
+// ids != NULL (expert-parallel shard): row t is skipped unless one of its k experts is resident -- the permutation
+// never reads the rows of the other tokens.
 __global__ void __launch_bounds__(256) fp8_quantize_rows_kernel(const __nv_bfloat16* __restrict__ X, int R, int d,
-                                                                uint8_t* __restrict__ Xq, float* __restrict__ row_scale) {
+                                                                uint8_t* __restrict__ Xq, float* __restrict__ row_scale,
+                                                                const int32_t* __restrict__ ids,
+                                                                const int32_t* __restrict__ emap, int k, int E,
+                                                                int E_loc) {
   const int lane = threadIdx.x & 31;
   const int vpr = d >> 3;
   for (int r = blockIdx.x * 8 + (threadIdx.x >> 5); r < R; r += gridDim.x * 8) {
+    if (ids != nullptr) {
+      bool res = false;
+      for (int j = lane; j < k; j += 32) {
+        const int e = __ldg(ids + (size_t)r * k + j);
+        if (e >= 0 && e < E) {
+          const int sl = emap ? __ldg(emap + e) : e;
+          res |= (sl >= 0 && sl < E_loc);
+        }
+      }
+      if (!__any_sync(0xffffffffu, res)) continue;
+    }
     const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)r * d);
     float amax = 0.0f;
     for (int v0 = lane; v0 < vpr; v0 += 128) {
@@ -128,6 +144,17 @@ vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_
   return VIBE_OK;
 }
 
+vibe_status fp8_quantize_resident_tokens(const void* X, int T, int d, void* Xq, float* tok_scale, const int32_t* ids,
+                                         const int32_t* emap, int k, int E, int E_loc, cudaStream_t st) {
+  if (T == 0) return VIBE_OK;
+  int blocks = (T + 7) / 8;
+  if (blocks > num_sms() * 16) blocks = num_sms() * 16;
+  fp8_quantize_rows_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(X), T, d,
+                                                   reinterpret_cast<uint8_t*>(Xq), tok_scale, ids, emap, k, E, E_loc);
+  VIBE_LAUNCH_CHECK("fp8_quantize_rows_kernel");
+  return VIBE_OK;
+}
+
 }  // namespace vibe
 
 extern "C" vibe_status vibe_fp8_quantize_rows(const void* X, int32_t R, int32_t d, void* Xq, float* row_scale,
@@ -142,7 +169,7 @@ extern "C" vibe_status vibe_fp8_quantize_rows(const void* X, int32_t R, int32_t 
   int blocks = (R + 7) / 8;
   if (blocks > num_sms() * 16) blocks = num_sms() * 16;
   fp8_quantize_rows_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const __nv_bfloat16*>(X), R, d,
-                                                   reinterpret_cast<uint8_t*>(Xq), row_scale);
+                                                   reinterpret_cast<uint8_t*>(Xq), row_scale, nullptr, nullptr, 0, 0, 0);
   VIBE_LAUNCH_CHECK("fp8_quantize_rows_kernel");
   return VIBE_OK;
 }

@@ -107,7 +107,11 @@ extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, con
   if ((s = vibe_route_topk(cfg, logits, T, ids, w, counts, stream)) != VIBE_OK) return s;
   // tokens are quantised BEFORE the permutation (T rows instead of T*k), and the permutation then moves
   // one-byte elements: to vibe_permute an e4m3 row of d bytes is a bf16 row of d/2 elements
-  if ((s = vibe_fp8_quantize_rows(X, T, d, base + a.Xq, tok_scale, stream)) != VIBE_OK) return s;
+  // (on an expert-parallel shard only the tokens with a resident expert are quantised)
+  VIBE_REQUIRE(T == 0 || (X != nullptr && aligned16(X)), VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_fp8: X NULL or misaligned");
+  if ((s = fp8_quantize_resident_tokens(X, T, d, base + a.Xq, tok_scale, (expert_map && E_loc < E) ? ids : nullptr,
+                                        expert_map, k, E, E_loc, reinterpret_cast<cudaStream_t>(stream))) != VIBE_OK)
+    return s;
   if ((s = vibe_permute(base + a.Xq, ids, counts, expert_map, T, d / 2, k, E, E_loc, 1, base + a.Xpq, offsets, r2a, a2r,
                         base + a.perm_ws, permute_ws_bytes(T, k, E_loc), stream)) != VIBE_OK)
     return s;
