@@ -246,13 +246,30 @@ VIBE_API vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg /*host*/, 
 /* Same, end to end from HOST buffers: copies logits_h and X_h (pinned or pageable host
  * memory) to the device, runs the layer, copies out_h and counts_h back, and waits for
  * the stream.  Weights, select_bias and expert_map stay device-resident (model state).
- * arena additionally holds the device copies: vibe_workspace_bytes(VIBE_WS_LAYER_HOST, ...). */
+ * arena additionally holds the device copies: vibe_workspace_bytes(VIBE_WS_LAYER_HOST, ...).
+ * The tokens are cut into chunks (a token's output does not depend on the other tokens of
+ * the batch; the histograms of the chunks are summed on the device): chunk c's copy-in,
+ * layer and copy-out run on three streams (two library-owned copy streams, created on
+ * first use, ordered after the work already on `stream`), so that with PINNED host
+ * buffers the PCIe transfers of both directions overlap the kernels.  The chunk count
+ * is chosen from the shapes by a pipeline estimate. */
 VIBE_API vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg /*host*/,
                                                  const float* logits_h /*host*/, const void* X_h /*host*/,
                                                  const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
                                                  int32_t E_loc, const void* W1, const void* W3, const void* W2,
                                                  void* out_h /*host*/, int32_t* counts_h /*host*/, void* arena,
                                                  size_t arena_bytes, void* stream);
+
+/* vibe_moe_layer_forward_host with the number of token chunks given: n_chunks = 0 lets the
+ * library choose, 1 is the unpipelined path, at most 8.  Chunks hold a multiple of 16
+ * tokens (the last one the remainder); out_h and counts_h do not depend on n_chunks. */
+VIBE_API vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg* cfg /*host*/,
+                                                         const float* logits_h /*host*/, const void* X_h /*host*/,
+                                                         const int32_t* expert_map, int32_t T, int32_t d,
+                                                         int32_t f, int32_t E_loc, const void* W1, const void* W3,
+                                                         const void* W2, void* out_h /*host*/,
+                                                         int32_t* counts_h /*host*/, int32_t n_chunks, void* arena,
+                                                         size_t arena_bytes, void* stream);
 
 /* The whole layer with the FP8 FFN (f2): route -> e4m3 quantisation of the T token rows -> permute (one-byte
  * rows) -> row-scale gather -> vibe_grouped_ffn_fp8 -> combine.  Packed weights / scales as in

@@ -37,7 +37,7 @@ EXPORTED_SYMBOLS = (
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
-    "vibe_profile_expert_latency_fp8",
+    "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward_host_chunked",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -115,6 +115,8 @@ def load() -> C.CDLL:
                                            vp, vp, vp, sz, vp]
     lib.vibe_moe_layer_forward_host.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
                                                 vp, vp, vp, sz, vp]
+    lib.vibe_moe_layer_forward_host_chunked.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp,
+                                                        vp, vp, vp, i32, vp, sz, vp]
     lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                                vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_workspace_bytes.argtypes = [i32] * 8
@@ -148,7 +150,7 @@ def load() -> C.CDLL:
     for name in ("vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_grouped_ffn_scatter",
                  "vibe_combine_scattered", "vibe_moe_layer_forward_fp8", "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8",
                  "vibe_profile_expert_latency", "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
-                 "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
+                 "vibe_moe_layer_forward_host_chunked", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
                  "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine"):
         getattr(lib, name).restype = C.c_int
@@ -463,18 +465,27 @@ def moe_layer_forward_fp8(cfg: RouteConfig, logits, X, expert_map, W1q, s1, W3q,
 
 
 def moe_layer_forward_host(cfg: RouteConfig, logits_h: torch.Tensor, X_h: torch.Tensor, expert_map, W1, W3, W2,
-                           out_h: torch.Tensor, counts_h: torch.Tensor, arena: torch.Tensor, stream=None):
-    """End to end from (pinned) HOST tensors; returns when out_h / counts_h are filled."""
+                           out_h: torch.Tensor, counts_h: torch.Tensor, arena: torch.Tensor, stream=None,
+                           n_chunks: int = 0):
+    """End to end from (pinned) HOST tensors; returns when out_h / counts_h are filled.  n_chunks: token chunks of
+    the copy/compute pipeline (0 = chosen by the library)."""
     lib = load()
     T, d = X_h.shape
     E_loc, _, f = W1.shape
     assert not logits_h.is_cuda and not X_h.is_cuda and not out_h.is_cuda and not counts_h.is_cuda
     c = cfg._c()
-    _ok(lib.vibe_moe_layer_forward_host(C.byref(c), logits_h.data_ptr(), X_h.data_ptr(),
-                                        expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
-                                        W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), out_h.data_ptr(),
-                                        counts_h.data_ptr(), arena.data_ptr(), arena.numel(), _stream(stream)),
-        "vibe_moe_layer_forward_host")
+    emap = expert_map.data_ptr() if expert_map is not None else None
+    if n_chunks == 0:
+        _ok(lib.vibe_moe_layer_forward_host(C.byref(c), logits_h.data_ptr(), X_h.data_ptr(), emap, T, d, f, E_loc,
+                                            W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), out_h.data_ptr(),
+                                            counts_h.data_ptr(), arena.data_ptr(), arena.numel(), _stream(stream)),
+            "vibe_moe_layer_forward_host")
+    else:
+        _ok(lib.vibe_moe_layer_forward_host_chunked(C.byref(c), logits_h.data_ptr(), X_h.data_ptr(), emap, T, d, f,
+                                                    E_loc, W1.data_ptr(), W3.data_ptr(), W2.data_ptr(),
+                                                    out_h.data_ptr(), counts_h.data_ptr(), int(n_chunks),
+                                                    arena.data_ptr(), arena.numel(), _stream(stream)),
+            "vibe_moe_layer_forward_host_chunked")
     return out_h, counts_h
 
 

@@ -113,7 +113,8 @@ extern "C" size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int3
     case VIBE_WS_LAYER_FP8: return layer_arena_fp8(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_HOST:
       return layer_arena(T, k, E_loc, d, f).total + round_up((size_t)T * E * 4, 256) +
-             round_up((size_t)T * d * 2, 256) * 2 + round_up((size_t)E * 4, 256);
+             round_up((size_t)T * d * 2, 256) * 2 + round_up((size_t)E * 4, 256) +
+             round_up((size_t)8 * E * 4, 256);  // + per-chunk histograms of the pipelined entry
     default: return 0;
   }
 }

@@ -1,6 +1,9 @@
 // layer.cu -- the whole per-GPU MoE layer (a1..a5) as one enqueue, from device or host buffers.
 #include "common.cuh"
 
+#include <cmath>
+#include <mutex>
+
 
 extern "C" vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg, const float* logits, const void* X,
                                               const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
@@ -39,16 +42,86 @@ extern "C" vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg, const f
   return vibe_combine(Y, a2r, w, T, k, d, out, stream);
 }
 
-extern "C" vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg, const float* logits_h,
-                                                   const void* X_h, const int32_t* expert_map, int32_t T, int32_t d,
-                                                   int32_t f, int32_t E_loc, const void* W1, const void* W3,
-                                                   const void* W2, void* out_h, int32_t* counts_h, void* arena,
-                                                   size_t arena_bytes, void* stream) {
+namespace {
+
+constexpr int kMaxHostChunks = 8;
+
+// Two copy streams and the events that order them against the caller's stream; created once per device.
+struct HostPipe {
+  cudaStream_t in = nullptr, out = nullptr;
+  cudaEvent_t entry = nullptr, out_done = nullptr;
+  cudaEvent_t in_done[kMaxHostChunks] = {}, comp_done[kMaxHostChunks] = {};
+  bool ready = false;
+};
+
+vibe_status host_pipe(HostPipe** pp) {
+  static std::mutex mu;
+  static HostPipe pipes[64];
+  int dev = 0;
+  VIBE_CUDA(cudaGetDevice(&dev));
+  VIBE_REQUIRE(dev >= 0 && dev < 64, VIBE_ERR_CUDA, "vibe_moe_layer_forward_host: device ordinal %d", dev);
+  std::lock_guard<std::mutex> lock(mu);
+  HostPipe& hp = pipes[dev];
+  if (!hp.ready) {
+    VIBE_CUDA(cudaStreamCreateWithFlags(&hp.in, cudaStreamNonBlocking));
+    VIBE_CUDA(cudaStreamCreateWithFlags(&hp.out, cudaStreamNonBlocking));
+    VIBE_CUDA(cudaEventCreateWithFlags(&hp.entry, cudaEventDisableTiming));
+    VIBE_CUDA(cudaEventCreateWithFlags(&hp.out_done, cudaEventDisableTiming));
+    for (int c = 0; c < kMaxHostChunks; ++c) {
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.in_done[c], cudaEventDisableTiming));
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.comp_done[c], cudaEventDisableTiming));
+    }
+    hp.ready = true;
+  }
+  *pp = &hp;
+  return VIBE_OK;
+}
+
+__global__ void sum_count_parts_kernel(const int32_t* __restrict__ parts, int n_parts, int E, int32_t* __restrict__ counts) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= E) return;
+  int32_t c = 0;
+  for (int p = 0; p < n_parts; ++p) c += parts[(size_t)p * E + e];
+  counts[e] = c;
+}
+
+// Number of token chunks that minimises a three-stage (copy in, compute, copy out) pipeline estimate:
+// makespan = a + b + c + (C - 1) * max(a, b, c) for per-chunk stage times a, b, c.  The compute estimate is the
+// larger of the FFN's flop time (with an efficiency that falls off below ~128 rows per expert tile) and its weight
+// streaming time; the constants are round B200 / PCIe Gen5 figures -- only the ordering of the candidates matters.
+int auto_host_chunks(int T, int k, int E, int E_loc, int d, int f) {
+  const double pcie = 50e9, hbm = 6.0e12, tensor = 1.25e15, launch = 40e-6;
+  const double in_bytes = (double)T * E * 4 + (double)T * d * 2, out_bytes = (double)T * d * 2;
+  int best = 1;
+  double best_t = 0;
+  for (int C = 1; C <= kMaxHostChunks; ++C) {
+    const double Tc = (double)T / C;
+    if (C > 1 && Tc < 256) break;
+    const double n = Tc * k / E;  // mean rows per expert in one chunk
+    const double flops = 6.0 * Tc * k * d * f * ((double)E_loc / E);
+    const double b = fmax(flops / (tensor * n / (n + 128.0)), 6.0 * d * f * E_loc / hbm) + launch;
+    const double a = in_bytes / C / pcie, c = out_bytes / C / pcie;
+    const double t = a + b + c + (C - 1) * fmax(a, fmax(b, c));
+    if (C == 1 || t < best_t) best = C, best_t = t;
+  }
+  return best;
+}
+
+}  // namespace
+
+extern "C" vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg* cfg, const float* logits_h,
+                                                           const void* X_h, const int32_t* expert_map, int32_t T,
+                                                           int32_t d, int32_t f, int32_t E_loc, const void* W1,
+                                                           const void* W3, const void* W2, void* out_h,
+                                                           int32_t* counts_h, int32_t n_chunks, void* arena,
+                                                           size_t arena_bytes, void* stream) {
   using namespace vibe;
   clear_error();
   VIBE_REQUIRE(cfg != nullptr, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host: cfg is NULL");
   VIBE_REQUIRE(T >= 1 && d >= 8 && f >= 8 && E_loc >= 1, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host: bad sizes");
   VIBE_REQUIRE(logits_h && X_h && out_h && counts_h, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host: NULL host buffer");
+  VIBE_REQUIRE(n_chunks >= 0 && n_chunks <= kMaxHostChunks, VIBE_ERR_INVALID_ARG,
+               "vibe_moe_layer_forward_host: n_chunks must be 0 (choose) .. %d", kMaxHostChunks);
   const int E = cfg->num_experts, k = cfg->top_k;
   VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host: need 1 <= k <= E");
   const size_t inner = vibe_workspace_bytes(VIBE_WS_LAYER, T, k, E, E_loc, d, f, 1);
@@ -60,20 +133,72 @@ extern "C" vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg, co
   char* p = reinterpret_cast<char*>(arena) + inner;
   float* logits_d = reinterpret_cast<float*>(p);
   p += round_up((size_t)T * E * 4, 256);
-  void* X_d = p;
+  char* X_d = p;
   p += round_up((size_t)T * d * 2, 256);
-  void* out_d = p;
+  char* out_d = p;
   p += round_up((size_t)T * d * 2, 256);
   int32_t* counts_d = reinterpret_cast<int32_t*>(p);
-  VIBE_CUDA(cudaMemcpyAsync(logits_d, logits_h, (size_t)T * E * 4, cudaMemcpyHostToDevice, st));
-  VIBE_CUDA(cudaMemcpyAsync(X_d, X_h, (size_t)T * d * 2, cudaMemcpyHostToDevice, st));
-  vibe_status s = vibe_moe_layer_forward(cfg, logits_d, X_d, expert_map, T, d, f, E_loc, W1, W3, W2, out_d, counts_d,
-                                         nullptr, nullptr, arena, inner, stream);
+  p += round_up((size_t)E * 4, 256);
+  int32_t* count_parts = reinterpret_cast<int32_t*>(p);
+
+  // chunks of Tc tokens (a multiple of 16, so that every chunk of every buffer starts 64-byte aligned)
+  int C = n_chunks ? n_chunks : auto_host_chunks(T, k, E, E_loc, d, f);
+  int Tc = (int)round_up((size_t)(T + C - 1) / C, 16);
+  C = (T + Tc - 1) / Tc;
+  const char* Xh = reinterpret_cast<const char*>(X_h);
+  char* outh = reinterpret_cast<char*>(out_h);
+  if (C == 1) {
+    VIBE_CUDA(cudaMemcpyAsync(logits_d, logits_h, (size_t)T * E * 4, cudaMemcpyHostToDevice, st));
+    VIBE_CUDA(cudaMemcpyAsync(X_d, X_h, (size_t)T * d * 2, cudaMemcpyHostToDevice, st));
+    vibe_status s = vibe_moe_layer_forward(cfg, logits_d, X_d, expert_map, T, d, f, E_loc, W1, W3, W2, out_d, counts_d,
+                                           nullptr, nullptr, arena, inner, stream);
+    if (s != VIBE_OK) return s;
+    VIBE_CUDA(cudaMemcpyAsync(out_h, out_d, (size_t)T * d * 2, cudaMemcpyDeviceToHost, st));
+    VIBE_CUDA(cudaMemcpyAsync(counts_h, counts_d, (size_t)E * 4, cudaMemcpyDeviceToHost, st));
+    VIBE_CUDA(cudaStreamSynchronize(st));
+    return VIBE_OK;
+  }
+  // Chunk c's copy-in (stream `in`), layer (caller's stream) and copy-out (stream `out`) overlap with the other
+  // chunks' stages; the layer's working buffers are shared by the chunks, which run in order on the caller's stream.
+  HostPipe* hp = nullptr;
+  vibe_status s = host_pipe(&hp);
   if (s != VIBE_OK) return s;
-  VIBE_CUDA(cudaMemcpyAsync(out_h, out_d, (size_t)T * d * 2, cudaMemcpyDeviceToHost, st));
+  VIBE_CUDA(cudaEventRecord(hp->entry, st));
+  VIBE_CUDA(cudaStreamWaitEvent(hp->in, hp->entry, 0));
+  VIBE_CUDA(cudaStreamWaitEvent(hp->out, hp->entry, 0));
+  for (int c = 0; c < C; ++c) {
+    const int t0 = c * Tc, tn = (T - t0 < Tc) ? T - t0 : Tc;
+    VIBE_CUDA(cudaMemcpyAsync(logits_d + (size_t)t0 * E, logits_h + (size_t)t0 * E, (size_t)tn * E * 4,
+                              cudaMemcpyHostToDevice, hp->in));
+    VIBE_CUDA(cudaMemcpyAsync(X_d + (size_t)t0 * d * 2, Xh + (size_t)t0 * d * 2, (size_t)tn * d * 2,
+                              cudaMemcpyHostToDevice, hp->in));
+    VIBE_CUDA(cudaEventRecord(hp->in_done[c], hp->in));
+    VIBE_CUDA(cudaStreamWaitEvent(st, hp->in_done[c], 0));
+    s = vibe_moe_layer_forward(cfg, logits_d + (size_t)t0 * E, X_d + (size_t)t0 * d * 2, expert_map, tn, d, f, E_loc, W1,
+                               W3, W2, out_d + (size_t)t0 * d * 2, count_parts + (size_t)c * E, nullptr, nullptr, arena,
+                               inner, stream);
+    if (s != VIBE_OK) return s;
+    VIBE_CUDA(cudaEventRecord(hp->comp_done[c], st));
+    VIBE_CUDA(cudaStreamWaitEvent(hp->out, hp->comp_done[c], 0));
+    VIBE_CUDA(cudaMemcpyAsync(outh + (size_t)t0 * d * 2, out_d + (size_t)t0 * d * 2, (size_t)tn * d * 2,
+                              cudaMemcpyDeviceToHost, hp->out));
+  }
+  sum_count_parts_kernel<<<(E + 255) / 256, 256, 0, st>>>(count_parts, C, E, counts_d);
+  VIBE_LAUNCH_CHECK("sum_count_parts_kernel");
   VIBE_CUDA(cudaMemcpyAsync(counts_h, counts_d, (size_t)E * 4, cudaMemcpyDeviceToHost, st));
+  VIBE_CUDA(cudaEventRecord(hp->out_done, hp->out));
+  VIBE_CUDA(cudaStreamWaitEvent(st, hp->out_done, 0));
   VIBE_CUDA(cudaStreamSynchronize(st));
   return VIBE_OK;
+}
+
+extern "C" vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg, const float* logits_h,
+                                                   const void* X_h, const int32_t* expert_map, int32_t T, int32_t d,
+                                                   int32_t f, int32_t E_loc, const void* W1, const void* W3,
+                                                   const void* W2, void* out_h, int32_t* counts_h, void* arena,
+                                                   size_t arena_bytes, void* stream) {
+  return vibe_moe_layer_forward_host_chunked(cfg, logits_h, X_h, expert_map, T, d, f, E_loc, W1, W3, W2, out_h,
+                                             counts_h, 0, arena, arena_bytes, stream);
 }
 
 extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, const float* logits, const void* X,

@@ -392,9 +392,14 @@ def test_layer_forward_matches_direct_definition(which):
     X_h = torch.from_numpy(L["X"].view(np.int16)).view(torch.bfloat16).pin_memory()
     out_h = torch.empty((T, d), dtype=torch.bfloat16).pin_memory()
     cnt_h = torch.empty((cfg.E,), dtype=torch.int32).pin_memory()
-    B.moe_layer_forward_host(rc, lg_h, X_h, emap, W1, W3, W2, out_h, cnt_h, arena)
-    assert np.array_equal(cnt_h.numpy(), c)
-    assert np.array_equal(out_h.view(torch.int16).numpy(), out.view(torch.int16).cpu().numpy())
+    # (0: chunk count chosen by the library; 1: unpipelined; 3 and 8: ragged last chunk, copies on the side streams)
+    for n_chunks in (0, 1, 3, 8):
+        out_h.zero_(); cnt_h.zero_()
+        B.moe_layer_forward_host(rc, lg_h, X_h, emap, W1, W3, W2, out_h, cnt_h, arena, n_chunks=n_chunks)
+        assert np.array_equal(cnt_h.numpy(), c), n_chunks
+        assert np.array_equal(out_h.view(torch.int16).numpy(), out.view(torch.int16).cpu().numpy()), n_chunks
+    with pytest.raises(B.VibeError):
+        B.moe_layer_forward_host(rc, lg_h, X_h, emap, W1, W3, W2, out_h, cnt_h, arena, n_chunks=9)
 
 
 @pytest.mark.parametrize("name", ["C2", "C1", "C3"])
