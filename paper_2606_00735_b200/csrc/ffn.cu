@@ -59,6 +59,7 @@ constexpr int ATOM_BYTES = 64 * BK * 2;         // 8 KB : 64 features x 64 K (MN
 constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumulator lanes
 constexpr int B_BYTES = (TN / 2) * BK * 2;      // 16 KB: this CTA's half of the token tile
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
+constexpr int NARROW_ROWS = 32;                 // rows of the small activation box (per CTA)
 constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
 // warps: 0 = TMA producer, 1 = MMA issuer, 2.. = epilogue.  GEMM-1 has 4 epilogue warps (its SwiGLU
 // epilogue needs ~200 registers per thread); the down projection has 8 -- two per TMEM lane quarter,
@@ -165,8 +166,8 @@ __device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv
 // scatter fused into the epilogue (vibe_grouped_ffn_scatter).
 template <int kMode>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 1)
-ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
-                const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
+ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmActN,
+                const __grid_constant__ CUtensorMap tmW0, const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
                 int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out,
                 const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w) {
   constexpr bool kGateUp = (kMode == 0);
@@ -185,6 +186,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   // ------------------------------------------------------------------ setup
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tmAct);
+    ptx::prefetch_tensormap(&tmActN);
     ptx::prefetch_tensormap(&tmW0);
     if (kGateUp) ptx::prefetch_tensormap(&tmW1);
     for (int s = 0; s < STAGES; ++s) {
@@ -267,10 +269,14 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         const int half = ((n_rows + 15) >> 4) << 3;          // UMMA N / 2: this CTA's share of the columns
         const int row_b = row0 + (int)rank * half;
         const int n0 = f_blk * FB + (int)rank * FC;
+        // a tile of at most 2 * NARROW_ROWS tokens loads the small activation box (4 KB instead of 16 KB a stage)
+        const bool narrow = half <= NARROW_ROWS;
+        const CUtensorMap* tm_b = narrow ? &tmActN : &tmAct;
+        const uint32_t tx_bytes = narrow ? 2u * (A_BYTES + NARROW_ROWS * BK * 2) : 2u * STAGE_BYTES;
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
           if (ptx::elect_one()) {
-            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), 2 * STAGE_BYTES);
+            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), tx_bytes);
             const uint32_t full = full0 + (uint32_t)stage * 8u;
             const uint32_t a_s = smem_base + (uint32_t)stage * STAGE_BYTES;
             const uint32_t b_s = a_s + A_BYTES;
@@ -282,7 +288,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
               ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);
               ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, n0 + 64, k0, e, pol_w);
             }
-            ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
+            ptx::tma_load_2d_2sm(b_s, tm_b, full, k0, row_b, pol_act);
           }
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -521,10 +527,12 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y,
                              cudaStream_t st, const int32_t* row_to_assign, const float* topk_w) {
-  CUtensorMap tmX, tmH, tmW1, tmW3, tmW2;
+  CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
   vibe_status s;
   if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
   if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W1, f, d, E_loc, 64, BK, &tmW1)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W3, f, d, E_loc, 64, BK, &tmW3)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W2, d, f, E_loc, 64, BK, &tmW2)) != VIBE_OK) return s;
@@ -540,15 +548,15 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d,
+  ffn_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmXN, tmW1, tmW3, offsets, E_loc, f, d,
                                                             reinterpret_cast<__nv_bfloat16*>(H_ws), f, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
   if (row_to_assign != nullptr)
-    ffn_gemm_kernel<2><<<grid, num_threads(2), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+    ffn_gemm_kernel<2><<<grid, num_threads(2), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f,
                                                               reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign,
                                                               topk_w);
   else
-    ffn_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f,
+    ffn_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f,
                                                               reinterpret_cast<__nv_bfloat16*>(Y), d, nullptr, nullptr);
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
