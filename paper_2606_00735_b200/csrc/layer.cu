@@ -52,6 +52,7 @@ struct HostPipe {
   cudaEvent_t entry = nullptr, out_done = nullptr;
   cudaEvent_t in_done[kMaxHostChunks] = {}, comp_done[kMaxHostChunks] = {};
   bool ready = false;
+  std::mutex in_use;   // one pipelined call per device at a time (the events are per device, and the call waits anyway)
 };
 
 vibe_status host_pipe(HostPipe** pp) {
@@ -163,6 +164,7 @@ extern "C" vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg*
   HostPipe* hp = nullptr;
   vibe_status s = host_pipe(&hp);
   if (s != VIBE_OK) return s;
+  std::lock_guard<std::mutex> one_call(hp->in_use);
   VIBE_CUDA(cudaEventRecord(hp->entry, st));
   VIBE_CUDA(cudaStreamWaitEvent(hp->in, hp->entry, 0));
   VIBE_CUDA(cudaStreamWaitEvent(hp->out, hp->entry, 0));
