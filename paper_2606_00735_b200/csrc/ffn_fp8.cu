@@ -29,6 +29,7 @@ constexpr int ATOM_BYTES = 64 * BK;             // 8 KB : 64 features x 128 K (K
 constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumulator lanes
 constexpr int B_BYTES = (TN / 2) * BK;          // 16 KB: this CTA's half of the token tile
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
+constexpr int NARROW_ROWS = 32;                 // rows of the small activation box (per CTA)
 constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
 constexpr int SX_BYTES = 4 * TN * 4;            // GEMM-1: the tile's row scales, one 1 KB slice per epilogue warp
 // warps: 0 = TMA producer, 1 = MMA issuer, 2.. = epilogue.  GEMM-1 has 4 epilogue warps (its SwiGLU
@@ -133,8 +134,8 @@ __device__ __forceinline__ void store_block_T_e4m3(const float (&v)[32], uint8_t
 // kMode: 0 = gate|up + SwiGLU (GEMM-1, writes Hq e4m3), 1 = down (GEMM-2, writes Y bf16).
 template <int kMode>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 1)
-ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmW0,
-                 const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
+ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmActN,
+                 const __grid_constant__ CUtensorMap tmW0, const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
                  int n_total, int k_total, void* __restrict__ out_v, int ld_out,
                  const float* __restrict__ row_scale /*GEMM-1: sx [R_cap]*/, const float* __restrict__ sw0 /*[E_loc]*/,
                  const float* __restrict__ sw1 /*[E_loc] (GEMM-1: W3)*/, const float* __restrict__ h_scale /*[E_loc]*/) {
@@ -155,6 +156,7 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
   // ------------------------------------------------------------------ setup
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tmAct);
+    ptx::prefetch_tensormap(&tmActN);
     ptx::prefetch_tensormap(&tmW0);
     if (kGateUp) ptx::prefetch_tensormap(&tmW1);
     for (int s = 0; s < STAGES; ++s) {
@@ -237,10 +239,14 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
         const int half = ((n_rows + 15) >> 4) << 3;          // UMMA N / 2: this CTA's share of the columns
         const int row_b = row0 + (int)rank * half;
         const int n0 = f_blk * FB + (int)rank * FC;
+        // a tile of at most 2 * NARROW_ROWS tokens loads the small activation box (4 KB instead of 16 KB a stage)
+        const bool narrow = half <= NARROW_ROWS;
+        const CUtensorMap* tm_b = narrow ? &tmActN : &tmAct;
+        const uint32_t tx_bytes = narrow ? 2u * (A_BYTES + NARROW_ROWS * BK) : 2u * STAGE_BYTES;
         for (int kb = 0; kb < KB; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
           if (ptx::elect_one()) {
-            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), 2 * STAGE_BYTES);
+            if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), tx_bytes);
             const uint32_t full = full0 + (uint32_t)stage * 8u;
             const uint32_t a_s = smem_base + (uint32_t)stage * STAGE_BYTES;
             const uint32_t b_s = a_s + A_BYTES;
@@ -252,7 +258,7 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
               ptx::tma_load_3d_2sm(a_s, &tmW0, full, k0, n0, e, pol_w);
               ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, k0, n0 + 64, e, pol_w);
             }
-            ptx::tma_load_2d_2sm(b_s, &tmAct, full, k0, row_b, pol_act);
+            ptx::tma_load_2d_2sm(b_s, tm_b, full, k0, row_b, pol_act);
           }
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -493,11 +499,13 @@ vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const i
                                  int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
                                  const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
                                  cudaStream_t st) {
-  CUtensorMap tmX, tmH, tmW1, tmW3, tmW2;
+  CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
   vibe_status s;
-  // activations [R_cap, K] and packed weights [E_loc, N, K]: K innermost, boxes of 128 K x (128 | 64) rows
+  // activations [R_cap, K] and packed weights [E_loc, N, K]: K innermost, boxes of 128 K x (128 | 32 | 64) rows
   if ((s = get_tensor_map(Xq, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
   if ((s = get_tensor_map(Hq, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(Xq, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(Hq, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W1q, d, f, E_loc, BK, 64, &tmW1)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W3q, d, f, E_loc, BK, 64, &tmW3)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W2q, f, d, E_loc, BK, 64, &tmW2)) != VIBE_OK) return s;
@@ -511,10 +519,10 @@ vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const i
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn8_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmW1, tmW3, offsets, E_loc, f, d, Hq, f, row_scale,
+  ffn8_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmXN, tmW1, tmW3, offsets, E_loc, f, d, Hq, f, row_scale,
                                                                 s1, s3, h_scale);
   VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<gate_up>");
-  ffn8_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmW2, tmW2, offsets, E_loc, d, f, Y, d, nullptr, s2,
+  ffn8_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f, Y, d, nullptr, s2,
                                                                 nullptr, h_scale);
   VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<down>");
   return VIBE_OK;
