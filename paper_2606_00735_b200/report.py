@@ -1,6 +1,6 @@
 """Per-kernel measurements on one B200 beyond the single bench.py line.
 
-    python -m paper_2606_00735_b200.report [--sections stages,ffn,fp8,fused,layer,profile,placement,variability,rack,recalibration]
+    python -m paper_2606_00735_b200.report [--sections stages,ffn,mixed,fp8,fused,layer,profile,placement,variability,rack,recalibration]
                                            [--out gpurun_out/report.json] [--quick]
 
 Sections (all through the C-ABI binding; seeded synthetic inputs):
@@ -344,6 +344,38 @@ def section_ffn(peaks, quick):
     return out
 
 
+def section_mixed(peaks, quick):
+    """Grouped FFN on skewed row distributions (S8(f) f4): a lone light expert, a few light
+    experts, every expert light, and heavy experts mixed with light ones.  The first case runs first with a fixed
+    number of launches, so that an ncu capture of the first ffn_gemm_kernel launches is the lone expert."""
+    out = []
+    cases = [("C3", I.C3, "1 x 32", [32] + [0] * 31), ("C3", I.C3, "4 x 32", [32] * 4 + [0] * 28),
+             ("C3", I.C3, "32 x 32", [32] * 32), ("C3", I.C3, "4 x 2048", [2048] * 4 + [0] * 28),
+             ("C3", I.C3, "4 x 2048 + 28 x 32", [2048] * 4 + [32] * 28),
+             ("C3", I.C3, "8 x 1024 + 24 x 64", [1024] * 8 + [64] * 24),
+             ("C2", I.C2, "128 x 16", [16] * 128), ("C2", I.C2, "24 x 1024", [1024] * 24 + [0] * 104),
+             ("C2", I.C2, "24 x 1024 + 104 x 64", [1024] * 24 + [64] * 104)]
+    held = {}
+    for shape, cfg, label, rows in cases:
+        E, d, f = cfg.E_loc, cfg.d, cfg.f
+        if shape not in held:
+            held.clear()
+            torch.cuda.empty_cache()
+            held[shape] = _weights(E, d, f)
+        W1, W3, W2 = held[shape]
+        R = int(sum(rows))
+        Xp = torch.randn((R, d), device="cuda").to(torch.bfloat16)
+        H = torch.empty((R, f), dtype=torch.bfloat16, device="cuda")
+        Y = torch.empty((R, d), dtype=torch.bfloat16, device="cuda")
+        off = torch.tensor(np.concatenate([[0], np.cumsum(rows)]), dtype=torch.int32, device="cuda")
+        us = _time(lambda i: B.grouped_ffn(Xp, off, W1, W3, W2, H, Y), 20 if quick else 100, warmup=3)
+        active = sum(1 for r in rows if r > 0)
+        out.append({"shape": shape, "rows_per_expert": label, "rows": R, "active_experts": active, "us": round(us, 1),
+                    "weight_TB/s": round(active * 6.0 * d * f / us / 1e6, 2),
+                    "TFLOP/s": round(6.0 * R * d * f / us / 1e6, 1)})
+    return out
+
+
 def section_profile(peaks, quick):
     out = {}
     for cfg in (I.C2, I.C3):
@@ -559,6 +591,13 @@ def write_markdown(r, path, command):
         o.append("|---|---|---|---|---|---|---|---|---|---|")
         for x in r['ffn_balanced']:
             o.append(f"| {x['shape']} | {x['E_loc']} | {x['d']} | {x['f']} | {x['tokens_per_expert']} | {x['us_per_expert']} | {x['TFLOP/s']} | {x['frac_sustained']} | {x['frac_burst']} | {x['frac_of_per_expert_roofline']} |")
+    if "ffn_mixed" in r:
+        o.append("\n## ffn_mixed: grouped FFN on skewed row distributions (CUDA graph; weight TB/s = weights of the active experts / time)\n")
+        o.append("| shape | rows per expert | rows | active experts | us | weight TB/s | TFLOP/s |")
+        o.append("|---|---|---|---|---|---|---|")
+        for x in r["ffn_mixed"]:
+            o.append(f"| {x['shape']} | {x['rows_per_expert']} | {x['rows']} | {x['active_experts']} | {x['us']} | {x['weight_TB/s']} | {x['TFLOP/s']} |")
+        o.append("\nA light expert occupies its CTA pairs for (weight bytes of the tile) / ~140 GB/s whatever else runs (DESIGN.md section 12): heavy and light experts add.\n")
     if "fused_scatter" in r:
         o.append("\n## fused_scatter: vibe_grouped_ffn + vibe_combine vs vibe_grouped_ffn_scatter + vibe_combine_scattered (routed batches)\n")
         o.append("| config | ffn + combine us | fused scatter us | speedup |\n|---|---|---|---|")
@@ -629,7 +668,7 @@ def write_markdown(r, path, command):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--sections", default="stages,ffn,fp8,fused,layer,profile,placement,variability,rack,recalibration")
+    ap.add_argument("--sections", default="stages,ffn,mixed,fp8,fused,layer,profile,placement,variability,rack,recalibration")
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "report.json"))
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--md", default="", help="also write the report as markdown tables (needs all sections)")
@@ -651,6 +690,10 @@ def main():
         rep["ffn_balanced"] = section_ffn(peaks, args.quick)
         for r in rep["ffn_balanced"]:
             print(r["shape"], r["tokens_per_expert"], r["us_per_expert"], r["TFLOP/s"], r["frac_sustained"], flush=True)
+    if "mixed" in want:
+        rep["ffn_mixed"] = section_mixed(peaks, args.quick)
+        for r in rep["ffn_mixed"]:
+            print(r, flush=True)
     if "fused" in want:
         rep["fused_scatter"] = section_fused(peaks, args.quick)
         for r in rep["fused_scatter"]:

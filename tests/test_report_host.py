@@ -16,6 +16,8 @@ def test_write_markdown_with_partial_and_full_sections(tmp_path):
                     "permute": stage, "combine": stage}],
         "ffn_balanced": [{"shape": "C1", "E_loc": 8, "d": 64, "f": 64, "tokens_per_expert": 512, "us_per_expert": 1.0,
                           "TFLOP/s": 1.0, "frac_sustained": 0.1, "frac_burst": 0.1, "frac_of_per_expert_roofline": 0.1}],
+        "ffn_mixed": [{"shape": "C3", "rows_per_expert": "1 x 32", "rows": 32, "active_experts": 1, "us": 39.0,
+                       "weight_TB/s": 2.26, "TFLOP/s": 72.3}],
         "fused_scatter": [{"config": "C1", "ffn_plus_combine_us": 1.0, "fused_scatter_us": 1.0, "speedup": 1.0}],
         "layer": [{"config": "C1", "eager_us": 1.0, "graph_us": 1.0, "tokens_per_s_eager": 1, "tokens_per_s_graph": 1}],
         "profile": {"C2": {"E_loc": 2, "d": 64, "f": 64, "rows": [
@@ -27,6 +29,6 @@ def test_write_markdown_with_partial_and_full_sections(tmp_path):
     })
     report.write_markdown(rep, str(p), "cmd")
     text = p.read_text()
-    for needle in ("## stages", "## ffn_balanced", "## fused_scatter", "## layer", "## profile", "## rack_projection"):
+    for needle in ("## stages", "## ffn_balanced", "## ffn_mixed", "## fused_scatter", "## layer", "## profile", "## rack_projection"):
         assert needle in text
     assert os.path.getsize(p) > 500
