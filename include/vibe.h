@@ -205,10 +205,13 @@ VIBE_API vibe_status vibe_grouped_ffn_fp8(const void* Xq, const float* row_scale
  *   mode 0 (uniform): every one of the E_loc experts receives n = tokens_per_expert[p]
  *           rows; latency_us[p] = median kernel time / E_loc   (per-expert cost l(n))
  *   mode 1 (solo):    expert 0 receives n rows, the others none; latency_us[p] = median time
- * Times are CUDA-event times of `iters` back-to-back calls (each call timed separately)
- * after `warmup` untimed calls per point.  Activations are an arbitrary finite pattern
- * written by the library into ws (latency does not depend on values).
- * This call SYNCHRONISES the stream.  tokens_per_expert, latency_us, samples_us: HOST.
+ * Times are CUDA-event times of `iters` back-to-back executions (each timed separately)
+ * after max(warmup, 1) untimed calls per point.  The timed executions replay one call
+ * captured into a CUDA graph, on a stream of the sweep's own, so that an event pair
+ * brackets the kernels and not the host's work between launches (a lone small expert
+ * takes less device time than the host needs to launch it).  Activations are an arbitrary
+ * finite pattern written by the library into ws (latency does not depend on values).
+ * This call SYNCHRONISES the stream (before the sweep) and returns when the sweep is done.  tokens_per_expert, latency_us, samples_us: HOST.
  * samples_us: optional host [n_points*iters] per-iteration times (NULL to skip).
  * ws: vibe_workspace_bytes(VIBE_WS_PROFILE, T = max tokens_per_expert, ...) bytes.
  * ---------------------------------------------------------------------------------- */

@@ -27,15 +27,25 @@ __global__ void fill_ones_kernel(float* p, size_t n) {
 
 namespace vibe {
 namespace {
-// the sweep itself: per point upload the offsets, `warmup` untimed + `iters` timed calls of run(), median
+// The sweep itself.  Per point: upload the offsets, max(warmup, 1) untimed calls of run(), then `iters` timed
+// executions, median.  The timed executions replay ONE call captured into a CUDA graph, so that an event pair
+// brackets the kernels of the call and not the host's work between two launches (tensor-map look-ups, two
+// launches with 640 bytes of parameters: ~6 us, more than a lone small expert takes on the device).  Everything
+// runs on a stream of the sweep's own, after the caller's stream has drained: the legacy default stream cannot be
+// captured.  If the capture fails the calls are timed one by one as launched.
 template <class Run>
 vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_points, int mode, int warmup, int iters,
-                          float* latency_us, float* samples_us, int32_t* offsets, cudaStream_t st, Run run) {
-  std::vector<cudaEvent_t> ev(2 * (size_t)iters);
-  for (auto& e : ev) VIBE_CUDA(cudaEventCreate(&e));
+                          float* latency_us, float* samples_us, int32_t* offsets, cudaStream_t caller, Run run) {
+  VIBE_CUDA(cudaStreamSynchronize(caller));
+  cudaStream_t st = nullptr;
+  VIBE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  std::vector<cudaEvent_t> ev(2 * (size_t)iters, nullptr);
+  vibe_status rc = VIBE_OK;
+  for (auto& e : ev)
+    if (cudaEventCreate(&e) != cudaSuccess) rc = VIBE_ERR_CUDA;
+  if (rc != VIBE_OK) set_error("vibe_profile_expert_latency: cudaEventCreate failed");
   std::vector<int32_t> off(E_loc + 1);
   std::vector<float> t(iters);
-  vibe_status rc = VIBE_OK;
   for (int p = 0; p < n_points && rc == VIBE_OK; ++p) {
     const int n = tokens_per_expert[p];
     off[0] = 0;
@@ -47,15 +57,35 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
       rc = VIBE_ERR_CUDA;
       break;
     }
-    for (int i = 0; i < warmup && rc == VIBE_OK; ++i)
-      rc = run();
+    for (int i = 0; i < std::max(warmup, 1) && rc == VIBE_OK; ++i) rc = run(st);
+    if (rc != VIBE_OK) break;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      const vibe_status cs = run(st);
+      if (cudaStreamEndCapture(st, &graph) != cudaSuccess || cs != VIBE_OK) {
+        if (graph) cudaGraphDestroy(graph);
+        graph = nullptr;
+      }
+      if (graph && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+    }
+    (void)cudaGetLastError();      // a failed capture leaves a sticky-free error behind; the fallback below still works
     for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
       cudaEventRecord(ev[2 * i], st);
-      rc = run();
+      if (exec) {
+        if (cudaGraphLaunch(exec, st) != cudaSuccess) {
+          set_error("vibe_profile_expert_latency: cudaGraphLaunch failed");
+          rc = VIBE_ERR_CUDA;
+        }
+      } else {
+        rc = run(st);
+      }
       cudaEventRecord(ev[2 * i + 1], st);
     }
-    if (rc != VIBE_OK) break;
     ce = cudaStreamSynchronize(st);
+    if (exec) cudaGraphExecDestroy(exec);
+    if (graph) cudaGraphDestroy(graph);
+    if (rc != VIBE_OK) break;
     if (ce != cudaSuccess) {
       set_error("vibe_profile_expert_latency: kernel failed: %s", cudaGetErrorString(ce));
       rc = VIBE_ERR_CUDA;
@@ -71,7 +101,9 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
     const float med = (iters & 1) ? t[iters / 2] : 0.5f * (t[iters / 2 - 1] + t[iters / 2]);
     latency_us[p] = (mode == 0) ? med / (float)E_loc : med;
   }
-  for (auto& e : ev) cudaEventDestroy(e);
+  for (auto& e : ev)
+    if (e) cudaEventDestroy(e);
+  cudaStreamDestroy(st);
   return rc;
 }
 }  // namespace
@@ -113,7 +145,7 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
   VIBE_LAUNCH_CHECK("fill_pattern_kernel");
 
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st,
-                       [&]() { return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, st); });
+                       [&](cudaStream_t ps) { return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, ps); });
 }
 
 extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
@@ -158,7 +190,7 @@ extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d,
   VIBE_CUDA(cudaMemsetAsync(Xq, 0x38, (size_t)R_cap * d, st));
   fill_ones_kernel<<<num_sms() * 2, 256, 0, st>>>(row_scale, (size_t)R_cap);
   VIBE_LAUNCH_CHECK("fill_ones_kernel");
-  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st, [&]() {
-    return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, st);
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st, [&](cudaStream_t ps) {
+    return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, ps);
   });
 }
