@@ -400,6 +400,12 @@ def test_layer_forward_matches_direct_definition(which):
         assert np.array_equal(out_h.view(torch.int16).numpy(), out.view(torch.int16).cpu().numpy()), n_chunks
     with pytest.raises(B.VibeError):
         B.moe_layer_forward_host(rc, lg_h, X_h, emap, W1, W3, W2, out_h, cnt_h, arena, n_chunks=9)
+    # pageable host memory is accepted too (the copies then do not overlap, the result is the same)
+    lg_p, X_p = torch.from_numpy(L["logits"].copy()), torch.from_numpy(L["X"].view(np.int16).copy()).view(torch.bfloat16)
+    out_p, cnt_p = torch.zeros((T, d), dtype=torch.bfloat16), torch.zeros((cfg.E,), dtype=torch.int32)
+    B.moe_layer_forward_host(rc, lg_p, X_p, emap, W1, W3, W2, out_p, cnt_p, arena, n_chunks=3)
+    assert np.array_equal(cnt_p.numpy(), c)
+    assert np.array_equal(out_p.view(torch.int16).numpy(), out.view(torch.int16).cpu().numpy())
 
 
 @pytest.mark.parametrize("name", ["C2", "C1", "C3"])
