@@ -274,8 +274,8 @@ VIBE_API vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg* c
                                                          int32_t* counts_h /*host*/, int32_t n_chunks, void* arena,
                                                          size_t arena_bytes, void* stream);
 
-/* The whole layer with the FP8 FFN (f2): route -> e4m3 quantisation of the T token rows -> permute (one-byte
- * rows) -> row-scale gather -> vibe_grouped_ffn_fp8 -> combine.  Packed weights / scales as in
+/* The whole layer with the FP8 FFN (f2): route -> e4m3 quantisation of the token rows (on an expert-parallel
+ * shard only of the tokens that have a resident expert) -> permute (one-byte rows) -> row-scale gather -> vibe_grouped_ffn_fp8 -> combine.  Packed weights / scales as in
  * vibe_grouped_ffn_fp8; arena: vibe_workspace_bytes(VIBE_WS_LAYER_FP8, ...) bytes, 256-byte aligned.
  * out [T,d] bf16, counts [E] i32 (device).  d % 128 == 0, f % 128 == 0. */
 VIBE_API vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg /*host*/, const float* logits,
