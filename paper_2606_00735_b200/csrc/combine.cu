@@ -3,6 +3,7 @@
 // Token-major, one thread per 16-byte output vector(s), up to 4*VPT row loads in flight per
 // thread.  HBM-bound: reads 2*R*d, writes 2*T*d bytes.  include/vibe.h, C1.
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace vibe {
 namespace {
@@ -37,6 +38,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const __nv_bfloat16* __res
                                                       __nv_bfloat16* __restrict__ out) {
   const int vpr = d >> 3;            // 16-byte vectors per row
   const int per_row = vpr / VPT;     // threads per row
+  ptx::griddep_wait();               // launched as a programmatic dependent of the kernel that writes Y
   const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
   if (g >= (long long)T * per_row) return;
   const int t = (int)(g / per_row);
@@ -128,9 +130,10 @@ vibe_status combine_impl(const char* who, const void* Y, const int32_t* assign_t
   const long long blocks = (threads + 255) / 256;
   VIBE_REQUIRE(blocks < (1ll << 31), VIBE_ERR_UNSUPPORTED, "%s: T*d too large for one launch", who);
   const unsigned gb = (unsigned)blocks;
+  cudaError_t launch_err = cudaSuccess;
 #define VIBE_COMBINE_CASE(V, K, S)                                                              \
   if (vpt == V && k4 == K && scat == S)                                                         \
-    combine_kernel<V, K, S><<<gb, 256, 0, st>>>(Yb, assign_to_row, topk_w, T, k, d, ob);
+    launch_err = launch_pdl(combine_kernel<V, K, S>, dim3(gb), dim3(256), 0, st, Yb, assign_to_row, topk_w, T, k, d, ob);
   VIBE_COMBINE_CASE(2, true, false)
   VIBE_COMBINE_CASE(2, false, false)
   VIBE_COMBINE_CASE(1, true, false)
@@ -140,6 +143,7 @@ vibe_status combine_impl(const char* who, const void* Y, const int32_t* assign_t
   VIBE_COMBINE_CASE(1, true, true)
   VIBE_COMBINE_CASE(1, false, true)
 #undef VIBE_COMBINE_CASE
+  VIBE_REQUIRE(launch_err == cudaSuccess, VIBE_ERR_CUDA, "combine_kernel launch failed: %s", cudaGetErrorString(launch_err));
   VIBE_LAUNCH_CHECK("combine_kernel");
   return VIBE_OK;
 }

@@ -67,6 +67,23 @@ vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_
                                   int k, int R_cap, float* row_scale, cudaStream_t st);
 vibe_status fp8_quantize_resident_tokens(const void* X, int T, int d, void* Xq, float* tok_scale, const int32_t* ids,
                                          const int32_t* emap, int k, int E, int E_loc, cudaStream_t st);
+// Launch with the programmatic-stream-serialization attribute (the kernel calls ptx::griddep_wait before it reads
+// what the preceding kernel of the stream wrote).
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = grid;
+  lc.blockDim = block;
+  lc.dynamicSmemBytes = smem;
+  lc.stream = st;
+  lc.attrs = attr;
+  lc.numAttrs = 1;
+  return cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
+}
+
 struct LayerArenaFp8 {
   size_t ids, w, offsets, r2a, a2r, Xq, tok_scale, Xpq, row_scale, Hq, Y, perm_ws, total;
   int64_t R_cap;

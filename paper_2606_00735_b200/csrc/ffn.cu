@@ -184,6 +184,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   const int KB = k_total / BK;
 
   // ------------------------------------------------------------------ setup
+  // (programmatic dependent launch: this grid's set-up below overlaps the tail of the preceding kernel; nothing
+  // that kernel wrote -- offsets, Xp or H -- is read before griddep_wait)
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tmAct);
     ptx::prefetch_tensormap(&tmActN);
@@ -203,6 +205,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     ptx::tmem_relinquish_2sm();
   } else if (warp == 2) {
     // segment starts + exclusive scan of token tiles per slot (warp-shuffle scan, 32 slots a step)
+    ptx::griddep_wait();
     int carry = 0;
     for (int base = 0; base < E_loc; base += 32) {
       const int e = base + lane;
@@ -234,6 +237,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       tail->total_t_tiles = carry;
     }
   }
+  if (warp != 2) ptx::griddep_wait();
   ptx::tc_fence_before();
   __syncthreads();
   ptx::cluster_sync_all();      // the peer's barriers are initialised before anything signals them
@@ -437,6 +441,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   // ------------------------------------------------------------------ teardown
   ptx::tc_fence_before();
   __syncthreads();
+  ptx::griddep_launch();        // all tiles of this CTA are done: the next kernel's CTAs may become resident
   ptx::cluster_sync_all();      // neither CTA frees TMEM / exits while the peer still uses the pair
   if (warp == 1) {
     ptx::tc_fence_after();
@@ -548,16 +553,20 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmXN, tmW1, tmW3, offsets, E_loc, f, d,
-                                                            reinterpret_cast<__nv_bfloat16*>(H_ws), f, nullptr, nullptr);
+  // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
+  const int32_t* no_map = nullptr;
+  const float* no_w = nullptr;
+  cudaError_t le = launch_pdl(ffn_gemm_kernel<0>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
+                              offsets, E_loc, f, d, reinterpret_cast<__nv_bfloat16*>(H_ws), f, no_map, no_w);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
   if (row_to_assign != nullptr)
-    ffn_gemm_kernel<2><<<grid, num_threads(2), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f,
-                                                              reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign,
-                                                              topk_w);
+    le = launch_pdl(ffn_gemm_kernel<2>, dim3(grid), dim3(num_threads(2)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
+                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign, topk_w);
   else
-    ffn_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f,
-                                                              reinterpret_cast<__nv_bfloat16*>(Y), d, nullptr, nullptr);
+    le = launch_pdl(ffn_gemm_kernel<1>, dim3(grid), dim3(num_threads(1)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
+                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, no_map, no_w);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
 }

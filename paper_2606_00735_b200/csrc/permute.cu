@@ -257,6 +257,7 @@ __global__ void __launch_bounds__(256) perm_rows_kernel(const __nv_bfloat16* __r
                                                         int d, __nv_bfloat16* __restrict__ Xp) {
   const int vpr = d >> 3;
   const int per_row = vpr / VPT;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the FFN's CTAs may become resident
   asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
   const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
   if (g >= (long long)T * per_row) return;
@@ -289,6 +290,7 @@ __global__ void __launch_bounds__(256) perm_rows_by_row_kernel(const __nv_bfloat
                                                                const int32_t* __restrict__ row_to_assign,
                                                                const int32_t* __restrict__ offsets, int E_loc,
                                                                int k, int d, __nv_bfloat16* __restrict__ Xp) {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the FFN's CTAs may become resident
   asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
   const int R = __ldg(offsets + E_loc);
   const int lane = threadIdx.x & 31;

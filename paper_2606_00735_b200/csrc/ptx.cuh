@@ -139,6 +139,13 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // descriptors, addresses and barriers in UNIFORM registers.  Wrapping a whole loop in
 // `if (lane == 0)` instead makes every operand "possibly divergent" and costs an ELECT /
 // R2UR.BROADCAST x7 / BRA.U.ANY sequence per tcgen05.mma or TMA instruction.
+// Programmatic dependent launch: a grid launched with the programmatic-stream-serialization attribute may become
+// resident once every CTA of the preceding grid has executed launch_dependents (or exited); it must execute
+// griddep_wait before it touches anything the preceding grid wrote (the wait returns when that grid has completed
+// and its writes are visible).  Both are no-ops for a grid launched the ordinary way.
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile(
