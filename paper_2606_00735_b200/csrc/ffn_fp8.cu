@@ -173,6 +173,7 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
     ptx::tmem_relinquish_2sm();
   } else if (warp == 2) {
     // segment starts + exclusive scan of token tiles per slot (warp-shuffle scan, 32 slots a step)
+    ptx::griddep_wait();          // programmatic dependent launch, as in ffn.cu: set-up overlaps the preceding kernel's tail
     int carry = 0;
     for (int base = 0; base < E_loc; base += 32) {
       const int e = base + lane;
@@ -204,6 +205,7 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
       tail->total_t_tiles = carry;
     }
   }
+  if (warp != 2) ptx::griddep_wait();
   ptx::tc_fence_before();
   __syncthreads();
   ptx::cluster_sync_all();      // the peer's barriers are initialised before anything signals them
@@ -408,6 +410,7 @@ ffn8_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constan
   // ------------------------------------------------------------------ teardown
   ptx::tc_fence_before();
   __syncthreads();
+  ptx::griddep_launch();        // all tiles of this CTA are done: the next kernel's CTAs may become resident
   ptx::cluster_sync_all();      // neither CTA frees TMEM / exits while the peer still uses the pair
   if (warp == 1) {
     ptx::tc_fence_after();
@@ -519,11 +522,14 @@ vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const i
   VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
                SMEM_BYTES, cudaGetErrorString(attr_err));
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  ffn8_gemm_kernel<0><<<grid, num_threads(0), SMEM_BYTES, st>>>(tmX, tmXN, tmW1, tmW3, offsets, E_loc, f, d, Hq, f, row_scale,
-                                                                s1, s3, h_scale);
+  const float* none = nullptr;
+  cudaError_t le = launch_pdl(ffn8_gemm_kernel<0>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
+                              offsets, E_loc, f, d, Hq, f, row_scale, s1, s3, h_scale);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn8_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<gate_up>");
-  ffn8_gemm_kernel<1><<<grid, num_threads(1), SMEM_BYTES, st>>>(tmH, tmHN, tmW2, tmW2, offsets, E_loc, d, f, Y, d, nullptr, s2,
-                                                                nullptr, h_scale);
+  le = launch_pdl(ffn8_gemm_kernel<1>, dim3(grid), dim3(num_threads(1)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
+                  E_loc, d, f, Y, d, none, s2, none, h_scale);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn8_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn8_gemm_kernel<down>");
   return VIBE_OK;
 }
