@@ -617,8 +617,10 @@ def e4m3_decode_table():
     return t
 
 
-def e4m3_encode(x):
-    """f64 -> e4m3 codes (uint8): round to nearest, ties to even mantissa, saturate at +-448 (no NaN made)."""
+def e4m3_encode_scalar(x):
+    """f64 -> e4m3 codes (uint8): round to nearest, ties to even mantissa, saturate at +-448 (no NaN made).
+    The definition, element by element (slow); e4m3_encode below is the same arithmetic on whole arrays and
+    is pinned against this one."""
     x = np.asarray(x, dtype=np.float64)
     out = np.zeros(x.shape, dtype=np.uint8)
     flat, o = x.reshape(-1), out.reshape(-1)
@@ -649,6 +651,20 @@ def e4m3_encode(x):
     return out
 
 
+def e4m3_encode(x):
+    """The same rounding as e4m3_encode_scalar on whole arrays: |v| clamped to 448 = n * 2^(ex-3) with
+    ex = max(floor(log2 |v|), -6) and n = rint(|v| / 2^(ex-3)) (np.rint: ties to even n, i.e. to the even
+    mantissa); code = ((ex + 6) << 3) + n  (n < 8: subnormal; n = 16: carries into the next exponent)."""
+    x = np.asarray(x, dtype=np.float64)
+    a = np.minimum(np.abs(x), E4M3_MAX)
+    _, fe = np.frexp(a)                          # a = m * 2^fe, 0.5 <= m < 1  ->  floor(log2 a) = fe - 1
+    ex = np.maximum(fe - 1, -6)
+    n = np.rint(a / np.ldexp(1.0, ex - 3)).astype(np.int64)
+    code = ((ex.astype(np.int64) + 6) << 3) + n
+    code = np.where(a == 0, 0, code)
+    return (np.where(np.signbit(x), 0x80, 0) | code).astype(np.uint8)
+
+
 def fp8_pack_weights(W_bits):
     """bf16 bits [E,K,N] -> (codes uint8 [E,N,K] (K contiguous), scale f32 [E] = absmax/448; all-zero expert: 1)."""
     W = bf16_bits_to_f64(W_bits)
@@ -659,7 +675,9 @@ def fp8_pack_weights(W_bits):
         amax = float(np.max(np.abs(W[e])))
         if amax > 0:
             scale[e] = np.float32(amax / E4M3_MAX)
-        # the quotient is formed in binary32 (Q3), as the kernel does, then rounded ONCE to e4m3
+        # Q3: the quantiser is an elementwise binary32 program (bf16 input widened to binary32, binary32 scale):
+        # the quotient is the correctly rounded binary32 quotient, then rounded ONCE to e4m3.  Pinned by
+        # tests/golden/fp8_quotient_precision_example.json (a row where the f64 quotient gives another code)
         codes[e] = e4m3_encode((W[e].T.astype(np.float32) / scale[e]).astype(np.float64))
     return codes, scale
 
@@ -676,6 +694,11 @@ def fp8_quantize_rows(X_bits):
     codes = (e4m3_encode((X.astype(np.float32) / scale[:, None]).astype(np.float64)) if R
              else np.zeros_like(X_bits, dtype=np.uint8))
     return codes, scale
+
+
+def fp8_quantize_static(v, scale):
+    """Q3 with a given scale: v -> binary32, quotient by the binary32 scale formed in binary32, ONE rounding to e4m3."""
+    return e4m3_encode((np.asarray(v).astype(np.float32) / np.float32(scale)).astype(np.float64))
 
 
 def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q, s2, h_scale):
@@ -696,10 +719,99 @@ def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q
         g = (x @ T8[W1q[e]].T) * sx * np.float64(s1[e])
         u = (x @ T8[W3q[e]].T) * sx * np.float64(s3[e])
         h = g / (1.0 + np.exp(-g)) * u
-        hq = e4m3_encode(h / np.float64(h_scale[e]))
+        # Q3 applies to H as to X: the value is a binary32 number (the epilogue's), the quotient h/sh is formed
+        # in binary32 and rounded ONCE to e4m3
+        hq = fp8_quantize_static(h, h_scale[e])
         Hq[rows] = hq
         Y[rows] = (T8[hq] @ T8[W2q[e]].T) * np.float64(h_scale[e]) * np.float64(s2[e])
     return Y, Hq
+
+
+# ======================================================================================
+# O12  Block-scaled FP8 ("MXFP8": e4m3 elements, one power-of-two UE8M0 scale per block of the contraction
+#      dimension) grouped FFN (f2 as S8(f) words it: "e4m3, block-scaled").  The paper says only "Precision:
+#      FP8" (Table 2a); readings Q5-Q8:
+#      Q5  a block = `block` consecutive elements along K of one row (activations: a token row; weights: one
+#          output feature), block = 32 (the OCP-MX / tensor-core native block) or 128 (DeepSeek-V3's
+#          activation tile, stored as the same scale repeated over its four 32-blocks); scale = 2^e, stored
+#          as the byte e + 127 (UE8M0), one byte per 32 elements in either case.
+#      Q6  e = the smallest integer with amax <= 448 * 2^e (no element saturates), clamped to [-127, 127];
+#          an all-zero block: e = 0.  x / 2^e is EXACT in binary arithmetic, so no quotient-precision
+#          question arises (contrast Q3); one rounding, to e4m3 (RNE).
+#      Q7  the intermediate H is block-scaled the same way, per row and 32 features, from its binary32 value.
+#      Q8  products of the dequantised values (code value * 2^e, exact) accumulated in f64 (fp32 in the
+#          tensor core); SwiGLU in f64; Y not rounded here (the caller rounds / compares, C2).
+# ======================================================================================
+
+MX_BLOCK = 32            # elements per stored scale byte
+
+
+def ue8m0_exponent(amax):
+    """Q6: smallest integer e with amax <= 448 * 2^e, clamped to [-127, 127]; amax == 0 -> 0.
+    amax = m * 2^x with 1 <= m < 2:  448 = 1.75 * 2^8, so e = x - 8 if m <= 1.75 else x - 7."""
+    amax = np.asarray(amax, dtype=np.float64)
+    mant, ex = np.frexp(amax)                 # amax = mant * 2^ex, 0.5 <= mant < 1  ->  m = 2 mant, x = ex - 1
+    e = np.where(mant <= 0.875, ex - 1 - 8, ex - 1 - 7)
+    e = np.clip(e, -127, 127)
+    return np.where(amax == 0, 0, e).astype(np.int64)
+
+
+def mx_quantize(V, block=32):
+    """V f64 [..., K] (K a multiple of `block`, block in {32, 128}) -> (codes uint8 [..., K],
+    sf uint8 [..., K/32] = e + 127).  Block by block: amax, exponent (Q6), exact division, e4m3 RNE."""
+    assert block in (32, 128)
+    V = np.asarray(V, dtype=np.float64)
+    K = V.shape[-1]
+    assert K % block == 0
+    lead = V.shape[:-1]
+    Vb = V.reshape(lead + (K // block, block))
+    e = ue8m0_exponent(np.max(np.abs(Vb), axis=-1))                      # [..., K/block]
+    q = Vb / np.ldexp(1.0, e)[..., None]                                 # exact
+    codes = e4m3_encode(q).reshape(V.shape)
+    sf = np.repeat((e + 127).astype(np.uint8), block // MX_BLOCK, axis=-1)
+    return codes, sf
+
+
+def mx_dequantize(codes, sf):
+    """codes [..., K], sf [..., K/32] -> exact f64 values code_value * 2^(sf - 127)."""
+    T8 = e4m3_decode_table()
+    return T8[codes] * np.repeat(np.ldexp(1.0, sf.astype(np.int64) - 127), MX_BLOCK, axis=-1)
+
+
+def mx_pack_weights(W_bits, block=32):
+    """bf16 bits [E,K,N] -> (codes uint8 [E,N,K] (K contiguous), sf uint8 [E,N,K/32]): one scale per
+    output feature and K-block (Q5)."""
+    W = bf16_bits_to_f64(W_bits)
+    return mx_quantize(np.transpose(W, (0, 2, 1)), block)
+
+
+def mx_quantize_rows(X_bits, block=32):
+    """bf16 bits [R,d] -> (codes uint8 [R,d], sf uint8 [R,d/32])."""
+    return mx_quantize(bf16_bits_to_f64(X_bits), block)
+
+
+def grouped_ffn_mxfp8(Xq, Xsf, offsets, row_to_assign, W1q, W1sf, W3q, W3sf, W2q, W2sf):
+    """Per resident expert e and real row r (Q8):  g = x . w1,  u = x . w3  on the dequantised values,
+    h = silu(g) u,  (hq, hsf) = block-32 quantisation of binary32(h) along f (Q7),  y = deq(hq) . w2.
+    Returns (Y f64 [R,d], Hq codes [R,f], Hsf [R,f/32])."""
+    R = int(offsets[-1])
+    f, d = W1q.shape[1], W1q.shape[2]
+    Y = np.zeros((R, d), dtype=np.float64)
+    Hq = np.zeros((R, f), dtype=np.uint8)
+    Hsf = np.full((R, f // MX_BLOCK), 127, dtype=np.uint8)
+    for e in range(len(offsets) - 1):
+        lo, hi = int(offsets[e]), int(offsets[e + 1])
+        rows = [r for r in range(lo, hi) if row_to_assign[r] >= 0]
+        if not rows:
+            continue
+        x = mx_dequantize(Xq[rows], Xsf[rows])                          # [n,d]
+        g = x @ mx_dequantize(W1q[e], W1sf[e]).T
+        u = x @ mx_dequantize(W3q[e], W3sf[e]).T
+        h = g / (1.0 + np.exp(-g)) * u
+        hq, hsf = mx_quantize(h.astype(np.float32).astype(np.float64), 32)
+        Hq[rows], Hsf[rows] = hq, hsf
+        Y[rows] = mx_dequantize(hq, hsf) @ mx_dequantize(W2q[e], W2sf[e]).T
+    return Y, Hq, Hsf
 
 
 # ======================================================================================
