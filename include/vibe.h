@@ -196,6 +196,51 @@ VIBE_API vibe_status vibe_grouped_ffn_fp8(const void* Xq, const float* row_scale
                                           void* stream);
 
 /* ------------------------------------------------------------------------------------
+ * f2 as SURVEY 8(f) words it: "e4m3, BLOCK-SCALED".  The same FFN with one power-of-two (UE8M0) scale per
+ * operand row and 32 elements of the contraction dimension K, applied by the tensor core itself
+ * (tcgen05.mma kind::mxf8f6f4.block_scale).  The paper says only "Precision: FP8" (Table 2a);
+ * the recipe is DESIGN.md readings Q5-Q8:
+ *   block  = `block` (32 | 128) consecutive K elements of a row (a token row of X / H, one output feature of a
+ *            weight matrix); 128 = the same scale stored for its four 32-blocks;
+ *   scale  = 2^e, e = the smallest integer with amax <= 448 * 2^e, clamped to [-127, 127], 0 for an all-zero
+ *            block; stored as the byte e + 127, ONE BYTE PER 32 ELEMENTS;   code = e4m3_rne(x / 2^e)  (exact division).
+ * Scale-factor layouts (byte offset of the scale of row r -- a token row, or output feature n -- and 32-block b;
+ * KS = K/128):
+ *   VIBE_MX_SF_ROWMAJOR  [rows][K/32]:                 r * (K/32) + b
+ *   VIBE_MX_SF_TOKENS    [KS][32][Rb] 32-bit words:    (((b/4)*32 + r%32) * Rb + r/32) * 4 + b%4,
+ *                        Rb = ceil(R_cap/32) rounded up to a multiple of 4   (what vibe_grouped_ffn_mxfp8 reads:
+ *                        an aligned {4 row blocks x 32 rows} box of it is the tensor core's scale layout, and a tile
+ *                        may start at its row block 0 or 2, i.e. on any multiple of 64 rows)
+ *   VIBE_MX_SF_GATE_UP   [E_loc][KS][N/64] chunks of 512 B, W1 and W3 JOINTLY (the gate|up kernel keeps 64 features
+ *                        of each in one CTA):  ((e*KS + b/4)*(N/64) + n/64)*512 + (n%32)*16 + ((n%64)/32 + 2*up)*4 + b%4
+ *   VIBE_MX_SF_DOWN      [E_loc][KS][N/128] chunks:    ((e*KS + b/4)*(N/128) + n/128)*512 + (n%32)*16 + ((n%128)/32)*4 + b%4
+ * vibe_mxfp8_sf_bytes(which, rows, K, E_loc): bytes of such an array (rows = R / R_cap / N).
+ *
+ * vibe_mxfp8_quantize_rows: X bf16 [R,d] -> Xq e4m3 [R,d] + scales in ROWMAJOR or TOKENS layout (R_cap: row
+ *                           capacity that fixes Rb; ignored for ROWMAJOR).  d % 128 == 0.
+ * vibe_mxfp8_pack_weights : W bf16 [E_loc,K,N] -> Wq e4m3 [E_loc,N,K] + scales; role DOWN writes a DOWN array,
+ *                           roles GATE and UP write their halves of ONE GATE_UP array (call once with W1 / GATE
+ *                           and once with W3 / UP on the same `sf`).  K, N % 128 == 0.  One-time pass.
+ * vibe_grouped_ffn_mxfp8  : per resident expert and row:  g = x . w1, u = x . w3 on the block-dequantised values
+ *                           (fp32 accumulate), h = silu(g) u, (Hq, Hsf) = block-32 quantisation of h along f,
+ *                           Y = bf16(deq(hq) . w2).  Xq [R_cap,d], Xsf TOKENS layout (K = d); Hq_ws [R_cap,f] and
+ *                           Hsf_ws (TOKENS layout, K = f) are scratch; `offsets` MUST be multiples of 64
+ *                           (vibe_permute with align = 64): token tiles start on an even scale row block.
+ *                           d % 128 == 0, f % 128 == 0.  Conventions as vibe_grouped_ffn.
+ * ---------------------------------------------------------------------------------- */
+enum { VIBE_MX_SF_ROWMAJOR = 0, VIBE_MX_SF_TOKENS = 1, VIBE_MX_SF_GATE_UP = 2, VIBE_MX_SF_DOWN = 3 };
+enum { VIBE_MX_ROLE_DOWN = 0, VIBE_MX_ROLE_GATE = 1, VIBE_MX_ROLE_UP = 2 };
+VIBE_API size_t vibe_mxfp8_sf_bytes(int32_t which, int32_t rows, int32_t K, int32_t E_loc);
+VIBE_API vibe_status vibe_mxfp8_quantize_rows(const void* X, int32_t R, int32_t d, int32_t block, void* Xq, void* sf,
+                                              int32_t sf_layout, int32_t R_cap, void* stream);
+VIBE_API vibe_status vibe_mxfp8_pack_weights(const void* W, int32_t E_loc, int32_t K, int32_t N, int32_t block,
+                                             int32_t role, void* Wq, void* sf, void* stream);
+VIBE_API vibe_status vibe_grouped_ffn_mxfp8(const void* Xq, const void* Xsf, const int32_t* offsets, int32_t E_loc,
+                                            int32_t R_cap, int32_t d, int32_t f, const void* W1q, const void* W3q,
+                                            const void* sf13, const void* W2q, const void* sf2, void* Hq_ws,
+                                            void* Hsf_ws, void* Y, void* stream);
+
+/* ------------------------------------------------------------------------------------
  * a6.  Per-expert latency profile: measured vibe_grouped_ffn time versus tokens per
  * expert, at warmed steady state -- "Each GPU is warmed to steady-state operating
  * conditions and profiled independently using the fused MoE kernel across a range of
@@ -285,6 +330,16 @@ VIBE_API vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg /*host
                                                 const float* h_scale, void* out, int32_t* counts, void* arena,
                                                 size_t arena_bytes, void* stream);
 
+/* The whole layer with the BLOCK-SCALED FP8 FFN: route -> block-32 quantisation of the token rows (ROWMAJOR scales;
+ * on an expert-parallel shard only tokens with a resident expert) -> permute with align = 64 (one-byte rows) ->
+ * scale gather into the TOKENS layout -> vibe_grouped_ffn_mxfp8 -> combine.  Weights / scales as there;
+ * arena: vibe_workspace_bytes(VIBE_WS_LAYER_MXFP8, ...) bytes, 256-byte aligned.  d % 128 == 0, f % 128 == 0. */
+VIBE_API vibe_status vibe_moe_layer_forward_mxfp8(const vibe_route_cfg* cfg /*host*/, const float* logits,
+                                                  const void* X, const int32_t* expert_map, int32_t T, int32_t d,
+                                                  int32_t f, int32_t E_loc, const void* W1q, const void* W3q,
+                                                  const void* sf13, const void* W2q, const void* sf2, void* out,
+                                                  int32_t* counts, void* arena, size_t arena_bytes, void* stream);
+
 /* Workspace sizing.  `which` selects the consumer. */
 enum {
   VIBE_WS_PERMUTE = 0,
@@ -292,7 +347,8 @@ enum {
   VIBE_WS_PROFILE = 2, /* T = max tokens per expert of the sweep */
   VIBE_WS_LAYER = 3,
   VIBE_WS_LAYER_HOST = 4,
-  VIBE_WS_LAYER_FP8 = 5
+  VIBE_WS_LAYER_FP8 = 5,
+  VIBE_WS_LAYER_MXFP8 = 6
 };
 VIBE_API size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int32_t E, int32_t E_loc, int32_t d,
                                      int32_t f, int32_t align);

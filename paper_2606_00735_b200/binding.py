@@ -26,7 +26,10 @@ LIB_PATH = os.path.join(_PKG, "libvibe.so")
 VIBE_OK = 0
 SCORE_SOFTMAX = 0
 SCORE_SIGMOID = 1
-WS_PERMUTE, WS_FFN, WS_PROFILE, WS_LAYER, WS_LAYER_HOST, WS_LAYER_FP8 = 0, 1, 2, 3, 4, 5
+WS_PERMUTE, WS_FFN, WS_PROFILE, WS_LAYER, WS_LAYER_HOST, WS_LAYER_FP8, WS_LAYER_MXFP8 = 0, 1, 2, 3, 4, 5, 6
+MX_SF_ROWMAJOR, MX_SF_TOKENS, MX_SF_GATE_UP, MX_SF_DOWN = 0, 1, 2, 3
+MX_ROLE_DOWN, MX_ROLE_GATE, MX_ROLE_UP = 0, 1, 2
+MX_ROW_ALIGN = 64
 MODEL_A, MODEL_B = 0, 1
 
 # every symbol include/vibe.h declares (tests check that the .so exports exactly these)
@@ -38,6 +41,8 @@ EXPORTED_SYMBOLS = (
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
     "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward_host_chunked",
+    "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
+    "vibe_moe_layer_forward_mxfp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
     "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine",
@@ -119,6 +124,13 @@ def load() -> C.CDLL:
                                                         vp, vp, vp, i32, vp, sz, vp]
     lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                                vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_mxfp8_sf_bytes.argtypes = [i32] * 4
+    lib.vibe_mxfp8_sf_bytes.restype = sz
+    lib.vibe_mxfp8_quantize_rows.argtypes = [vp, i32, i32, i32, vp, vp, i32, i32, vp]
+    lib.vibe_mxfp8_pack_weights.argtypes = [vp, i32, i32, i32, i32, i32, vp, vp, vp]
+    lib.vibe_grouped_ffn_mxfp8.argtypes = [vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vibe_moe_layer_forward_mxfp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
+                                                 vp, vp, vp, sz, vp]
     lib.vibe_workspace_bytes.argtypes = [i32] * 8
     lib.vibe_workspace_bytes.restype = sz
     lib.vibe_rows_cap.argtypes = [i32] * 4
@@ -152,6 +164,7 @@ def load() -> C.CDLL:
                  "vibe_profile_expert_latency", "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host",
                  "vibe_moe_layer_forward_host_chunked", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
                  "vibe_drift_monitor_set_reference", "vibe_drift_monitor_rearranged",
+                 "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8", "vibe_moe_layer_forward_mxfp8",
                  "vibe_drift_monitor_window_mean", "vibe_placement_swap_refine"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
@@ -349,6 +362,110 @@ def grouped_ffn_fp8(Xq, row_scale, offsets, W1q, s1, W3q, s3, W2q, s2, h_scale, 
 
 
 # ------------------------------------------------------------------------------------ a5
+# ------------------------------------------------------------------------------------ f2: block-scaled FP8
+def mxfp8_sf_bytes(which: int, rows: int, K: int, E_loc: int = 1) -> int:
+    return int(load().vibe_mxfp8_sf_bytes(which, rows, K, E_loc))
+
+
+def mxfp8_sf_offsets(which: int, rows: int, K: int, R_cap: int = 0, role: int = MX_ROLE_DOWN):
+    """Byte offsets [rows, K/32] (int64, CPU) of the scale of (row r, 32-block b) inside one expert's part of a
+    scale array: the layout formulas of include/vibe.h written out as index arithmetic (no arithmetic of the
+    method).  Tests use it to read a device layout back into row-major order."""
+    r = torch.arange(rows, dtype=torch.int64)[:, None]
+    b = torch.arange(K // 32, dtype=torch.int64)[None, :]
+    if which == MX_SF_ROWMAJOR:
+        return r * (K // 32) + b
+    if which == MX_SF_TOKENS:
+        Rb = ((max(R_cap, rows) + 31) // 32 + 3) // 4 * 4
+        return (((b // 4) * 32 + r % 32) * Rb + r // 32) * 4 + b % 4
+    if which == MX_SF_GATE_UP:
+        return ((b // 4) * (rows // 64) + r // 64) * 512 + (r % 32) * 16 + ((r % 64) // 32 + (2 if role == MX_ROLE_UP else 0)) * 4 + b % 4
+    if which == MX_SF_DOWN:
+        return ((b // 4) * (rows // 128) + r // 128) * 512 + (r % 32) * 16 + ((r % 128) // 32) * 4 + b % 4
+    raise VibeError("bad scale-factor layout")
+
+
+def mxfp8_quantize_rows(X: torch.Tensor, block: int = 32, sf_layout: int = MX_SF_ROWMAJOR, R_cap: int = 0, stream=None):
+    """bf16 [R,d] -> (Xq uint8 e4m3 codes [R,d], sf uint8: [R,d/32] row-major, or the flat TOKENS-layout array)"""
+    lib = load()
+    _check(X, torch.bfloat16, "X")
+    R, d = X.shape
+    R_cap = max(R_cap, R)
+    Xq = torch.empty((R, d), dtype=torch.uint8, device=X.device)
+    if sf_layout == MX_SF_ROWMAJOR:
+        sf = torch.empty((R, d // 32), dtype=torch.uint8, device=X.device)
+    else:
+        sf = torch.full((max(16, mxfp8_sf_bytes(MX_SF_TOKENS, R_cap, d)),), 127, dtype=torch.uint8, device=X.device)
+    _ok(lib.vibe_mxfp8_quantize_rows(X.data_ptr(), R, d, block, Xq.data_ptr(), sf.data_ptr(), sf_layout, R_cap,
+                                     _stream(stream)), "vibe_mxfp8_quantize_rows")
+    return Xq, sf
+
+
+def mxfp8_pack_weights(W: torch.Tensor, role: int, block: int = 32, sf: Optional[torch.Tensor] = None, stream=None):
+    """bf16 [E,K,N] -> (Wq uint8 e4m3 codes [E,N,K], sf uint8 flat): role DOWN -> a DOWN scale array; roles GATE / UP
+    fill their halves of one GATE_UP array (pass the array returned for W1 as `sf` when packing W3)."""
+    lib = load()
+    _check(W, torch.bfloat16, "W")
+    E, K, N = W.shape
+    Wq = torch.empty((E, N, K), dtype=torch.uint8, device=W.device)
+    if sf is None:
+        which = MX_SF_DOWN if role == MX_ROLE_DOWN else MX_SF_GATE_UP
+        sf = torch.full((max(16, mxfp8_sf_bytes(which, N, K, E)),), 127, dtype=torch.uint8, device=W.device)
+    _ok(lib.vibe_mxfp8_pack_weights(W.data_ptr(), E, K, N, block, role, Wq.data_ptr(), sf.data_ptr(), _stream(stream)),
+        "vibe_mxfp8_pack_weights")
+    return Wq, sf
+
+
+def grouped_ffn_mxfp8(Xq, Xsf, offsets, W1q, W3q, sf13, W2q, sf2, Hq=None, Hsf=None, Y=None, stream=None):
+    """-> (Y bf16 [R_cap,d], Hq uint8 [R_cap,f], Hsf uint8 flat (TOKENS layout, K = f)); offsets multiples of 32."""
+    lib = load()
+    for t, n in ((Xq, "Xq"), (Xsf, "Xsf"), (W1q, "W1q"), (W3q, "W3q"), (W2q, "W2q"), (sf13, "sf13"), (sf2, "sf2")):
+        _check(t, torch.uint8, n)
+    _check(offsets, torch.int32, "offsets")
+    Rcap, d = Xq.shape
+    E_loc, f, d1 = W1q.shape
+    if d1 != d or tuple(W3q.shape) != (E_loc, f, d) or tuple(W2q.shape) != (E_loc, d, f):
+        raise VibeError("packed weight shapes must be W1q,W3q [E_loc,f,d], W2q [E_loc,d,f]")
+    if Xsf.numel() < mxfp8_sf_bytes(MX_SF_TOKENS, Rcap, d) or sf13.numel() < mxfp8_sf_bytes(MX_SF_GATE_UP, f, d, E_loc) \
+            or sf2.numel() < mxfp8_sf_bytes(MX_SF_DOWN, d, f, E_loc):
+        raise VibeError("scale-factor array too small for its layout")
+    if Hq is None:
+        Hq = torch.empty((Rcap, f), dtype=torch.uint8, device=Xq.device)
+    if Hsf is None:
+        Hsf = torch.full((max(16, mxfp8_sf_bytes(MX_SF_TOKENS, Rcap, f)),), 127, dtype=torch.uint8, device=Xq.device)
+    if Y is None:
+        Y = torch.empty((Rcap, d), dtype=torch.bfloat16, device=Xq.device)
+    _ok(lib.vibe_grouped_ffn_mxfp8(Xq.data_ptr(), Xsf.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1q.data_ptr(),
+                                   W3q.data_ptr(), sf13.data_ptr(), W2q.data_ptr(), sf2.data_ptr(), Hq.data_ptr(),
+                                   Hsf.data_ptr(), Y.data_ptr(), _stream(stream)), "vibe_grouped_ffn_mxfp8")
+    return Y, Hq, Hsf
+
+
+def moe_layer_forward_mxfp8(cfg: RouteConfig, logits, X, expert_map, W1q, W3q, sf13, W2q, sf2, out=None, counts=None,
+                            arena=None, stream=None):
+    """The whole layer with the block-scaled FP8 FFN (weights packed by mxfp8_pack_weights)."""
+    lib = load()
+    _check(logits, torch.float32, "logits")
+    _check(X, torch.bfloat16, "X")
+    T, d = X.shape
+    E_loc, f, _ = W1q.shape
+    dev = X.device
+    if out is None:
+        out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
+    if counts is None:
+        counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
+    need = workspace_bytes(WS_LAYER_MXFP8, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
+    if arena is None:
+        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+    c = cfg._c()
+    _ok(lib.vibe_moe_layer_forward_mxfp8(C.byref(c), logits.data_ptr(), X.data_ptr(),
+                                         expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
+                                         W1q.data_ptr(), W3q.data_ptr(), sf13.data_ptr(), W2q.data_ptr(), sf2.data_ptr(),
+                                         out.data_ptr(), counts.data_ptr(), arena.data_ptr(), arena.numel(),
+                                         _stream(stream)), "vibe_moe_layer_forward_mxfp8")
+    return out, counts
+
+
 def combine(Y: torch.Tensor, assign_to_row: torch.Tensor, topk_w: torch.Tensor, T: int, k: int,
             out: Optional[torch.Tensor] = None, stream=None):
     lib = load()

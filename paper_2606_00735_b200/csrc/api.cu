@@ -81,6 +81,35 @@ LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f) {
   return a;
 }
 
+LayerArenaMx layer_arena_mx(int T, int k, int E_loc, int d, int f) {
+  LayerArenaMx a{};
+  const size_t A = (size_t)T * k;
+  a.R_cap = vibe_rows_cap(T, k, E_loc, kMxRowAlign);
+  if (a.R_cap < 1) a.R_cap = 1;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o += round_up(bytes ? bytes : 16, 256);
+    return at;
+  };
+  const size_t Rb = (size_t)mx_row_blocks((int)a.R_cap);
+  a.ids = take(A * 4);
+  a.w = take(A * 4);
+  a.offsets = take((size_t)(E_loc + 1) * 4);
+  a.r2a = take((size_t)a.R_cap * 4);
+  a.a2r = take(A * 4);
+  a.Xq = take((size_t)T * d);
+  a.tok_sf = take((size_t)T * (d / 32));
+  a.Xpq = take((size_t)a.R_cap * d);
+  a.xsf = take((size_t)(d / 128) * 32 * Rb * 4);
+  a.Hq = take((size_t)a.R_cap * f);
+  a.hsf = take((size_t)(f / 128) * 32 * Rb * 4);
+  a.Y = take((size_t)a.R_cap * d * 2);
+  a.perm_ws = take(permute_ws_bytes(T, k, E_loc));
+  a.total = o;
+  return a;
+}
+
 }  // namespace vibe
 
 extern "C" const char* vibe_status_string(vibe_status s) {
@@ -111,6 +140,7 @@ extern "C" size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int3
     }
     case VIBE_WS_LAYER: return layer_arena(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_FP8: return layer_arena_fp8(T, k, E_loc, d, f).total;
+    case VIBE_WS_LAYER_MXFP8: return (d % 128 || f % 128 || d < 128 || f < 128) ? 0 : layer_arena_mx(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_HOST:
       return layer_arena(T, k, E_loc, d, f).total + round_up((size_t)T * E * 4, 256) +
              round_up((size_t)T * d * 2, 256) * 2 + round_up((size_t)E * 4, 256) +

@@ -60,6 +60,13 @@ vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const i
                                  int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
                                  const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
                                  cudaStream_t st);
+vibe_status grouped_ffn_mxfp8_impl(const void* Xq, const void* xsf, const int32_t* offsets, int E_loc, int R_cap, int d,
+                                   int f, const void* W1q, const void* W3q, const void* sf13, const void* W2q,
+                                   const void* sf2, void* Hq, void* hsf, void* Y, cudaStream_t st);
+// words per (K stage, lane) row of a token-scale array [K/128][32][Rb]: the 32-row blocks of R_cap rows, rounded up to
+// a 16-byte row pitch (a TMA global stride; the kernel only fetches boxes of 4 row blocks that start on a multiple of 4,
+// so a box is entirely inside or entirely outside the tensor)
+static inline int mx_row_blocks(int R_cap) { return (((R_cap + 31) / 32) + 3) & ~3; }
 vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                               const void* W1, const void* W3, const void* W2, void* H_ws, void* Y);
 
@@ -67,6 +74,10 @@ vibe_status fp8_gather_row_scales(const float* tok_scale, const int32_t* row_to_
                                   int k, int R_cap, float* row_scale, cudaStream_t st);
 vibe_status fp8_quantize_resident_tokens(const void* X, int T, int d, void* Xq, float* tok_scale, const int32_t* ids,
                                          const int32_t* emap, int k, int E, int E_loc, cudaStream_t st);
+vibe_status mx_gather_row_sf(const void* tok_sf, const int32_t* row_to_assign, const int32_t* offsets, int E_loc, int k,
+                             int R_cap, int d, void* out, cudaStream_t st);
+vibe_status mx_quantize_rows(const void* X, int R, int d, int block, void* Xq, void* sf, int sf_layout, int R_cap,
+                             const int32_t* ids, const int32_t* emap, int k, int E, int E_loc, cudaStream_t st);
 // Launch with the programmatic-stream-serialization attribute (the kernel calls ptx::griddep_wait before it reads
 // what the preceding kernel of the stream wrote).
 template <class... KArgs, class... Args>
@@ -89,6 +100,12 @@ struct LayerArenaFp8 {
   int64_t R_cap;
 };
 LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f);
+struct LayerArenaMx {
+  size_t ids, w, offsets, r2a, a2r, Xq, tok_sf, Xpq, xsf, Hq, hsf, Y, perm_ws, total;
+  int64_t R_cap;
+};
+LayerArenaMx layer_arena_mx(int T, int k, int E_loc, int d, int f);
+constexpr int kMxRowAlign = 64;   // vibe_permute align of the block-scaled path: token tiles start on an even scale row block
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 static inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }

@@ -251,3 +251,50 @@ extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, con
     return s;
   return vibe_combine(base + a.Y, a2r, w, T, k, d, out, stream);
 }
+
+extern "C" vibe_status vibe_moe_layer_forward_mxfp8(const vibe_route_cfg* cfg, const float* logits, const void* X,
+                                                    const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
+                                                    int32_t E_loc, const void* W1q, const void* W3q, const void* sf13,
+                                                    const void* W2q, const void* sf2, void* out, int32_t* counts,
+                                                    void* arena, size_t arena_bytes, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(cfg != nullptr, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: cfg is NULL");
+  VIBE_REQUIRE(T >= 0 && d >= 128 && f >= 128 && E_loc >= 1, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: bad sizes");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0, VIBE_ERR_UNSUPPORTED,
+               "vibe_moe_layer_forward_mxfp8: d and f must be multiples of 128 (d=%d f=%d)", d, f);
+  VIBE_REQUIRE(E_loc <= 512, VIBE_ERR_UNSUPPORTED, "vibe_moe_layer_forward_mxfp8: E_loc > 512 not implemented");
+  const int E = cfg->num_experts, k = cfg->top_k;
+  VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: need 1 <= k <= E");
+  VIBE_REQUIRE(W1q && W3q && sf13 && W2q && sf2 && aligned16(W1q) && aligned16(W3q) && aligned16(sf13) && aligned16(W2q) &&
+                   aligned16(sf2),
+               VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: weight / scale tensor NULL or not 16-byte aligned");
+  const LayerArenaMx a = layer_arena_mx(T, k, E_loc, d, f);
+  VIBE_REQUIRE(arena != nullptr && arena_bytes >= a.total && (reinterpret_cast<uintptr_t>(arena) & 255u) == 0,
+               VIBE_ERR_WORKSPACE, "vibe_moe_layer_forward_mxfp8: arena needs %zu bytes, 256-byte aligned (got %zu)",
+               a.total, arena_bytes);
+  VIBE_REQUIRE(a.R_cap < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: row capacity >= 2^31");
+  VIBE_REQUIRE(T == 0 || (X != nullptr && aligned16(X)), VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_mxfp8: X NULL or misaligned");
+  char* base = reinterpret_cast<char*>(arena);
+  int32_t* ids = reinterpret_cast<int32_t*>(base + a.ids);
+  float* w = reinterpret_cast<float*>(base + a.w);
+  int32_t* offsets = reinterpret_cast<int32_t*>(base + a.offsets);
+  int32_t* r2a = reinterpret_cast<int32_t*>(base + a.r2a);
+  int32_t* a2r = reinterpret_cast<int32_t*>(base + a.a2r);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  vibe_status s;
+  if ((s = vibe_route_topk(cfg, logits, T, ids, w, counts, stream)) != VIBE_OK) return s;
+  // tokens are quantised BEFORE the permutation (T rows instead of T*k); the permutation then moves one-byte rows
+  if ((s = mx_quantize_rows(X, T, d, 32, base + a.Xq, base + a.tok_sf, VIBE_MX_SF_ROWMAJOR, T,
+                            (expert_map && E_loc < E) ? ids : nullptr, expert_map, k, E, E_loc, st)) != VIBE_OK)
+    return s;
+  if ((s = vibe_permute(base + a.Xq, ids, counts, expert_map, T, d / 2, k, E, E_loc, kMxRowAlign, base + a.Xpq, offsets, r2a,
+                        a2r, base + a.perm_ws, permute_ws_bytes(T, k, E_loc), stream)) != VIBE_OK)
+    return s;
+  if (T == 0) return VIBE_OK;
+  if ((s = mx_gather_row_sf(base + a.tok_sf, r2a, offsets, E_loc, k, (int)a.R_cap, d, base + a.xsf, st)) != VIBE_OK) return s;
+  if ((s = grouped_ffn_mxfp8_impl(base + a.Xpq, base + a.xsf, offsets, E_loc, (int)a.R_cap, d, f, W1q, W3q, sf13, W2q, sf2,
+                                  base + a.Hq, base + a.hsf, base + a.Y, st)) != VIBE_OK)
+    return s;
+  return vibe_combine(base + a.Y, a2r, w, T, k, d, out, stream);
+}

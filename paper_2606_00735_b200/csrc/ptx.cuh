@@ -279,5 +279,40 @@ __device__ __forceinline__ uint32_t pack2_e4m3(float lo, float hi) {
   return (uint32_t)r;
 }
 
+
+// ---------------------------------------------------------------- block-scaled e4m3 (kind::mxf8f6f4.block_scale)
+// One UE8M0 scale per operand row and 32 K elements; the scales of a K = 128 stage live in TMEM as 32-bit words
+// (byte j = K-block j): operand row r of the instruction's tile -> lane r % 32 (replicated in the four lane
+// quarters), column base + r / 32.  Instruction descriptor (32-bit):
+//   [4,6) B scale-factor id (byte of the word)   [7,10) A format: 0 = e4m3   [10,13) B format: 0 = e4m3
+//   [15] A major 0 = K   [16] B major 0 = K   [17,23) N >> 3   [23] scale format: 1 = UE8M0   [24,29) M >> 4
+//   [29,31) A scale-factor id
+__host__ __device__ constexpr uint32_t make_idesc_mxe4m3(int M, int N) {
+  return ((uint32_t)(N >> 3) << 17) | (1u << 23) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void umma_mxf8_2sm(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                              uint32_t accumulate, uint32_t tmem_sfa, uint32_t tmem_sfb) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n\t}" ::"r"(tmem_d),
+      "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate), "r"(tmem_sfa), "r"(tmem_sfb)
+      : "memory");
+}
+// shared memory -> TMEM, 32 rows x 16 bytes broadcast to the four lane quarters, in BOTH CTAs of the pair (each
+// from its own shared memory at the descriptor's offset); ordered with the MMAs of the issuing thread.
+__device__ __forceinline__ void tmem_cp_32x128b_warpx4_2sm(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::2.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+// descriptor of 32 contiguous 16-byte rows (no swizzle: 8-row core matrices 128 bytes apart)
+__device__ __forceinline__ uint64_t make_smem_desc_rows16(uint32_t smem_addr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((smem_addr >> 4) & 0x3fffu);
+  d |= (uint64_t)(128u >> 4) << 16;
+  d |= (uint64_t)(128u >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  return d;
+}
+
 }  // namespace ptx
 }  // namespace vibe
