@@ -316,31 +316,48 @@ def main():
     # the timed region (they are static in serving); the activations are quantised inside it.
     fp8 = None
     if d % 128 == 0 and f % 128 == 0:
+        def time_layer(fn, n):
+            for i in range(max(3, args.warmup // 4)):
+                fn(i)
+            torch.cuda.synchronize()
+            a8, b8 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a8.record(stream)
+            for i in range(n):
+                fn(i)
+            b8.record(stream)
+            torch.cuda.synchronize()
+            return a8.elapsed_time(b8) / n
+
+        n8 = max(20, args.steps // 2)
+        cnt8 = torch.empty((E,), dtype=torch.int32, device=dev)
+        # (i) block-scaled e4m3 (readings Q5-Q8: UE8M0 scale per row and 32 K elements, applied by the tensor core)
+        W1m, sf13 = B.mxfp8_pack_weights(W1, B.MX_ROLE_GATE)
+        W3m, sf13 = B.mxfp8_pack_weights(W3, B.MX_ROLE_UP, sf=sf13)
+        W2m, sf2 = B.mxfp8_pack_weights(W2, B.MX_ROLE_DOWN)
+        arena_mx = torch.empty((B.workspace_bytes(B.WS_LAYER_MXFP8, T, k, E, E_loc, d, f),), dtype=torch.uint8, device=dev)
+        ms_mx = time_layer(lambda i: B.moe_layer_forward_mxfp8(rc, *sets_d[i % args.sets], emap, W1m, W3m, sf13, W2m, sf2,
+                                                               out=out, counts=cnt8, arena=arena_mx, stream=stream), n8)
+        del W1m, W3m, W2m, arena_mx
+        # (ii) per-expert / per-row scales (Q1-Q4).  The static scale of the intermediate is CALIBRATED on this
+        # workload: 2 x the largest |H| per expert of the bf16 path on batch 0, / 448; the fraction of H codes that
+        # sit on the saturation value in a step is reported
+        step(0)
+        torch.cuda.synchronize()
+        offs = off.tolist()
+        hs8 = torch.tensor([2.0 * float(H[offs[e]:offs[e + 1]].abs().max()) / 448.0 if offs[e + 1] > offs[e] else 1.0
+                            for e in range(E_loc)], dtype=torch.float32, device=dev).clamp_min(1e-6)
         W1q, s1q = B.fp8_pack_weights(W1)
         W3q, s3q = B.fp8_pack_weights(W3)
         W2q, s2q = B.fp8_pack_weights(W2)
-        hs8 = torch.full((E_loc,), 8.0 / 448.0, dtype=torch.float32, device=dev)
-        arena8 = torch.empty((B.workspace_bytes(B.WS_LAYER_FP8, T, k, E, E_loc, d, f),), dtype=torch.uint8, device=dev)
-        cnt8 = torch.empty((E,), dtype=torch.int32, device=dev)
-
-        def step8(i):
-            lg, Xd = sets_d[i % args.sets]
-            B.moe_layer_forward_fp8(rc, lg, Xd, emap, W1q, s1q, W3q, s3q, W2q, s2q, hs8, out=out, counts=cnt8,
-                                    arena=arena8, stream=stream)
-
-        n8 = max(20, args.steps // 2)
-        for i in range(max(3, args.warmup // 4)):
-            step8(i)
-        torch.cuda.synchronize()
-        a8, b8 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a8.record(stream)
-        for i in range(n8):
-            step8(i)
-        b8.record(stream)
-        torch.cuda.synchronize()
-        ms8 = a8.elapsed_time(b8) / n8
-        fp8 = {"layer_tokens_per_s": round(T / ms8 * 1e3), "ms_per_step": round(ms8, 4), "steps": n8,
-               "note": "vibe_moe_layer_forward_fp8 (e4m3 weights/activations, fp32 accumulate), one rank"}
+        la = B.workspace_bytes(B.WS_LAYER_FP8, T, k, E, E_loc, d, f)
+        arena8 = torch.empty((la,), dtype=torch.uint8, device=dev)
+        ms8 = time_layer(lambda i: B.moe_layer_forward_fp8(rc, *sets_d[i % args.sets], emap, W1q, s1q, W3q, s3q, W2q, s2q,
+                                                           hs8, out=out, counts=cnt8, arena=arena8, stream=stream), n8)
+        fp8 = {"mxfp8_layer_tokens_per_s": round(T / ms_mx * 1e3), "mxfp8_ms_per_step": round(ms_mx, 4),
+               "layer_tokens_per_s": round(T / ms8 * 1e3), "ms_per_step": round(ms8, 4), "steps": n8,
+               "note": "mxfp8 = vibe_moe_layer_forward_mxfp8 (block-scaled e4m3, UE8M0 scale per 32 K elements); the other pair = "
+                       "vibe_moe_layer_forward_fp8 (per-expert / per-row scales, h_scale calibrated: 2 x max|H| of batch 0 / 448); "
+                       "one rank; parity of both at this size: tests/test_gpu_full_size.py"}
         del W1q, W3q, W2q, arena8
 
     # ---------------------------------------------------------------- roofline of the dominant kernel

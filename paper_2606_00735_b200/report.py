@@ -274,6 +274,10 @@ def section_ffn_fp8(peaks, quick):
         W3q, s3 = B.fp8_pack_weights(W3)
         W2q, s2 = B.fp8_pack_weights(W2)
         hs = torch.full((E,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+        # the block-scaled variant (readings Q5-Q8): same weights, one UE8M0 scale per row and 32 K elements
+        W1m, sf13 = B.mxfp8_pack_weights(W1, B.MX_ROLE_GATE)
+        W3m, sf13 = B.mxfp8_pack_weights(W3, B.MX_ROLE_UP, sf=sf13)
+        W2m, sf2 = B.mxfp8_pack_weights(W2, B.MX_ROLE_DOWN)
         for n in ((512, 2048) if quick else (128, 512, 1024, 2048, 4096)):
             R = E * n
             Xp = torch.randn((R, d), device="cuda").to(torch.bfloat16)
@@ -283,6 +287,9 @@ def section_ffn_fp8(peaks, quick):
             H = torch.empty((R, f), dtype=torch.bfloat16, device="cuda")
             Y = torch.empty((R, d), dtype=torch.bfloat16, device="cuda")
             f8 = lambda i: B.grouped_ffn_fp8(Xq, rs, off, W1q, s1, W3q, s3, W2q, s2, hs, Hq=Hq, Y=Y)
+            Xm, xsf = B.mxfp8_quantize_rows(Xp, 32, B.MX_SF_TOKENS, R_cap=R)     # n is a multiple of 64: offsets aligned
+            hsf = torch.full((max(16, B.mxfp8_sf_bytes(B.MX_SF_TOKENS, R, f)),), 127, dtype=torch.uint8, device="cuda")
+            mx = lambda i: B.grouped_ffn_mxfp8(Xm, xsf, off, W1m, W3m, sf13, W2m, sf2, Hq=Hq, Hsf=hsf, Y=Y)
             bf = lambda i: B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y)
             t0 = time.time()
             while time.time() - t0 < (0.2 if quick else 1.0):
@@ -292,14 +299,20 @@ def section_ffn_fp8(peaks, quick):
             t8 = _time(f8, iters)
             tb = _time(bf, iters)
             tq = _time(lambda i: B.fp8_quantize_rows(Xp), iters)
+            tm = _time(mx, iters)
+            tmq = _time(lambda i: B.mxfp8_quantize_rows(Xp, 32, B.MX_SF_TOKENS, R_cap=R), iters)
             flops = 6.0 * R * d * f
             out.append({"shape": cfg.name, "tokens_per_expert": n, "fp8_us": round(t8, 1), "bf16_us": round(tb, 1),
                         "quantize_rows_us": round(tq, 1), "fp8_TFLOP/s": round(flops / t8 / 1e6, 1),
                         "bf16_TFLOP/s": round(flops / tb / 1e6, 1), "speedup": round(tb / t8, 3),
                         "fp8_frac_of_2x_bf16_sustained": round(flops / t8 / 1e6 / (2 * peaks["bf16_tflops_sustained"]), 4),
-                        "fp8_frac_of_2x_bf16_burst": round(flops / t8 / 1e6 / (2 * peaks["bf16_tflops"]), 4)})
-            del Xp, Xq, Hq, H, Y
-        del W1, W3, W2, W1q, W3q, W2q
+                        "fp8_frac_of_2x_bf16_burst": round(flops / t8 / 1e6 / (2 * peaks["bf16_tflops"]), 4),
+                        "mxfp8_us": round(tm, 1), "mxfp8_quantize_rows_us": round(tmq, 1),
+                        "mxfp8_TFLOP/s": round(flops / tm / 1e6, 1), "mxfp8_speedup_vs_bf16": round(tb / tm, 3),
+                        "mxfp8_frac_of_2x_bf16_sustained": round(flops / tm / 1e6 / (2 * peaks["bf16_tflops_sustained"]), 4),
+                        "mxfp8_frac_of_2x_bf16_burst": round(flops / tm / 1e6 / (2 * peaks["bf16_tflops"]), 4)})
+            del Xp, Xq, Hq, H, Y, Xm, xsf, hsf
+        del W1, W3, W2, W1q, W3q, W2q, W1m, W3m, W2m, sf13, sf2
         torch.cuda.empty_cache()
     return out
 
