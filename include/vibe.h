@@ -254,7 +254,11 @@ VIBE_API vibe_status vibe_grouped_ffn_mxfp8(const void* Xq, const void* Xsf, con
  * after max(warmup, 1) untimed calls per point.  The timed executions replay one call
  * captured into a CUDA graph, on a stream of the sweep's own, so that an event pair
  * brackets the kernels and not the host's work between launches (a lone small expert
- * takes less device time than the host needs to launch it).  Activations are an arbitrary
+ * takes less device time than the host needs to launch it).  Every timed execution starts
+ * COLD: before its first event an evict_last read sweep over 256 MB (twice the L2; a region at
+ * the end of ws) evicts what the previous execution left in L2 -- a sweep point whose weights
+ * fit the 126 MB L2 would otherwise be replayed on L2-resident weights and read faster than it
+ * does inside a model.  Activations are an arbitrary
  * finite pattern written by the library into ws (latency does not depend on values).
  * This call SYNCHRONISES the stream (before the sweep) and returns when the sweep is done.  tokens_per_expert, latency_us, samples_us: HOST.
  * samples_us: optional host [n_points*iters] per-iteration times (NULL to skip).

@@ -191,6 +191,16 @@ def _stream(stream) -> int:
     return s.cuda_stream
 
 
+def _scratch(nbytes: int, device, stream) -> torch.Tensor:
+    """A temporary workspace / arena the call itself allocates.  It is allocated UNDER the launch stream: the caching
+    allocator then ties its reuse to that stream, so returning it to the pool right after the (asynchronous) call is
+    safe even when `stream` is not torch's current stream."""
+    if stream is None:
+        return torch.empty((max(nbytes, 16),), dtype=torch.uint8, device=device)
+    with torch.cuda.stream(stream):
+        return torch.empty((max(nbytes, 16),), dtype=torch.uint8, device=device)
+
+
 def launch_count() -> int:
     return int(load().vibe_launch_count())
 
@@ -244,7 +254,7 @@ def permute(X: torch.Tensor, topk_ids: torch.Tensor, counts: Optional[torch.Tens
         Xp, offsets, r2a, a2r = out
     need = workspace_bytes(WS_PERMUTE, T, k, E, E_loc, d, 0, align)
     if ws is None:
-        ws = torch.empty((max(need, 16),), dtype=torch.uint8, device=dev)
+        ws = _scratch(need, dev, stream)
     _ok(lib.vibe_permute(X.data_ptr(), topk_ids.data_ptr(), counts.data_ptr() if counts is not None else None,
                          expert_map.data_ptr() if expert_map is not None else None, T, d, k, E, E_loc, align,
                          Xp.data_ptr(), offsets.data_ptr(), r2a.data_ptr(), a2r.data_ptr(), ws.data_ptr(),
@@ -456,7 +466,7 @@ def moe_layer_forward_mxfp8(cfg: RouteConfig, logits, X, expert_map, W1q, W3q, s
         counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
     need = workspace_bytes(WS_LAYER_MXFP8, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
     if arena is None:
-        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+        arena = _scratch(need, dev, stream)
     c = cfg._c()
     _ok(lib.vibe_moe_layer_forward_mxfp8(C.byref(c), logits.data_ptr(), X.data_ptr(),
                                          expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
@@ -500,7 +510,7 @@ def profile_expert_latency(W1: torch.Tensor, W3: torch.Tensor, W2: torch.Tensor,
     samples = (C.c_float * (npts * iters))() if return_samples else None
     need = workspace_bytes(WS_PROFILE, max(tokens_per_expert), 1, E_loc, E_loc, d, f, 1)
     if ws is None:
-        ws = torch.empty((need,), dtype=torch.uint8, device=W1.device)
+        ws = _scratch(need, W1.device, stream)
     _ok(lib.vibe_profile_expert_latency(E_loc, d, f, W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), toks, npts, mode,
                                         warmup, iters, lat, samples, ws.data_ptr(), ws.numel(), _stream(stream)),
         "vibe_profile_expert_latency")
@@ -521,7 +531,7 @@ def profile_expert_latency_fp8(W1q, s1, W3q, s3, W2q, s2, h_scale, tokens_per_ex
     nmax = max(tokens_per_expert)
     need = (workspace_bytes(WS_PROFILE, nmax, 1, E_loc, E_loc, d, f, 1) + 255) // 256 * 256 + \
         (4 * E_loc * max(nmax, 1) + 255) // 256 * 256
-    ws = torch.empty((need,), dtype=torch.uint8, device=W1q.device)
+    ws = _scratch(need, W1q.device, stream)
     _ok(lib.vibe_profile_expert_latency_fp8(E_loc, d, f, W1q.data_ptr(), s1.data_ptr(), W3q.data_ptr(), s3.data_ptr(),
                                             W2q.data_ptr(), s2.data_ptr(), h_scale.data_ptr(), toks, npts, mode, warmup,
                                             iters, lat, None, ws.data_ptr(), ws.numel(), _stream(stream)),
@@ -544,7 +554,7 @@ def moe_layer_forward(cfg: RouteConfig, logits, X, expert_map, W1, W3, W2, out=N
         counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
     need = workspace_bytes(WS_LAYER, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
     if arena is None:
-        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+        arena = _scratch(need, dev, stream)
     c = cfg._c()
     _ok(lib.vibe_moe_layer_forward(C.byref(c), logits.data_ptr(), X.data_ptr(),
                                    expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
@@ -570,7 +580,7 @@ def moe_layer_forward_fp8(cfg: RouteConfig, logits, X, expert_map, W1q, s1, W3q,
         counts = torch.empty((cfg.num_experts,), dtype=torch.int32, device=dev)
     need = workspace_bytes(WS_LAYER_FP8, T, cfg.top_k, cfg.num_experts, E_loc, d, f, 1)
     if arena is None:
-        arena = torch.empty((need,), dtype=torch.uint8, device=dev)
+        arena = _scratch(need, dev, stream)
     c = cfg._c()
     _ok(lib.vibe_moe_layer_forward_fp8(C.byref(c), logits.data_ptr(), X.data_ptr(),
                                        expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,

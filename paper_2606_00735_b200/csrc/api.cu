@@ -1,5 +1,6 @@
 // api.cu -- status / error text / workspace sizing / launch accounting of libvibe.so.
 #include <string.h>
+#include <atomic>
 
 #include "common.cuh"
 
@@ -17,17 +18,23 @@ void set_error(const char* fmt, ...) {
 void clear_error() { g_err[0] = '\0'; }
 void count_launch(int n) { g_launches += n; }
 
+int current_device() {
+  int dev = 0;
+  return (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices) ? dev : 0;
+}
+
+// SM count of the CURRENT device (cached per device ordinal: a process may drive several GPUs)
 int num_sms() {
-  static int sms = 0;
-  if (sms == 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-      sms = v;
+  static std::atomic<int> sms[kMaxDevices];
+  const int dev = current_device();
+  int v = sms[dev].load(std::memory_order_relaxed);
+  if (v == 0) {
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+      sms[dev].store(v, std::memory_order_relaxed);
     else
       return 148;  // B200; only reached when no device is present (launch will fail loudly)
   }
-  return sms;
+  return v;
 }
 
 LayerArena layer_arena(int T, int k, int E_loc, int d, int f) {
@@ -136,7 +143,7 @@ extern "C" size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int3
     case VIBE_WS_FFN: return 0;
     case VIBE_WS_PROFILE: {
       const size_t R = (size_t)E_loc * (size_t)(T > 0 ? T : 1);
-      return round_up(R * d * 2, 256) * 2 + round_up(R * f * 2, 256) + round_up((size_t)(E_loc + 1) * 4, 256);
+      return round_up(R * d * 2, 256) * 2 + round_up(R * f * 2, 256) + round_up((size_t)(E_loc + 1) * 4, 256) + kProfileFlushBytes;
     }
     case VIBE_WS_LAYER: return layer_arena(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_FP8: return layer_arena_fp8(T, k, E_loc, d, f).total;

@@ -15,7 +15,10 @@ namespace vibe {
 void set_error(const char* fmt, ...);
 void clear_error();
 void count_launch(int n = 1);
-int num_sms();
+int num_sms();            // of the current device
+constexpr int kMaxDevices = 64;
+constexpr size_t kProfileFlushBytes = (size_t)256 << 20;   // L2 flush region at the END of a VIBE_WS_PROFILE workspace (2 x the 126 MB L2)
+int current_device();     // ordinal in [0, kMaxDevices)
 
 #define VIBE_REQUIRE(cond, status, ...)         \
   do {                                          \
@@ -67,6 +70,7 @@ vibe_status grouped_ffn_mxfp8_impl(const void* Xq, const void* xsf, const int32_
 // a 16-byte row pitch (a TMA global stride; the kernel only fetches boxes of 4 row blocks that start on a multiple of 4,
 // so a box is entirely inside or entirely outside the tensor)
 static inline int mx_row_blocks(int R_cap) { return (((R_cap + 31) / 32) + 3) & ~3; }
+vibe_status grouped_ffn_limits(const char* who, int E_loc, int d, int f, const void* W1, const void* W3, const void* W2);
 vibe_status grouped_ffn_check(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                               const void* W1, const void* W3, const void* W2, void* H_ws, void* Y);
 

@@ -541,17 +541,19 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   if ((s = get_tensor_map(W1, f, d, E_loc, 64, BK, &tmW1)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W3, f, d, E_loc, 64, BK, &tmW3)) != VIBE_OK) return s;
   if ((s = get_tensor_map(W2, d, f, E_loc, 64, BK, &tmW2)) != VIBE_OK) return s;
-  static std::once_flag once;
-  static cudaError_t attr_err = cudaSuccess;
-  std::call_once(once, [] {
-    attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
-    if (attr_err == cudaSuccess)
-      attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
-    if (attr_err == cudaSuccess)
-      attr_err = cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES);
-  });
-  VIBE_REQUIRE(attr_err == cudaSuccess, VIBE_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s",
-               SMEM_BYTES, cudaGetErrorString(attr_err));
+  {
+    // the opt-in to > 48 KB of dynamic shared memory is per device: once for each device this process uses
+    static std::mutex mu;
+    static bool done[kMaxDevices] = {};
+    const int dev = current_device();
+    std::lock_guard<std::mutex> lk(mu);
+    if (!done[dev]) {
+      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+      done[dev] = true;
+    }
+  }
   const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
   // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
   const int32_t* no_map = nullptr;
@@ -568,6 +570,16 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
                     E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, no_map, no_w);
   VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
+  return VIBE_OK;
+}
+
+// the shape / alignment limits of the FFN kernels, checkable before anything is enqueued (the layer entry points
+// call this first: "argument errors are detected before any launch")
+vibe_status grouped_ffn_limits(const char* who, int E_loc, int d, int f, const void* W1, const void* W3, const void* W2) {
+  VIBE_REQUIRE(W1 && W3 && W2, VIBE_ERR_INVALID_ARG, "%s: NULL weight tensor", who);
+  VIBE_REQUIRE(d % 64 == 0 && f % 64 == 0, VIBE_ERR_UNSUPPORTED, "%s: d and f must be multiples of 64 (d=%d f=%d)", who, d, f);
+  VIBE_REQUIRE(E_loc <= MAX_SLOTS, VIBE_ERR_UNSUPPORTED, "%s: E_loc > %d not implemented", who, MAX_SLOTS);
+  VIBE_REQUIRE(aligned16(W1) && aligned16(W3) && aligned16(W2), VIBE_ERR_INVALID_ARG, "%s: weight tensors must be 16-byte aligned", who);
   return VIBE_OK;
 }
 

@@ -593,10 +593,8 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
 // the opt-in to > 48 KB of dynamic shared memory is per device: done once for each device this process uses
 vibe_status set_smem_attrs() {
   static std::mutex mu;
-  static bool done[64] = {};
-  int dev = 0;
-  VIBE_CUDA(cudaGetDevice(&dev));
-  VIBE_REQUIRE(dev >= 0 && dev < 64, VIBE_ERR_CUDA, "device ordinal %d", dev);
+  static bool done[kMaxDevices] = {};
+  const int dev = current_device();
   std::lock_guard<std::mutex> lk(mu);
   if (done[dev]) return VIBE_OK;
   VIBE_CUDA(cudaFuncSetAttribute(ffn8_gemm_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));

@@ -16,6 +16,12 @@ extern "C" vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg, const f
   VIBE_REQUIRE(T >= 0 && d >= 8 && f >= 8 && E_loc >= 1, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward: bad sizes");
   const int E = cfg->num_experts, k = cfg->top_k;
   VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward: need 1 <= k <= E");
+  {
+    vibe_status lim = grouped_ffn_limits("vibe_moe_layer_forward", E_loc, d, f, W1, W3, W2);   // before any launch
+    if (lim != VIBE_OK) return lim;
+  }
+  VIBE_REQUIRE(out != nullptr && counts != nullptr && logits != nullptr && (T == 0 || X != nullptr), VIBE_ERR_INVALID_ARG,
+               "vibe_moe_layer_forward: NULL tensor");
   const LayerArena a = layer_arena(T, k, E_loc, d, f);
   VIBE_REQUIRE(arena != nullptr && arena_bytes >= a.total && (reinterpret_cast<uintptr_t>(arena) & 255u) == 0,
                VIBE_ERR_WORKSPACE, "vibe_moe_layer_forward: arena needs %zu bytes, 256-byte aligned (got %zu)", a.total,
@@ -125,6 +131,10 @@ extern "C" vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg*
                "vibe_moe_layer_forward_host: n_chunks must be 0 (choose) .. %d", kMaxHostChunks);
   const int E = cfg->num_experts, k = cfg->top_k;
   VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host: need 1 <= k <= E");
+  {
+    vibe_status lim = grouped_ffn_limits("vibe_moe_layer_forward_host", E_loc, d, f, W1, W3, W2);   // before any copy / launch
+    if (lim != VIBE_OK) return lim;
+  }
   const size_t inner = vibe_workspace_bytes(VIBE_WS_LAYER, T, k, E, E_loc, d, f, 1);
   const size_t need = vibe_workspace_bytes(VIBE_WS_LAYER_HOST, T, k, E, E_loc, d, f, 1);
   VIBE_REQUIRE(arena != nullptr && arena_bytes >= need && (reinterpret_cast<uintptr_t>(arena) & 255u) == 0,
@@ -179,7 +189,13 @@ extern "C" vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg*
     s = vibe_moe_layer_forward(cfg, logits_d + (size_t)t0 * E, X_d + (size_t)t0 * d * 2, expert_map, tn, d, f, E_loc, W1,
                                W3, W2, out_d + (size_t)t0 * d * 2, count_parts + (size_t)c * E, nullptr, nullptr, arena,
                                inner, stream);
-    if (s != VIBE_OK) return s;
+    if (s != VIBE_OK) {
+      // copies of this and earlier chunks may still be in flight: the host buffers must be quiet when we return
+      cudaStreamSynchronize(hp->in);
+      cudaStreamSynchronize(st);
+      cudaStreamSynchronize(hp->out);
+      return s;
+    }
     VIBE_CUDA(cudaEventRecord(hp->comp_done[c], st));
     VIBE_CUDA(cudaStreamWaitEvent(hp->out, hp->comp_done[c], 0));
     VIBE_CUDA(cudaMemcpyAsync(outh + (size_t)t0 * d * 2, out_d + (size_t)t0 * d * 2, (size_t)tn * d * 2,
@@ -217,6 +233,10 @@ extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, con
                "vibe_moe_layer_forward_fp8: d and f must be multiples of 128 (d=%d f=%d)", d, f);
   const int E = cfg->num_experts, k = cfg->top_k;
   VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_fp8: need 1 <= k <= E");
+  VIBE_REQUIRE(E_loc <= 512, VIBE_ERR_UNSUPPORTED, "vibe_moe_layer_forward_fp8: E_loc > 512 not implemented");
+  VIBE_REQUIRE(W1q && s1 && W3q && s3 && W2q && s2 && h_scale && aligned16(W1q) && aligned16(W3q) && aligned16(W2q) && out &&
+                   counts && logits,
+               VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_fp8: NULL or misaligned tensor");
   const LayerArenaFp8 a = layer_arena_fp8(T, k, E_loc, d, f);
   VIBE_REQUIRE(arena != nullptr && arena_bytes >= a.total && (reinterpret_cast<uintptr_t>(arena) & 255u) == 0,
                VIBE_ERR_WORKSPACE, "vibe_moe_layer_forward_fp8: arena needs %zu bytes, 256-byte aligned (got %zu)",

@@ -370,10 +370,11 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   const int warps = G * kIdxWarps;
   int WCH = (((A + warps - 1) / warps) + 31) / 32 * 32;
   const size_t smem1 = (size_t)((kIdxWarps + 3) * E_loc + 1 + 2 * kIdxThreads) * sizeof(int);
-  static std::atomic<size_t> smem_set{0};
-  if (smem1 > 48 * 1024 && smem1 > smem_set.load()) {
+  static std::atomic<size_t> smem_set[kMaxDevices];   // per device: the opt-in above 48 KB is a per-device attribute
+  std::atomic<size_t>& set = smem_set[current_device()];
+  if (smem1 > 48 * 1024 && smem1 > set.load()) {
     VIBE_CUDA(cudaFuncSetAttribute(perm_index_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
-    smem_set.store(smem1);
+    set.store(smem1);
   }
   __nv_bfloat16* Xpb = reinterpret_cast<__nv_bfloat16*>(Xp);
   int32_t* tbl = reinterpret_cast<int32_t*>(ws);

@@ -19,6 +19,22 @@ __global__ void fill_pattern_kernel(__nv_bfloat16* p, size_t n) {
     p[i] = __float2bfloat16_rn(((int)(h & 0xffff) - 32768) * (1.0f / 32768.0f));
   }
 }
+// Reads `n16` 16-byte vectors with the L2 evict_last policy -- the policy the FFN kernels load their operands with.
+// A sweep of twice the L2 size therefore pushes out whatever the previous execution left there, including lines
+// that a plain (evict_normal) sweep would never displace.  The sum goes to `sink` so the loads are not dead.
+__global__ void __launch_bounds__(256) l2_flush_kernel(const uint4* __restrict__ p, size_t n16, uint32_t* __restrict__ sink) {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  uint32_t acc = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x) {
+    uint4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p + i), "l"(pol));
+    acc ^= v.x ^ v.y ^ v.z ^ v.w;
+  }
+  if (acc == 0x9e3779b9u) *sink = acc;     // practically never: keeps the loads alive without a store per thread
+}
 __global__ void fill_ones_kernel(float* p, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 1.0f;
 }
@@ -33,9 +49,13 @@ namespace {
 // launches with 640 bytes of parameters: ~6 us, more than a lone small expert takes on the device).  Everything
 // runs on a stream of the sweep's own, after the caller's stream has drained: the legacy default stream cannot be
 // captured.  If the capture fails the calls are timed one by one as launched.
+// Every timed execution starts COLD: before its first event an evict_last read sweep of kProfileFlushBytes (twice the
+// 126 MB L2) runs on the same stream, outside the event pair.  Without it a sweep point whose operands fit the L2
+// (a lone C3 expert: 88 MB of weights; the C2 shape: 9 MB per expert) would be replayed on L2-resident weights and
+// read faster than it ever does inside a model, where the other layers' traffic has evicted them.
 template <class Run>
 vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_points, int mode, int warmup, int iters,
-                          float* latency_us, float* samples_us, int32_t* offsets, cudaStream_t caller, Run run) {
+                          float* latency_us, float* samples_us, int32_t* offsets, void* flush, cudaStream_t caller, Run run) {
   VIBE_CUDA(cudaStreamSynchronize(caller));
   cudaStream_t st = nullptr;
   VIBE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
@@ -71,6 +91,9 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
     }
     (void)cudaGetLastError();      // a failed capture leaves a sticky-free error behind; the fallback below still works
     for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
+      l2_flush_kernel<<<num_sms() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(flush), kProfileFlushBytes / 16,
+                                                     reinterpret_cast<uint32_t*>(flush));
+      count_launch();
       cudaEventRecord(ev[2 * i], st);
       if (exec) {
         if (cudaGraphLaunch(exec, st) != cudaSuccess) {
@@ -138,13 +161,15 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
   void* H = base + 2 * round_up((size_t)R_cap * d * 2, 256);
   int32_t* offsets = reinterpret_cast<int32_t*>(base + 2 * round_up((size_t)R_cap * d * 2, 256) +
                                                 round_up((size_t)R_cap * f * 2, 256));
+  void* flush = base + need - kProfileFlushBytes;
   vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y);
   if (s != VIBE_OK) return s;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   fill_pattern_kernel<<<num_sms() * 4, 256, 0, st>>>(reinterpret_cast<__nv_bfloat16*>(Xp), (size_t)R_cap * d);
   VIBE_LAUNCH_CHECK("fill_pattern_kernel");
 
-  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st,
+  VIBE_CUDA(cudaMemsetAsync(flush, 0, kProfileFlushBytes, st));
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st,
                        [&](cudaStream_t ps) { return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, ps); });
 }
 
@@ -185,12 +210,14 @@ extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d,
   void* Hq = Hreg;
   int32_t* offsets = reinterpret_cast<int32_t*>(Hreg + round_up((size_t)R_cap * f * 2, 256));
   float* row_scale = reinterpret_cast<float*>(base + base_need);
+  void* flush = base + base_need - kProfileFlushBytes;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   // arbitrary finite codes (0x38 = 1.0) and unit row scales: latency does not depend on the values
   VIBE_CUDA(cudaMemsetAsync(Xq, 0x38, (size_t)R_cap * d, st));
   fill_ones_kernel<<<num_sms() * 2, 256, 0, st>>>(row_scale, (size_t)R_cap);
   VIBE_LAUNCH_CHECK("fill_ones_kernel");
-  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, st, [&](cudaStream_t ps) {
+  VIBE_CUDA(cudaMemsetAsync(flush, 0, kProfileFlushBytes, st));
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st, [&](cudaStream_t ps) {
     return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, ps);
   });
 }

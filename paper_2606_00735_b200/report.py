@@ -521,10 +521,18 @@ def section_rack(peaks, quick, profile):
     rc = B.RouteConfig(num_experts=E, top_k=k)
     lg = torch.from_numpy(I.make_logits(16384, E, 1.2, 7, 1.0)).cuda()
     load = B.route_topk(lg, rc)[2].cpu().numpy().astype(np.float64)
+    return rack_sweep(load, model, E, (8, 16, 32, 64, 128), range(4 if quick else 16))
+
+
+def rack_sweep(load, model, E, Gs, seeds):
+    """The evaluator sweep behind the rack-scale projection (host only: placement calls of the C ABI): for every G,
+    sigma_g resampled per seed (inputs.make_throughput_scales(G, 100 + seed)), cap = E/G, model B; gain of the
+    latency-balanced greedy over the token-balanced one and over contiguous placement, and max/mean bin latency of
+    the latency-balanced placement.  tests/test_report_host.py pins it against the oracle's placement functions."""
     out = []
-    for G in (8, 16, 32, 64, 128):
+    for G in Gs:
         gains_t, gains_c, ratio = [], [], []
-        for seed in range(4 if quick else 16):
+        for seed in seeds:
             scale = I.make_throughput_scales(G, 100 + seed)
             cap = E // G
             tb = B.placement_token_balanced(load, G, cap)

@@ -444,16 +444,20 @@ def test_profile_expert_latency_sanity():
     cfg = I.scaled(I.C2, E=16, E_loc=16)
     W1, W3, W2 = (dev_bf16(x) for x in I.make_weights(cfg.E_loc, cfg.d, cfg.f, 0))
     sweep = [1, 16, 128, 512, 2048]
-    lat, samples = B.profile_expert_latency(W1, W3, W2, sweep, mode=0, warmup=3, iters=15, return_samples=True)
-    assert lat.shape == (5,) and samples.shape == (5, 15)
+    lat, samples = B.profile_expert_latency(W1, W3, W2, sweep, mode=0, warmup=3, iters=41, return_samples=True)
+    assert lat.shape == (5,) and samples.shape == (5, 41)
     assert np.all(lat > 0) and np.all(np.isfinite(lat))
-    # non-decreasing (within 20 %: the flat weight-streaming region is a timing of ~20 us kernels) and
-    # large-n cost per token well below small-n cost per token
-    assert np.all(lat[1:] >= lat[:-1] * 0.8), lat
+    # non-decreasing within 10 % (the flat weight-streaming region is a timing of ~25 us kernels; the median of 41
+    # cold executions is stable to a few percent) and large-n cost per token well below small-n cost per token
+    assert np.all(lat[1:] >= lat[:-1] * 0.9), lat
     assert lat[-1] / 2048 < lat[0] / 1
     # flop floor at the nominal dense bf16 peak (2.25 PFLOP/s): cannot be faster than that
     flops = 6.0 * 2048 * cfg.d * cfg.f
     assert lat[-1] * 1e-6 >= flops / 2.25e15
+    # weight-stream floor (S8(c) a6): every timed execution starts with a flushed L2, so an expert's 6 d f bytes of
+    # weights come from HBM each time.  The allowance: a read-only stream may beat the measured COPY peak (6.5 TB/s
+    # counts read + write), so the floor is taken at HBM3e's nominal 8 TB/s, which nothing can exceed.
+    assert np.all(lat * 1e-6 >= 6.0 * cfg.d * cfg.f / 8.0e12), lat
     solo = B.profile_expert_latency(W1, W3, W2, [128], mode=1, warmup=2, iters=5)
     assert solo[0] > 0
 

@@ -32,3 +32,40 @@ def test_write_markdown_with_partial_and_full_sections(tmp_path):
     for needle in ("## stages", "## ffn_balanced", "## ffn_mixed", "## fused_scatter", "## layer", "## profile", "## rack_projection"):
         assert needle in text
     assert os.path.getsize(p) > 500
+
+
+def test_rack_projection_sweep_against_the_oracle():
+    """P:L337-L347 (Fig. 15): the rack-scale projection is an evaluator sweep over G.  report.rack_sweep (C-ABI
+    placement calls) against the same sweep written with the oracle's placement functions, G = 8, 32, 128."""
+    import numpy as np
+    from oracle import vibe_oracle as O
+    from paper_2606_00735_b200 import binding as B
+    from paper_2606_00735_b200 import inputs as I
+    E, k, T = 256, 8, 512
+    kw = dict(num_experts=E, top_k=k)
+    load = O.route_topk(I.make_logits(T, E, 1.2, 7, 1.0), **kw)[2].astype(np.float64)
+    tokens = [1.0, 8.0, 64.0, 512.0, 4096.0]
+    lat = [13.0, 13.2, 14.5, 40.0, 300.0]                       # a weight-streaming floor, then linear growth
+    Gs, seeds = (8, 32, 128), range(3)
+    got = report.rack_sweep(load, B.LatencyModel(tokens, lat, 32), E, Gs, seeds)
+    om = O.LatencyModel(tokens, lat, 32)
+    for row, G in zip(got, Gs):
+        gt, gc, ratio = [], [], []
+        for seed in seeds:
+            scale = I.make_throughput_scales(G, 100 + seed)
+            cap = E // G
+            tb = O.placement_token_balanced(load, G, cap)
+            lb = O.placement_greedy(load, G, scale, om, cap)
+            ct = O.placement_contiguous(E, G)
+            s_tb = O.placement_eval(tb, load, G, scale, om, O.MODEL_B)[0]
+            s_lb, per = O.placement_eval(lb, load, G, scale, om, O.MODEL_B)
+            s_ct = O.placement_eval(ct, load, G, scale, om, O.MODEL_B)[0]
+            gt.append(1.0 - s_lb / s_tb); gc.append(1.0 - s_lb / s_ct); ratio.append(s_lb / float(np.mean(per)))
+        assert row["G"] == G and row["experts_per_gpu"] == E // G
+        assert row["gain_latency_vs_token_median"] == round(float(np.median(gt)), 4)
+        assert row["gain_latency_vs_token_min"] == round(float(min(gt)), 4)
+        assert row["gain_latency_vs_token_max"] == round(float(max(gt)), 4)
+        assert row["gain_latency_vs_contiguous_median"] == round(float(np.median(gc)), 4)
+        assert row["latency_balanced_max_over_mean_median"] == round(float(np.median(ratio)), 4)
+    # the paper's qualitative claim: with fewer experts per GPU the straggler dominates whatever the policy
+    assert got[-1]["latency_balanced_max_over_mean_median"] > got[0]["latency_balanced_max_over_mean_median"]
