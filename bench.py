@@ -237,6 +237,7 @@ def main():
     a2r = torch.empty((A,), dtype=torch.int32, device=dev)
     out = torch.empty((T, d), dtype=torch.bfloat16, device=dev)
     pws = torch.empty((max(16, B.workspace_bytes(B.WS_PERMUTE, T, k, E, E_loc, d, f)),), dtype=torch.uint8, device=dev)
+    fws = torch.empty((max(16, B.workspace_bytes(B.WS_FFN, T, k, E, E_loc, d, f)),), dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
 
     def step(i, ev=None):
@@ -249,7 +250,7 @@ def main():
         B.permute(Xd, ids, counts, emap, E, E_loc, 1, out=(Xp, off, r2a, a2r), ws=pws, stream=stream)
         if ev:
             ev[2].record(stream)
-        B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y, stream=stream)
+        B.grouped_ffn(Xp, off, W1, W3, W2, H=H, Y=Y, stream=stream, ws=fws)
         if ev:
             ev[3].record(stream)
         B.combine(Y, a2r, gw, T, k, out=out, stream=stream)

@@ -134,7 +134,12 @@ VIBE_API vibe_status vibe_permute(const void* X, const int32_t* topk_ids, const 
  * in place (no repacking).  H_ws [R_cap,f] bf16 scratch; Y [R_cap,d] bf16.
  * Shape limits of the tcgen05 kernels: d % 64 == 0, f % 64 == 0, all base pointers
  * 16-byte aligned (TMA), R_cap >= 1.  Rows >= offsets[E_loc] of H_ws / Y are not written.
- * ws: vibe_workspace_bytes(VIBE_WS_FFN, ...) bytes (may be 0 -> ws may be NULL).
+ * ws: vibe_workspace_bytes(VIBE_WS_FFN, ...) bytes, 16-byte aligned, or NULL.  It holds the fp32 partial sums and the
+ *     arrival counters of the SPLIT-K path: when a launch has at most half as many tiles as the GPU
+ *     has CTA pairs -- a lone or a few light experts, the decode regime P:L108 / L130 calls low-intensity -- every
+ *     tile's K range is cut over several pairs and reduced in fp32 in a fixed order.  With ws = NULL (or too small)
+ *     the call is still correct; such launches then stream their weights on as many SM pairs as they have tiles.
+ *     Calls that may run concurrently must use different workspaces.
  * ---------------------------------------------------------------------------------- */
 VIBE_API vibe_status vibe_grouped_ffn(const void* Xp, const int32_t* offsets, int32_t E_loc, int32_t R_cap,
                                       int32_t d, int32_t f, const void* W1, const void* W3, const void* W2,
@@ -270,6 +275,12 @@ VIBE_API vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int32
                                                  int32_t mode, int32_t warmup, int32_t iters,
                                                  float* latency_us /*host*/, float* samples_us /*host|NULL*/,
                                                  void* ws, size_t ws_bytes, void* stream);
+
+/* Measurement utility (the protocol of a6, for callers that time kernels themselves): reads `bytes` of `scratch`
+ * (device, 16-byte aligned; use >= 2 x the L2 size, 256 MB on B200) with the L2 evict_last policy, which evicts
+ * what earlier kernels left in L2 -- including the evict_last operand lines of the FFN kernels that a plain memset
+ * would not displace.  Asynchronous on `stream`; the buffer's contents are not changed. */
+VIBE_API vibe_status vibe_l2_flush(void* scratch, size_t bytes, void* stream);
 
 /* a6 in the paper's precision (f2): the same profile of vibe_grouped_ffn_fp8 (packed weights and scales as there).
  * ws: vibe_workspace_bytes(VIBE_WS_PROFILE, T = max tokens_per_expert, ...) rounded up to 256, plus

@@ -41,7 +41,7 @@ EXPORTED_SYMBOLS = (
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
     "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward_host_chunked",
-    "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
+    "vibe_l2_flush", "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
     "vibe_moe_layer_forward_mxfp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
@@ -124,6 +124,8 @@ def load() -> C.CDLL:
                                                         vp, vp, vp, i32, vp, sz, vp]
     lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                                vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_l2_flush.argtypes = [vp, sz, vp]
+    lib.vibe_l2_flush.restype = C.c_int
     lib.vibe_mxfp8_sf_bytes.argtypes = [i32] * 4
     lib.vibe_mxfp8_sf_bytes.restype = sz
     lib.vibe_mxfp8_quantize_rows.argtypes = [vp, i32, i32, i32, vp, vp, i32, i32, vp]
@@ -201,6 +203,11 @@ def _scratch(nbytes: int, device, stream) -> torch.Tensor:
         return torch.empty((max(nbytes, 16),), dtype=torch.uint8, device=device)
 
 
+def l2_flush(scratch: torch.Tensor, stream=None) -> None:
+    """evict the L2 before a timed region (scratch: a uint8 CUDA tensor of >= 2 x the L2 size)"""
+    _ok(load().vibe_l2_flush(scratch.data_ptr(), scratch.numel(), _stream(stream)), "vibe_l2_flush")
+
+
 def launch_count() -> int:
     return int(load().vibe_launch_count())
 
@@ -264,8 +271,9 @@ def permute(X: torch.Tensor, topk_ids: torch.Tensor, counts: Optional[torch.Tens
 
 # ------------------------------------------------------------------------------------ a4
 def grouped_ffn(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: torch.Tensor, W2: torch.Tensor,
-                H: Optional[torch.Tensor] = None, Y: Optional[torch.Tensor] = None, stream=None):
-    """-> Y bf16 [R_cap,d]  (H bf16 [R_cap,f] scratch is returned too)"""
+                H: Optional[torch.Tensor] = None, Y: Optional[torch.Tensor] = None, stream=None, ws="auto"):
+    """-> Y bf16 [R_cap,d]  (H bf16 [R_cap,f] scratch is returned too).  ws: split-K workspace (WS_FFN bytes);
+    "auto" allocates one for the call, None runs without (no split-K)."""
     lib = load()
     for t, n in ((Xp, "Xp"), (W1, "W1"), (W3, "W3"), (W2, "W2")):
         _check(t, torch.bfloat16, n)
@@ -280,14 +288,17 @@ def grouped_ffn(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: t
         H = torch.empty((Rcap, f), dtype=torch.bfloat16, device=Xp.device)
     if Y is None:
         Y = torch.empty((Rcap, d), dtype=torch.bfloat16, device=Xp.device)
+    if isinstance(ws, str):
+        ws = _scratch(workspace_bytes(WS_FFN, 1, 1, 1, E_loc, d, f, 1), Xp.device, stream)
     _ok(lib.vibe_grouped_ffn(Xp.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1.data_ptr(), W3.data_ptr(),
-                             W2.data_ptr(), H.data_ptr(), Y.data_ptr(), None, 0, _stream(stream)), "vibe_grouped_ffn")
+                             W2.data_ptr(), H.data_ptr(), Y.data_ptr(), ws.data_ptr() if ws is not None else None,
+                             ws.numel() if ws is not None else 0, _stream(stream)), "vibe_grouped_ffn")
     return Y, H
 
 
 def grouped_ffn_scatter(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tensor, W3: torch.Tensor,
                         W2: torch.Tensor, row_to_assign: torch.Tensor, topk_w: torch.Tensor,
-                        H: Optional[torch.Tensor] = None, Yw: Optional[torch.Tensor] = None, stream=None):
+                        H: Optional[torch.Tensor] = None, Yw: Optional[torch.Tensor] = None, stream=None, ws="auto"):
     """-> Yw bf16 [T*k, d] in assignment order, gate-weighted (rows of non-resident assignments untouched)"""
     lib = load()
     for t, n in ((Xp, "Xp"), (W1, "W1"), (W3, "W3"), (W2, "W2")):
@@ -303,9 +314,12 @@ def grouped_ffn_scatter(Xp: torch.Tensor, offsets: torch.Tensor, W1: torch.Tenso
         H = torch.empty((Rcap, f), dtype=torch.bfloat16, device=Xp.device)
     if Yw is None:
         Yw = torch.empty((topk_w.numel(), d), dtype=torch.bfloat16, device=Xp.device)
+    if isinstance(ws, str):
+        ws = _scratch(workspace_bytes(WS_FFN, 1, 1, 1, E_loc, d, f, 1), Xp.device, stream)
     _ok(lib.vibe_grouped_ffn_scatter(Xp.data_ptr(), offsets.data_ptr(), E_loc, Rcap, d, f, W1.data_ptr(),
                                      W3.data_ptr(), W2.data_ptr(), row_to_assign.data_ptr(), topk_w.data_ptr(),
-                                     H.data_ptr(), Yw.data_ptr(), None, 0, _stream(stream)),
+                                     H.data_ptr(), Yw.data_ptr(), ws.data_ptr() if ws is not None else None,
+                                     ws.numel() if ws is not None else 0, _stream(stream)),
         "vibe_grouped_ffn_scatter")
     return Yw, H
 

@@ -57,6 +57,7 @@ LayerArena layer_arena(int T, int k, int E_loc, int d, int f) {
   a.H = take((size_t)a.R_cap * f * 2);
   a.Y = take((size_t)a.R_cap * d * 2);
   a.perm_ws = take(permute_ws_bytes(T, k, E_loc));
+  a.ffn_ws = take(grouped_ffn_ws_bytes());
   a.total = o;
   return a;
 }
@@ -140,10 +141,11 @@ extern "C" size_t vibe_workspace_bytes(int32_t which, int32_t T, int32_t k, int3
   if (T < 0 || k < 1 || E < 1 || E_loc < 1 || d < 0 || f < 0) return 0;
   switch (which) {
     case VIBE_WS_PERMUTE: return permute_ws_bytes(T, k, E_loc);
-    case VIBE_WS_FFN: return 0;
+    case VIBE_WS_FFN: return grouped_ffn_ws_bytes();
     case VIBE_WS_PROFILE: {
       const size_t R = (size_t)E_loc * (size_t)(T > 0 ? T : 1);
-      return round_up(R * d * 2, 256) * 2 + round_up(R * f * 2, 256) + round_up((size_t)(E_loc + 1) * 4, 256) + kProfileFlushBytes;
+      return round_up(R * d * 2, 256) * 2 + round_up(R * f * 2, 256) + round_up((size_t)(E_loc + 1) * 4, 256) +
+             round_up(grouped_ffn_ws_bytes(), 256) + kProfileFlushBytes;
     }
     case VIBE_WS_LAYER: return layer_arena(T, k, E_loc, d, f).total;
     case VIBE_WS_LAYER_FP8: return layer_arena_fp8(T, k, E_loc, d, f).total;

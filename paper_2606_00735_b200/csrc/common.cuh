@@ -51,14 +51,17 @@ int current_device();     // ordinal in [0, kMaxDevices)
 
 // ---- internal cross-file declarations -------------------------------------------------
 struct LayerArena {
-  size_t ids, w, offsets, r2a, a2r, Xp, H, Y, perm_ws, total;
+  size_t ids, w, offsets, r2a, a2r, Xp, H, Y, perm_ws, ffn_ws, total;
   int64_t R_cap;
 };
 LayerArena layer_arena(int T, int k, int E_loc, int d, int f);
 size_t permute_ws_bytes(int T, int k, int E_loc);
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y, cudaStream_t st,
-                             const int32_t* row_to_assign = nullptr, const float* topk_w = nullptr);
+                             const int32_t* row_to_assign = nullptr, const float* topk_w = nullptr, void* ws = nullptr,
+                             size_t ws_bytes = 0, bool ws_zeroed = false);
+size_t grouped_ffn_ws_bytes();   // split-K partial buffer + counters (VIBE_WS_FFN)
+vibe_status grouped_ffn_zero_counters(void* ws, cudaStream_t st);   // what ws_zeroed = true promises
 vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const int32_t* offsets, int E_loc, int R_cap,
                                  int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
                                  const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,

@@ -39,6 +39,14 @@
 // Epilogue: tcgen05.ld 32 lanes x 32 columns, bf16x2 pack + one shuffle + byte permute per token
 // pair (the output is the TRANSPOSE of the accumulator), 4-byte stores of two adjacent features.
 //
+// Split-K (S8(f) f4, the few-active-experts regime): when the launch has at most half as many tiles as the grid has
+// CTA pairs (a lone expert of a decode step: 16 / 28 tiles for 74 pairs, each pair limited to ~140 GB/s of weight
+// streaming), every tile's K range is cut into S = min(pairs / tiles, 8, K steps / 4) slices, one (tile, slice) unit
+// per pair.  A unit dumps its fp32 accumulator to the caller's workspace; the LAST unit of a tile portion to
+// arrive (one counter per tile, CTA rank and epilogue warp role) sums the S partials in slice order -- a fixed
+// order, so the result does not depend on which unit came last -- and runs the normal epilogue on the sum.
+// S is derived on the device from `offsets`, like everything else.
+//
 // Semantics: include/vibe.h (vibe_grouped_ffn); F1-F4.
 #include <mutex>
 #include <unordered_map>
@@ -69,6 +77,13 @@ constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 
 __host__ __device__ constexpr int num_threads(int mode) { return mode == 0 ? 192 : 320; }
 constexpr int MAX_SLOTS = 512;
 constexpr int TMEM_COLS = 512;
+// split-K workspace: partial accumulators [unit][column][256 features of the pair tile] fp32, then the counters
+constexpr int SPLIT_MAX = 8;               // K slices per tile at most
+constexpr int SPLIT_MIN_STEPS = 4;         // K steps per slice at least
+constexpr int SPLIT_MAX_UNITS = 128;       // >= CTA pairs of any supported device (B200: 74)
+constexpr size_t SPLIT_PART_BYTES = (size_t)SPLIT_MAX_UNITS * TN * 256 * sizeof(float);
+constexpr int SPLIT_COUNTERS = SPLIT_MAX_UNITS * 16;     // per tile: 2 CTA ranks x 8 epilogue-warp roles
+constexpr size_t SPLIT_WS_BYTES = SPLIT_PART_BYTES + 2 * (size_t)SPLIT_COUNTERS * sizeof(int);   // counters of GEMM-1, of GEMM-2
 
 struct SmemTail {
   uint64_t full[STAGES];          // leader CTA: both CTAs' TMA bytes of a stage have landed
@@ -77,6 +92,7 @@ struct SmemTail {
   uint64_t tempty[2];             // leader CTA: all 8 epilogue warps of the pair drained it
   uint32_t tmem_base;
   int32_t total_t_tiles;
+  int32_t split;                  // K slices per tile (1 = no split-K)
   int32_t off[MAX_SLOTS + 1];     // segment starts (rows)
   int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
   int32_t tsz[MAX_SLOTS];         // rows per token tile of the slot (multiple of 16, <= TN)
@@ -169,7 +185,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmActN,
                 const __grid_constant__ CUtensorMap tmW0, const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
                 int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out,
-                const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w) {
+                const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w,
+                float* __restrict__ split_part /*NULL: no split-K*/, int* __restrict__ split_cnt) {
   constexpr bool kGateUp = (kMode == 0);
   constexpr int FB = kGateUp ? 128 : 256;   // output features per pair tile
   constexpr int FC = FB / 2;                // ... per CTA
@@ -235,6 +252,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       tail->cum[E_loc] = carry;
       tail->off[E_loc] = offsets[E_loc];
       tail->total_t_tiles = carry;
+      int S = 1;
+      const int total = carry * NB;
+      if (split_part != nullptr && total > 0 && 2 * total <= num_pairs && num_pairs <= SPLIT_MAX_UNITS)
+        S = max(1, min(min(num_pairs / total, SPLIT_MAX), KB / SPLIT_MIN_STEPS));
+      tail->split = S;
     }
   }
   if (warp != 2) ptx::griddep_wait();
@@ -244,7 +266,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   ptx::tc_fence_after();
 
   const uint32_t tmem_base = tail->tmem_base;
-  const int total_tiles = tail->total_t_tiles * NB;
+  const int S = tail->split;                               // K slices per tile
+  const int total_units = tail->total_t_tiles * NB * S;    // a unit = (tile, K slice); S = 1: a unit is a tile
 
   if (warp == 0) {
     // ================================================================ TMA producer (both CTAs)
@@ -263,8 +286,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
-      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, tile = tile_of(rnd, pair, num_pairs)) {
+      for (int rnd = 0, unit = pair; unit < total_units; ++rnd, unit = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
+        const int tile = unit / S, slice = unit - tile * S;
+        const int kb_lo = slice * KB / S, kb_hi = (slice + 1) * KB / S;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
         const int tsz = tail->tsz[e];
@@ -277,7 +302,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         const bool narrow = half <= NARROW_ROWS;
         const CUtensorMap* tm_b = narrow ? &tmActN : &tmAct;
         const uint32_t tx_bytes = narrow ? 2u * (A_BYTES + NARROW_ROWS * BK * 2) : 2u * STAGE_BYTES;
-        for (int kb = 0; kb < KB; ++kb) {
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
           if (ptx::elect_one()) {
             if (rank == 0) ptx::mbar_arrive_expect_tx(ptx::smem_u32(&tail->full[stage]), tx_bytes);
@@ -314,8 +339,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
+      for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
+        const int tile = unit / S, slice = unit - tile * S;
+        const int kb_lo = slice * KB / S, kb_hi = (slice + 1) * KB / S;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
         const int tsz = tail->tsz[e];
@@ -327,7 +354,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         ptx::mbar_wait(ptx::smem_u32(&tail->tempty[acc]), acc_phase ^ 1u);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)acc * TN;
-        for (int kb = 0; kb < KB; ++kb) {
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->full[stage]), phase);
           ptx::tc_fence_after();
           if (ptx::elect_one()) {
@@ -339,10 +366,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
             for (int k = 0; k < BK / UMMA_K; ++k) {
               const uint64_t da = ((uint64_t)DESC_HI << 32) | (uint64_t)(a_lo + (uint32_t)k * (UMMA_K * 128 / 16));
               const uint64_t db = ((uint64_t)DESC_HI << 32) | (uint64_t)(b_lo + (uint32_t)k * (UMMA_K * 2 / 16));
-              ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb | k) != 0));
+              ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb > kb_lo) | (k != 0)));
             }
             ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
-            if (kb == KB - 1)
+            if (kb == kb_hi - 1)
               ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->tfull[acc]), 3);   // accumulator ready in both CTAs
           }
           __syncwarp();
@@ -356,8 +383,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     const int blk_par = (warp - 2) >> 2;   // down projection: which 32-column blocks (even / odd) are mine
     TileCursor cur;
     int it = 0;
-    for (int rnd = 0, tile = pair; tile < total_tiles; ++rnd, ++it, tile = tile_of(rnd, pair, num_pairs)) {
+    for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
       int f_blk, t_blk;
+      const int tile = unit / S;
       cur.decode(tail, tile, NB, f_blk, t_blk);
       const int e = cur.e;
       const int tsz = tail->tsz[e];
@@ -383,6 +411,79 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
+      if (S > 1) {
+        // ------------------------------------------------------------ split-K unit
+        // (1) dump this warp's part of the fp32 accumulator: part[unit][column][rank * 128 + TMEM lane]
+        float* mypart = split_part + ((size_t)unit * TN) * 256 + rank * 128 + q * 32 + lane;
+        for (int c0 = kGateUp ? 0 : blk_par * 32; c0 < n_rows; c0 += kGateUp ? 32 : 64) {
+          uint32_t a[32];
+          ptx::tmem_ld_32x32(taddr + c0, a);
+          ptx::tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) __stcg(mypart + (size_t)(c0 + i) * 256, __uint_as_float(a[i]));
+        }
+        // the accumulator stage is free again
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa_u32(ptx::smem_u32(&tail->tempty[acc]), 0));
+        // (2) arrive on the counter of this tile portion; the last of its S (x 2: gate and up warp) arrivals finishes it
+        const int role = kGateUp ? (q & 1) : (warp - 2);
+        int* cnt = split_cnt + (tile * 2 + (int)rank) * 8 + role;
+        const int expect = kGateUp ? 2 * S : S;
+        __threadfence();
+        int last = 0;
+        if (lane == 0) {
+          last = (atomicAdd(cnt, 1) == expect - 1);
+          if (last) *cnt = 0;               // re-armed for the next call on this workspace
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (last) {
+          __threadfence();
+          // (3) sum the S partials in slice order, then the normal epilogue on the sum
+          const float* p0 = split_part + ((size_t)tile * S * TN) * 256 + rank * 128;
+          if (kGateUp) {
+            const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
+            const bool feat_ok = feat < n_total;
+            const float* pg = p0 + (q & 1) * 32 + lane;        // gate: TMEM lanes 0..63, up: the same feature + 64
+            for (int c0 = 0; c0 < n_rows; c0 += 32) {
+              // slice loop OUTSIDE, the 32 columns unrolled inside: 64 independent L2 loads in flight per slice
+              float g[32], u[32];
+#pragma unroll
+              for (int i = 0; i < 32; ++i) g[i] = u[i] = 0.0f;
+              for (int sl = 0; sl < S; ++sl) {
+                const float* pc = pg + ((size_t)sl * TN + (size_t)c0) * 256;
+#pragma unroll
+                for (int i = 0; i < 32; ++i) {
+                  g[i] += __ldcg(pc + (size_t)i * 256);
+                  u[i] += __ldcg(pc + (size_t)i * 256 + 64);
+                }
+              }
+#pragma unroll
+              for (int i = 0; i < 32; ++i) g[i] = swiglu(g[i], u[i]);
+              store_block_T(g, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+            }
+          } else {
+            const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
+            const bool feat_ok = feat < n_total;
+            const float* pv = p0 + q * 32 + lane;
+            for (int c0 = blk_par * 32; c0 < n_rows; c0 += 64) {
+              float v[32];
+#pragma unroll
+              for (int i = 0; i < 32; ++i) v[i] = 0.0f;
+              for (int sl = 0; sl < S; ++sl) {
+                const float* pc = pv + ((size_t)sl * TN + (size_t)c0) * 256;
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] += __ldcg(pc + (size_t)i * 256);
+              }
+              if (kMode == 2)
+                store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_wt + c0, sc_asg + c0);
+              else
+                store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+            }
+          }
+        }
+        continue;
+      }
       if (kGateUp) {
         // lanes 0..63 gate (q = 0,1), lanes 64..127 up (q = 2,3) of the same 64 features.
         // Per 64 columns: the gate warp finishes columns 0..31 (needs the partner's up block),
@@ -529,9 +630,19 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
 
 }  // namespace
 
+size_t grouped_ffn_ws_bytes() { return SPLIT_WS_BYTES; }
+vibe_status grouped_ffn_zero_counters(void* ws, cudaStream_t st) {
+  VIBE_CUDA(cudaMemsetAsync(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
+  return VIBE_OK;
+}
+
+// ws (may be NULL or short: split-K is then off): SPLIT_WS_BYTES bytes; ws_zeroed: the caller has already zeroed the
+// counters behind the partial buffer on this stream (the layer entry does it before the route kernel so that no
+// memset sits between the permutation and the FFN kernels, which are chained by programmatic dependent launch)
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y,
-                             cudaStream_t st, const int32_t* row_to_assign, const float* topk_w) {
+                             cudaStream_t st, const int32_t* row_to_assign, const float* topk_w, void* ws,
+                             size_t ws_bytes, bool ws_zeroed) {
   CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
   vibe_status s;
   if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
@@ -558,16 +669,25 @@ vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, 
   // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
   const int32_t* no_map = nullptr;
   const float* no_w = nullptr;
+  float* part = nullptr;
+  int* cnt1 = nullptr;
+  int* cnt2 = nullptr;
+  if (ws != nullptr && ws_bytes >= SPLIT_WS_BYTES && (reinterpret_cast<uintptr_t>(ws) & 15u) == 0) {
+    part = reinterpret_cast<float*>(ws);
+    cnt1 = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES);
+    cnt2 = cnt1 + SPLIT_COUNTERS;
+    if (!ws_zeroed) VIBE_CUDA(cudaMemsetAsync(cnt1, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
+  }
   cudaError_t le = launch_pdl(ffn_gemm_kernel<0>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
-                              offsets, E_loc, f, d, reinterpret_cast<__nv_bfloat16*>(H_ws), f, no_map, no_w);
+                              offsets, E_loc, f, d, reinterpret_cast<__nv_bfloat16*>(H_ws), f, no_map, no_w, part, cnt1);
   VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
   if (row_to_assign != nullptr)
     le = launch_pdl(ffn_gemm_kernel<2>, dim3(grid), dim3(num_threads(2)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
-                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign, topk_w);
+                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign, topk_w, part, cnt2);
   else
     le = launch_pdl(ffn_gemm_kernel<1>, dim3(grid), dim3(num_threads(1)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
-                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, no_map, no_w);
+                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, no_map, no_w, part, cnt2);
   VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
@@ -602,13 +722,11 @@ extern "C" vibe_status vibe_grouped_ffn(const void* Xp, const int32_t* offsets, 
                                         int32_t d, int32_t f, const void* W1, const void* W3, const void* W2,
                                         void* H_ws, void* Y, void* ws, size_t ws_bytes, void* stream) {
   using namespace vibe;
-  (void)ws;
-  (void)ws_bytes;
   clear_error();
   vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Y);
   if (s != VIBE_OK) return s;
   return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Y,
-                          reinterpret_cast<cudaStream_t>(stream), nullptr, nullptr);
+                          reinterpret_cast<cudaStream_t>(stream), nullptr, nullptr, ws, ws_bytes, false);
 }
 
 extern "C" vibe_status vibe_grouped_ffn_scatter(const void* Xp, const int32_t* offsets, int32_t E_loc, int32_t R_cap,
@@ -616,12 +734,10 @@ extern "C" vibe_status vibe_grouped_ffn_scatter(const void* Xp, const int32_t* o
                                                 const void* W2, const int32_t* row_to_assign, const float* topk_w,
                                                 void* H_ws, void* Yw, void* ws, size_t ws_bytes, void* stream) {
   using namespace vibe;
-  (void)ws;
-  (void)ws_bytes;
   clear_error();
   vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Yw);
   if (s != VIBE_OK) return s;
   VIBE_REQUIRE(row_to_assign && topk_w, VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_scatter: NULL row_to_assign / topk_w");
   return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Yw,
-                          reinterpret_cast<cudaStream_t>(stream), row_to_assign, topk_w);
+                          reinterpret_cast<cudaStream_t>(stream), row_to_assign, topk_w, ws, ws_bytes, false);
 }

@@ -37,13 +37,17 @@ extern "C" vibe_status vibe_moe_layer_forward(const vibe_route_cfg* cfg, const f
   void* H = base + a.H;
   void* Y = base + a.Y;
   vibe_status s;
+  // the split-K counters of the FFN are zeroed HERE, ahead of the route kernel: a memset between the permutation and
+  // the FFN kernels would cut their programmatic-dependent-launch chain
+  if (T > 0 && (s = grouped_ffn_zero_counters(base + a.ffn_ws, reinterpret_cast<cudaStream_t>(stream))) != VIBE_OK) return s;
   if ((s = vibe_route_topk(cfg, logits, T, ids, w, counts, stream)) != VIBE_OK) return s;
   if ((s = vibe_permute(X, ids, counts, expert_map, T, d, k, E, E_loc, 1, Xp, offsets, r2a, a2r, base + a.perm_ws,
                         permute_ws_bytes(T, k, E_loc), stream)) != VIBE_OK)
     return s;
   if (T == 0) return VIBE_OK;
-  if ((s = vibe_grouped_ffn(Xp, offsets, E_loc, (int32_t)a.R_cap, d, f, W1, W3, W2, H, Y, nullptr, 0, stream)) !=
-      VIBE_OK)
+  if ((s = grouped_ffn_check(Xp, offsets, E_loc, (int)a.R_cap, d, f, W1, W3, W2, H, Y)) != VIBE_OK) return s;
+  if ((s = grouped_ffn_impl(Xp, offsets, E_loc, (int)a.R_cap, d, f, W1, W3, W2, H, Y, reinterpret_cast<cudaStream_t>(stream),
+                            nullptr, nullptr, base + a.ffn_ws, grouped_ffn_ws_bytes(), true)) != VIBE_OK)
     return s;
   return vibe_combine(Y, a2r, w, T, k, d, out, stream);
 }

@@ -162,6 +162,7 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
   int32_t* offsets = reinterpret_cast<int32_t*>(base + 2 * round_up((size_t)R_cap * d * 2, 256) +
                                                 round_up((size_t)R_cap * f * 2, 256));
   void* flush = base + need - kProfileFlushBytes;
+  void* ffn_ws = base + need - kProfileFlushBytes - round_up(grouped_ffn_ws_bytes(), 256);
   vibe_status s = grouped_ffn_check(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y);
   if (s != VIBE_OK) return s;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
@@ -170,7 +171,10 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
 
   VIBE_CUDA(cudaMemsetAsync(flush, 0, kProfileFlushBytes, st));
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st,
-                       [&](cudaStream_t ps) { return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, ps); });
+                       [&](cudaStream_t ps) {
+                         return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, ps, nullptr, nullptr, ffn_ws,
+                                                 grouped_ffn_ws_bytes(), false);
+                       });
 }
 
 extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
@@ -220,4 +224,16 @@ extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d,
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st, [&](cudaStream_t ps) {
     return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, ps);
   });
+}
+
+// Measurement utility: evict the L2 (evict_last read sweep, see l2_flush_kernel) before a timed region.
+extern "C" vibe_status vibe_l2_flush(void* scratch, size_t bytes, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(scratch != nullptr && bytes >= 64 && aligned16(scratch), VIBE_ERR_INVALID_ARG,
+               "vibe_l2_flush: scratch must be a 16-byte aligned device buffer of at least 64 bytes");
+  l2_flush_kernel<<<num_sms() * 8, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(
+      reinterpret_cast<const uint4*>(scratch), bytes / 16, reinterpret_cast<uint32_t*>(scratch));
+  VIBE_LAUNCH_CHECK("l2_flush_kernel");
+  return VIBE_OK;
 }

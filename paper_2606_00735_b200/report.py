@@ -80,6 +80,32 @@ def _time(fn, iters, warmup=5, period=1):
     return e0.elapsed_time(e1) * 1e3 / (reps * period)
 
 
+_FLUSH = None
+
+
+def _time_cold(fn, iters, warmup=3):
+    """Median CUDA-event time [us] of one fn() call that starts with a FLUSHED L2 (vibe_l2_flush before every timed
+    call, outside the event pair): what a kernel costs inside a model, where other layers have evicted its operands.
+    The call is captured into a CUDA graph, so the events bracket device time only."""
+    global _FLUSH
+    if _FLUSH is None:
+        _FLUSH = torch.zeros((256 << 20,), dtype=torch.uint8, device="cuda")
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        fn()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    for a, b in ev:
+        B.l2_flush(_FLUSH)
+        a.record()
+        g.replay()
+        b.record()
+    torch.cuda.synchronize()
+    return float(np.median([a.elapsed_time(b) for a, b in ev])) * 1e3
+
+
 def _dev_bf16(bits):
     return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
 
@@ -369,6 +395,7 @@ def section_mixed(peaks, quick):
              ("C2", I.C2, "128 x 16", [16] * 128), ("C2", I.C2, "24 x 1024", [1024] * 24 + [0] * 104),
              ("C2", I.C2, "24 x 1024 + 104 x 64", [1024] * 24 + [64] * 104)]
     held = {}
+    fws = torch.empty((max(16, B.workspace_bytes(B.WS_FFN, 1, 1, 1, 1, 64, 64)),), dtype=torch.uint8, device="cuda")
     for shape, cfg, label, rows in cases:
         E, d, f = cfg.E_loc, cfg.d, cfg.f
         if shape not in held:
@@ -381,12 +408,20 @@ def section_mixed(peaks, quick):
         H = torch.empty((R, f), dtype=torch.bfloat16, device="cuda")
         Y = torch.empty((R, d), dtype=torch.bfloat16, device="cuda")
         off = torch.tensor(np.concatenate([[0], np.cumsum(rows)]), dtype=torch.int32, device="cuda")
-        # timed twice, the smaller kept: the first case follows an idle device (weights just generated)
-        us = min(_time(lambda i: B.grouped_ffn(Xp, off, W1, W3, W2, H, Y), 20 if quick else 100, warmup=3)
+        # timed twice, the smaller kept: the first case follows an idle device (weights just generated).
+        # `us` = back-to-back replays (operands that fit the 126 MB L2 stay there: a lone C3 expert has 88 MB of
+        # weights); `cold_us` = every call after an L2 flush; `no_split_cold_us` = the same without the split-K workspace
+        us = min(_time(lambda i: B.grouped_ffn(Xp, off, W1, W3, W2, H, Y, ws=fws), 20 if quick else 100, warmup=3)
                  for _ in range(2))
+        cold = _time_cold(lambda: B.grouped_ffn(Xp, off, W1, W3, W2, H, Y, ws=fws), 15 if quick else 41)
+        cold_ns = _time_cold(lambda: B.grouped_ffn(Xp, off, W1, W3, W2, H, Y, ws=None), 15 if quick else 41)
         active = sum(1 for r in rows if r > 0)
+        floor_us = (active * 6.0 * d * f + 4.0 * R * d + 4.0 * R * f) / (peaks["hbm_gbs"] * 1e3)
         out.append({"shape": shape, "rows_per_expert": label, "rows": R, "active_experts": active, "us": round(us, 1),
+                    "cold_us": round(cold, 1), "no_split_cold_us": round(cold_ns, 1),
+                    "weight_stream_floor_us": round(floor_us, 1), "cold_over_floor": round(cold / floor_us, 2),
                     "weight_TB/s": round(active * 6.0 * d * f / us / 1e6, 2),
+                    "cold_weight_TB/s": round(active * 6.0 * d * f / cold / 1e6, 2),
                     "TFLOP/s": round(6.0 * R * d * f / us / 1e6, 1)})
     return out
 
@@ -616,11 +651,11 @@ def write_markdown(r, path, command):
             o.append(f"| {x['shape']} | {x['E_loc']} | {x['d']} | {x['f']} | {x['tokens_per_expert']} | {x['us_per_expert']} | {x['TFLOP/s']} | {x['frac_sustained']} | {x['frac_burst']} | {x['frac_of_per_expert_roofline']} |")
     if "ffn_mixed" in r:
         o.append("\n## ffn_mixed: grouped FFN on skewed row distributions (CUDA graph; weight TB/s = weights of the active experts / time)\n")
-        o.append("| shape | rows per expert | rows | active experts | us | weight TB/s | TFLOP/s |")
-        o.append("|---|---|---|---|---|---|---|")
+        o.append("| shape | rows per expert | rows | active experts | us (replayed) | weight TB/s | cold us (L2 flushed) | cold, no split-K | weight-stream floor us | cold / floor | TFLOP/s |")
+        o.append("|---|---|---|---|---|---|---|---|---|---|---|")
         for x in r["ffn_mixed"]:
-            o.append(f"| {x['shape']} | {x['rows_per_expert']} | {x['rows']} | {x['active_experts']} | {x['us']} | {x['weight_TB/s']} | {x['TFLOP/s']} |")
-        o.append("\nA light expert occupies its CTA pairs for (weight bytes of the tile) / ~140 GB/s whatever else runs (DESIGN.md section 12): heavy and light experts add.\n")
+            o.append(f"| {x['shape']} | {x['rows_per_expert']} | {x['rows']} | {x['active_experts']} | {x['us']} | {x['weight_TB/s']} | {x.get('cold_us', '')} | {x.get('no_split_cold_us', '')} | {x.get('weight_stream_floor_us', '')} | {x.get('cold_over_floor', '')} | {x['TFLOP/s']} |")
+        o.append("\nA light expert occupies its CTA pairs for (weight bytes of the tile) / ~140 GB/s whatever else runs (DESIGN.md section 12): heavy and light experts add; with at most half as many tiles as CTA pairs the split-K path spreads a tile's K range over several pairs.\n")
     if "fused_scatter" in r:
         o.append("\n## fused_scatter: vibe_grouped_ffn + vibe_combine vs vibe_grouped_ffn_scatter + vibe_combine_scattered (routed batches)\n")
         o.append("| config | ffn + combine us | fused scatter us | speedup |\n|---|---|---|---|")

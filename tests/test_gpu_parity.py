@@ -630,3 +630,43 @@ def test_ffn_fp8_ragged_token_tiles(rows, d, f):
     assert (Hq.cpu().numpy()[:R] != Hq_o).mean() <= 0.02
     m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_o)
     assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
+
+
+# ================================================================== f4: split-K for few active experts
+@pytest.mark.parametrize("shape,rows", [("C3", [1] + [0] * 31), ("C3", [0] * 5 + [16] + [0] * 26), ("C3", [17] + [0] * 31),
+                                        ("C3", [0] * 31 + [32]), ("C3", [300] + [0] * 31), ("C2", [0, 40, 0, 7] + [0] * 124),
+                                        ("small", [0, 33, 0, 0])])
+def test_ffn_split_k_few_active_experts(shape, rows):
+    """At most half as many tiles as CTA pairs: the split-K path (K range of a tile cut over several pairs, fp32
+    partials summed in slice order).  Same oracle, same bars; the result must not depend on the workspace being
+    given (ws = None runs the unsplit kernel) beyond fp32 summation order, and repeated calls on ONE workspace must
+    agree bit for bit (the arrival counters re-arm themselves)."""
+    E = len(rows)
+    d, f = {"C3": (7168, 2048), "C2": (2048, 768), "small": (256, 512)}[shape]
+    off = np.concatenate([[0], np.cumsum(rows)]).astype(np.int32)
+    R = int(off[-1])
+    Xp = I.make_X(R, d, 91)
+    act = [e for e in range(E) if rows[e] > 0]
+    W1a, W3a, W2a = I.make_weights(len(act), d, f, 92)            # weights of the active experts only (the others are never read)
+    W1 = torch.zeros((E, d, f), dtype=torch.bfloat16, device="cuda")
+    W3 = torch.zeros((E, d, f), dtype=torch.bfloat16, device="cuda")
+    W2 = torch.zeros((E, f, d), dtype=torch.bfloat16, device="cuda")
+    for i, e in enumerate(act):
+        W1[e], W3[e], W2[e] = dev_bf16(W1a[i]), dev_bf16(W3a[i]), dev_bf16(W2a[i])
+    off_c = np.concatenate([[0], np.cumsum([rows[e] for e in act])]).astype(np.int32)
+    Y_ref, H_ref = O.grouped_ffn(Xp, off_c, np.arange(R, dtype=np.int32), W1a, W3a, W2a)
+    Xp_d = torch.full((R + 40, d), float("nan"), dtype=torch.bfloat16, device="cuda")
+    Xp_d[:R] = dev_bf16(Xp)
+    ws = torch.empty((B.workspace_bytes(B.WS_FFN, 1, 1, E, E, d, f),), dtype=torch.uint8, device="cuda")
+    ws.fill_(0xA5)                                                # garbage: the call must not rely on its contents
+    Y1, H1 = B.grouped_ffn(Xp_d, dev(off), W1, W3, W2, ws=ws)
+    Y1, H1 = Y1.clone(), H1.clone()
+    Y2, H2 = B.grouped_ffn(Xp_d, dev(off), W1, W3, W2, ws=ws)
+    Y0, H0 = B.grouped_ffn(Xp_d, dev(off), W1, W3, W2, ws=None)
+    torch.cuda.synchronize()
+    assert torch.equal(Y1[:R].view(torch.int16), Y2[:R].view(torch.int16)) and torch.equal(H1[:R].view(torch.int16), H2[:R].view(torch.int16))
+    for Y, H in ((Y1, H1), (Y0, H0)):
+        mh = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(H)[:R]), H_ref)
+        assert mh["mean_rel_err"] <= FFN_MEAN, mh
+        m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_ref)
+        assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
