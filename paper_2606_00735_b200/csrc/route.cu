@@ -284,6 +284,199 @@ __global__ void __launch_bounds__(256) route_topk_kernel(const RouteParams p) {
   }
 }
 
+
+// ------------------------------------------------------------------------------------------------------------
+// Wide-lane variant for E = 8 * VPL experts (VPL = 16 | 32: the 128- and 256-expert configs): one token per 8-lane
+// group, FOUR tokens per warp, every lane owns VPL CONSECUTIVE experts (so lane order = expert order and the
+// ballot's lowest lane is the lowest index among equal keys, as above).  Every warp-wide instruction of the
+// selection rounds (redux, ballot, shuffle) now serves four tokens, and a lane keeps its first FOUR candidates in
+// pick order (key, index) sorted in registers: a lane gives away more than four of a token's k <= 8 picks about
+// once in a thousand tokens (then it rebuilds its heads from its registers).  ncu at 64K tokens x 256 experts, top-8:
+// see profiles/r2_route_ncu.md (the 32-lane kernel needed 702 warp-instructions per token).
+// Group-limited routing is supported when a group is exactly one lane's experts (n_group = 8: DeepSeek-V3's 8
+// groups of 32): the group score is the lane's own top-2 sum, no cross-lane merge.
+// ------------------------------------------------------------------------------------------------------------
+#ifndef ROUTE8_MIN_BLOCKS
+#define ROUTE8_MIN_BLOCKS 4
+#endif
+template <int VPL, bool SIGMOID>
+__global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(const RouteParams p) {
+  extern __shared__ int s_mem[];
+  int* s_hist = s_mem;
+  float* s_bias = reinterpret_cast<float*>(s_mem + p.E);      // [8][VPL + 1]: lane-major, padded (conflict-free)
+  for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
+    s_hist[i] = 0;
+    if (SIGMOID) s_bias[(i / VPL) * (VPL + 1) + i % VPL] = p.bias != nullptr ? p.bias[i] : 0.0f;
+  }
+  __syncthreads();
+  constexpr int LANES = 8;
+  const int lane = threadIdx.x & 31;
+  const int sub = lane & 7;
+  // Every collective below is issued with the FULL warp mask and stays inside the 8-lane groups by construction
+  // (xor-shuffles with offsets 1, 2, 4; a full ballot of which each group reads its own byte; indexed shuffles with
+  // a source lane of the own group): one instruction then serves the four tokens of the warp.  The same operations
+  // with a per-group member mask execute once per distinct mask -- four times -- which is what made a first version
+  // of this kernel slower than the 32-lane one.
+  constexpr unsigned FULL = 0xffffffffu;
+  const int gbase = lane & ~7;
+  auto gmax_u32 = [&](uint32_t v) {
+    v = max(v, __shfl_xor_sync(FULL, v, 1));
+    v = max(v, __shfl_xor_sync(FULL, v, 2));
+    return max(v, __shfl_xor_sync(FULL, v, 4));
+  };
+  auto gsum_f64 = [&](double v) {
+    v += __shfl_xor_sync(FULL, v, 4);
+    v += __shfl_xor_sync(FULL, v, 2);
+    return v + __shfl_xor_sync(FULL, v, 1);
+  };
+  const int gidx = threadIdx.x >> 3;
+  const int e0 = sub * VPL;
+  const int E = p.E, k = p.k;
+  const float NEG_INF = __int_as_float(0xff800000);
+
+  const float* my_bias = s_bias + sub * (VPL + 1);
+  auto unordered = [](uint32_t o) { return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o); };
+
+  // the trip count is WARP-uniform (full-mask collectives inside): a group past the last token works on a copy of
+  // token T-1 and stores nothing
+  for (int tw = blockIdx.x * 32 + (gidx & ~3); tw < p.T; tw += gridDim.x * 32) {
+    const bool valid = tw + (gidx & 3) < p.T;
+    const int t = valid ? tw + (gidx & 3) : p.T - 1;
+    // a lane's VPL * 4 bytes are contiguous: both 16-byte halves of every 32-byte sector are this lane's, read by
+    // consecutive instructions, so the loads allocate in L1 (the second half is then an L1 hit, not a second L2 request)
+    // Only the ordered keys stay in registers (the logits are recovered from them where the softmax needs them:
+    // the map is a bijection up to -0 -> +0, which exp does not see).
+    uint32_t uk[VPL];
+    const uint4* row4 = reinterpret_cast<const uint4*>(p.logits + (size_t)t * E + e0);
+#pragma unroll
+    for (int q = 0; q < VPL / 4; ++q) {
+      const uint4 u = __ldg(row4 + q);
+      const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        uk[4 * q + c] = SIGMOID ? ordered_u32(__fadd_rn(vsig(xv[c]), my_bias[4 * q + c])) : ordered_u32(xv[c]);
+    }
+    // ---- sorted first four (key, index) of this lane; strict > keeps the lower index first among equal keys ----
+    uint32_t h0 = kTaken, h1 = kTaken, h2 = kTaken, h3 = kTaken;
+    int i0 = 0, i1 = 0, i2 = 0, i3 = 0;
+    auto insert = [&](uint32_t c, int v) {
+      const bool b0 = c > h0, b1 = c > h1, b2 = c > h2, b3 = c > h3;
+      h3 = b2 ? h2 : (b3 ? c : h3);
+      i3 = b2 ? i2 : (b3 ? v : i3);
+      h2 = b1 ? h1 : (b2 ? c : h2);
+      i2 = b1 ? i1 : (b2 ? v : i2);
+      h1 = b0 ? h0 : (b1 ? c : h1);
+      i1 = b0 ? i0 : (b1 ? v : i1);
+      h0 = b0 ? c : h0;
+      i0 = b0 ? v : i0;
+    };
+#pragma unroll
+    for (int v = 0; v < VPL; ++v) insert(uk[v], v);
+    // ---- group-limited routing (R6), one group per lane: score = sum of the lane's two largest keys ----
+    if (p.n_group > 1) {
+      const float k0 = unordered(h0);
+      const float k1 = unordered(h1);
+      const float score = (VPL >= 2) ? __fadd_rn(k0, k1) : k0;
+      int rank = 0;
+#pragma unroll
+      for (int g2 = 0; g2 < LANES; ++g2) {
+        const float s2 = __shfl_sync(FULL, score, gbase + g2);
+        rank += (s2 > score || (s2 == score && g2 < sub)) ? 1 : 0;
+      }
+      if (rank >= p.topk_group) {
+        const uint32_t ninf = ordered_u32(NEG_INF);
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) uk[v] = ninf;
+        h0 = h1 = h2 = h3 = ninf;      // indices 0..3 in order: still the lane's first four in pick order
+        i0 = 0; i1 = 1; i2 = 2; i3 = 3;
+      }
+    }
+    // ---- k rounds: redux-max over the lane heads, ballot, lowest lane wins, pop in the winner ----
+    uint32_t lk = 0xffffffffu;
+    int lv = -1;
+    bool dry = false;
+    int my_id = 0;
+    uint32_t my_key = 0;
+    for (int j = 0; j < k; ++j) {
+      const uint32_t gm = gmax_u32(h0);
+      const unsigned b = (__ballot_sync(FULL, h0 == gm) >> gbase) & 0xffu;
+      const int win = gbase + __ffs(b) - 1;
+      const int id = __shfl_sync(FULL, e0 + i0, win);
+      if (sub == j) { my_id = id; my_key = gm; }
+      if (lane == win) {
+        lk = h0; lv = i0;
+        h0 = h1; i0 = i1; h1 = h2; i1 = i2; h2 = h3; i2 = i3; h3 = kTaken;
+      }
+      const bool need = (h0 == kTaken) && !dry;
+      if (__any_sync(FULL, need)) {            // rare: this lane gave away all four heads -> rebuild after (lk, lv)
+        h0 = h1 = h2 = h3 = kTaken;
+        i0 = i1 = i2 = i3 = 0;
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) {
+          const uint32_t c0 = uk[v];
+          const bool elig = (c0 < lk) || (c0 == lk && v > lv);
+          insert(elig ? c0 : kTaken, v);
+        }
+        dry = (h0 == kTaken);
+      }
+    }
+    const float* row = p.logits + (size_t)t * E;
+    float my_x = 0.0f;
+    if (sub < k) {
+      if (SIGMOID) my_x = __ldg(row + my_id);
+      else my_x = unordered(my_key);
+    }
+    // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
+    double wj = 0.0;
+    if (SIGMOID) {
+      const double sj = (sub < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
+      wj = sj;
+      if (p.renorm) wj = sj / gsum_f64(sj);
+    } else {
+      uint32_t lmx = uk[0];                    // (not h0: the heads have been popped)
+#pragma unroll
+      for (int v = 1; v < VPL; ++v) lmx = max(lmx, uk[v]);
+      const float mx = unordered(gmax_u32(lmx));
+      const double ej = (sub < k) ? exp((double)my_x - (double)mx) : 0.0;
+      double denom;
+      if (p.renorm) {
+        denom = gsum_f64(ej);
+      } else {
+        double part = 0.0;
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) part += (double)expf(unordered(uk[v]) - mx);
+        denom = gsum_f64(part);
+      }
+      wj = ej / denom;
+    }
+    wj *= (double)p.scale;
+    if (sub < k && valid) {
+      p.ids[(size_t)t * k + sub] = my_id;
+      p.w[(size_t)t * k + sub] = __double2float_rn(wj);
+      atomicAdd(&s_hist[my_id], 1);
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
+    const int c = s_hist[i];
+    if (c) atomicAdd(&p.counts[i], c);
+  }
+}
+
+template <int VPL>
+vibe_status launch_route8(const RouteParams& p, bool sigmoid, cudaStream_t st) {
+  int blocks = (p.T + 31) / 32;
+  const int cap = num_sms() * 8;
+  if (blocks > cap) blocks = cap;
+  const size_t smem = (size_t)p.E * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0);
+  if (sigmoid)
+    route_topk8_kernel<VPL, true><<<blocks, 256, smem, st>>>(p);
+  else
+    route_topk8_kernel<VPL, false><<<blocks, 256, smem, st>>>(p);
+  VIBE_LAUNCH_CHECK("route_topk8_kernel");
+  return VIBE_OK;
+}
+
 template <int LANES, int VPL>
 vibe_status launch_route(const RouteParams& p, bool sigmoid, cudaStream_t st) {
   constexpr int gpb = 256 / LANES;
@@ -346,6 +539,11 @@ extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* l
   p.topk_group = cfg->topk_group;
   const bool sig = cfg->score_fn == VIBE_SCORE_SIGMOID;
 
+  // 128 / 256 experts, top-k <= 8: four tokens per warp (route_topk8_kernel); group-limited only with 8 groups
+  if ((E == 128 || E == 256) && k <= 8 && (ng == 0 || ng == 8)) {
+    p.fast_groups = 1;
+    return E == 256 ? launch_route8<32>(p, sig, st) : launch_route8<16>(p, sig, st);
+  }
   int lanes, vpl;
   if (E <= 64 && k <= 8) {
     lanes = 8;

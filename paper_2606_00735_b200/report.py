@@ -171,6 +171,10 @@ def section_stages(peaks, quick, only=None):
         t_route = _time(route, iters, period=nsets)
         t_perm = _time(permute, iters, period=nsets)
         t_comb = _time(combine, iters, period=nsets)
+        # the floor of the route OP on this box: a selection-free kernel that only streams the same logits once
+        # (vibe_l2_flush: 16-byte loads, no arithmetic) -- what reading 4*T*E bytes costs including the launch
+        lgb = [x["lg"].view(torch.uint8).view(-1) for x in sets]
+        t_read = _time(lambda i: B.l2_flush(lgb[i % nsets]), iters, period=nsets)
         s0 = sets[0]
         R = int(s0["off"][-1].item())
         res_tok = int((s0["a2r"].view(T, k) >= 0).any(dim=1).sum().item())
@@ -184,6 +188,8 @@ def section_stages(peaks, quick, only=None):
             gbs = by[name] / t / 1e3
             row[name] = {"us": round(t, 2), "bytes": by[name], "GB/s": round(gbs, 1), "frac_hbm": round(gbs / hbm, 4),
                          "us_at_hbm_peak": round(by[name] / hbm / 1e3, 2)}
+        row["route"]["logit_read_stream_us"] = round(t_read, 2)
+        row["route"]["frac_of_read_stream"] = round(t_read / t_route, 4)
         out.append(row)
         del sets
         torch.cuda.empty_cache()
