@@ -334,6 +334,23 @@ VIBE_API vibe_status vibe_moe_layer_forward_host_chunked(const vibe_route_cfg* c
                                                          int32_t* counts_h /*host*/, int32_t n_chunks, void* arena,
                                                          size_t arena_bytes, void* stream);
 
+/* ASYNCHRONOUS host entry: the same work as vibe_moe_layer_forward_host with one token chunk, but the call only
+ * ENQUEUES it -- copy-in on the library's copy-in stream, the layer on `stream`, copy-out on the library's copy-out
+ * stream -- and returns a ticket; vibe_host_wait(ticket) blocks until out_h and counts_h of that call are filled.
+ * Issued back to back with TWO arenas (and two result buffers), step i+1's copy-in and step i-1's copy-out overlap
+ * step i's kernels, and every step still streams the weights once over the whole batch (no token chunks).
+ * Contract: host buffers must be PINNED (pageable memory makes the copies synchronous: still correct, no overlap);
+ * an arena, its out_h / counts_h and the host inputs of a call belong to that call until its ticket has been waited
+ * for; at most 8 tickets may be outstanding per device; tickets are waited for in any order, each exactly once.
+ * out_h / counts_h are bit-identical to vibe_moe_layer_forward_host's. */
+VIBE_API vibe_status vibe_moe_layer_forward_host_async(const vibe_route_cfg* cfg /*host*/,
+                                                       const float* logits_h /*host*/, const void* X_h /*host*/,
+                                                       const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
+                                                       int32_t E_loc, const void* W1, const void* W3, const void* W2,
+                                                       void* out_h /*host*/, int32_t* counts_h /*host*/, void* arena,
+                                                       size_t arena_bytes, void* stream, int32_t* ticket /*host, out*/);
+VIBE_API vibe_status vibe_host_wait(int32_t ticket);
+
 /* The whole layer with the FP8 FFN (f2): route -> e4m3 quantisation of the token rows (on an expert-parallel
  * shard only of the tokens that have a resident expert) -> permute (one-byte rows) -> row-scale gather -> vibe_grouped_ffn_fp8 -> combine.  Packed weights / scales as in
  * vibe_grouped_ffn_fp8; arena: vibe_workspace_bytes(VIBE_WS_LAYER_FP8, ...) bytes, 256-byte aligned.

@@ -41,7 +41,7 @@ EXPORTED_SYMBOLS = (
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
     "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward_host_chunked",
-    "vibe_l2_flush", "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
+    "vibe_l2_flush", "vibe_moe_layer_forward_host_async", "vibe_host_wait", "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
     "vibe_moe_layer_forward_mxfp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
@@ -124,6 +124,11 @@ def load() -> C.CDLL:
                                                         vp, vp, vp, i32, vp, sz, vp]
     lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                                vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_moe_layer_forward_host_async.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
+                                                      vp, vp, vp, sz, vp, C.POINTER(i32)]
+    lib.vibe_moe_layer_forward_host_async.restype = C.c_int
+    lib.vibe_host_wait.argtypes = [i32]
+    lib.vibe_host_wait.restype = C.c_int
     lib.vibe_l2_flush.argtypes = [vp, sz, vp]
     lib.vibe_l2_flush.restype = C.c_int
     lib.vibe_mxfp8_sf_bytes.argtypes = [i32] * 4
@@ -628,6 +633,29 @@ def moe_layer_forward_host(cfg: RouteConfig, logits_h: torch.Tensor, X_h: torch.
                                                     arena.data_ptr(), arena.numel(), _stream(stream)),
             "vibe_moe_layer_forward_host_chunked")
     return out_h, counts_h
+
+
+def moe_layer_forward_host_async(cfg: RouteConfig, logits_h: torch.Tensor, X_h: torch.Tensor, expert_map, W1, W3, W2,
+                                 out_h: torch.Tensor, counts_h: torch.Tensor, arena: torch.Tensor, stream=None) -> int:
+    """Enqueue one step from PINNED host tensors and return its ticket; host_wait(ticket) blocks until out_h / counts_h
+    are filled.  The arena, the result buffers and the inputs belong to the call until then (use two sets to overlap
+    consecutive steps)."""
+    lib = load()
+    T, d = X_h.shape
+    E_loc, _, f = W1.shape
+    assert not logits_h.is_cuda and not X_h.is_cuda and not out_h.is_cuda and not counts_h.is_cuda
+    c = cfg._c()
+    t = C.c_int32(-1)
+    _ok(lib.vibe_moe_layer_forward_host_async(C.byref(c), logits_h.data_ptr(), X_h.data_ptr(),
+                                              expert_map.data_ptr() if expert_map is not None else None, T, d, f, E_loc,
+                                              W1.data_ptr(), W3.data_ptr(), W2.data_ptr(), out_h.data_ptr(),
+                                              counts_h.data_ptr(), arena.data_ptr(), arena.numel(), _stream(stream),
+                                              C.byref(t)), "vibe_moe_layer_forward_host_async")
+    return int(t.value)
+
+
+def host_wait(ticket: int) -> None:
+    _ok(load().vibe_host_wait(int(ticket)), "vibe_host_wait")
 
 
 # ------------------------------------------------------------------------------------ placement (host)

@@ -57,10 +57,15 @@ namespace {
 constexpr int kMaxHostChunks = 8;
 
 // Two copy streams and the events that order them against the caller's stream; created once per device.
+constexpr int kMaxTickets = 8;     // outstanding asynchronous host calls per device
+
 struct HostPipe {
   cudaStream_t in = nullptr, out = nullptr;
   cudaEvent_t entry = nullptr, out_done = nullptr;
   cudaEvent_t in_done[kMaxHostChunks] = {}, comp_done[kMaxHostChunks] = {};
+  // the asynchronous entry: one event triple per ticket slot
+  cudaEvent_t t_entry[kMaxTickets] = {}, t_in[kMaxTickets] = {}, t_comp[kMaxTickets] = {}, t_done[kMaxTickets] = {};
+  bool t_busy[kMaxTickets] = {};
   bool ready = false;
   std::mutex in_use;   // one pipelined call per device at a time (the events are per device, and the call waits anyway)
 };
@@ -81,6 +86,12 @@ vibe_status host_pipe(HostPipe** pp) {
     for (int c = 0; c < kMaxHostChunks; ++c) {
       VIBE_CUDA(cudaEventCreateWithFlags(&hp.in_done[c], cudaEventDisableTiming));
       VIBE_CUDA(cudaEventCreateWithFlags(&hp.comp_done[c], cudaEventDisableTiming));
+    }
+    for (int c = 0; c < kMaxTickets; ++c) {
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.t_entry[c], cudaEventDisableTiming));
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.t_in[c], cudaEventDisableTiming));
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.t_comp[c], cudaEventDisableTiming));
+      VIBE_CUDA(cudaEventCreateWithFlags(&hp.t_done[c], cudaEventDisableTiming));
     }
     hp.ready = true;
   }
@@ -221,6 +232,103 @@ extern "C" vibe_status vibe_moe_layer_forward_host(const vibe_route_cfg* cfg, co
                                                    size_t arena_bytes, void* stream) {
   return vibe_moe_layer_forward_host_chunked(cfg, logits_h, X_h, expert_map, T, d, f, E_loc, W1, W3, W2, out_h,
                                              counts_h, 0, arena, arena_bytes, stream);
+}
+
+extern "C" vibe_status vibe_moe_layer_forward_host_async(const vibe_route_cfg* cfg, const float* logits_h, const void* X_h,
+                                                         const int32_t* expert_map, int32_t T, int32_t d, int32_t f,
+                                                         int32_t E_loc, const void* W1, const void* W3, const void* W2,
+                                                         void* out_h, int32_t* counts_h, void* arena, size_t arena_bytes,
+                                                         void* stream, int32_t* ticket) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(cfg != nullptr && ticket != nullptr, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host_async: cfg / ticket is NULL");
+  VIBE_REQUIRE(T >= 1 && d >= 8 && f >= 8 && E_loc >= 1, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host_async: bad sizes");
+  VIBE_REQUIRE(logits_h && X_h && out_h && counts_h, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host_async: NULL host buffer");
+  const int E = cfg->num_experts, k = cfg->top_k;
+  VIBE_REQUIRE(E >= 1 && k >= 1 && k <= E, VIBE_ERR_INVALID_ARG, "vibe_moe_layer_forward_host_async: need 1 <= k <= E");
+  {
+    vibe_status lim = grouped_ffn_limits("vibe_moe_layer_forward_host_async", E_loc, d, f, W1, W3, W2);
+    if (lim != VIBE_OK) return lim;
+  }
+  const size_t inner = vibe_workspace_bytes(VIBE_WS_LAYER, T, k, E, E_loc, d, f, 1);
+  const size_t need = vibe_workspace_bytes(VIBE_WS_LAYER_HOST, T, k, E, E_loc, d, f, 1);
+  VIBE_REQUIRE(arena != nullptr && arena_bytes >= need && (reinterpret_cast<uintptr_t>(arena) & 255u) == 0,
+               VIBE_ERR_WORKSPACE, "vibe_moe_layer_forward_host_async: arena needs %zu bytes, 256-byte aligned (got %zu)",
+               need, arena_bytes);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  char* p = reinterpret_cast<char*>(arena) + inner;
+  float* logits_d = reinterpret_cast<float*>(p);
+  p += round_up((size_t)T * E * 4, 256);
+  char* X_d = p;
+  p += round_up((size_t)T * d * 2, 256);
+  char* out_d = p;
+  p += round_up((size_t)T * d * 2, 256);
+  int32_t* counts_d = reinterpret_cast<int32_t*>(p);
+  HostPipe* hp = nullptr;
+  vibe_status s = host_pipe(&hp);
+  if (s != VIBE_OK) return s;
+  int dev = current_device(), slot = -1;
+  {
+    std::lock_guard<std::mutex> lk(hp->in_use);
+    for (int c = 0; c < kMaxTickets && slot < 0; ++c)
+      if (!hp->t_busy[c]) slot = c;
+    VIBE_REQUIRE(slot >= 0, VIBE_ERR_UNSUPPORTED, "vibe_moe_layer_forward_host_async: %d tickets outstanding on this device", kMaxTickets);
+    // copy-in (NOT ordered after the work on `stream`: the previous step's kernels are there, and the copy must
+    // overlap them; the host inputs are the host's and ready when the call is made, the arena is free by contract),
+    // then the layer on `stream`, then the copy-out; the three queues of consecutive calls overlap
+    VIBE_CUDA(cudaMemcpyAsync(logits_d, logits_h, (size_t)T * E * 4, cudaMemcpyHostToDevice, hp->in));
+    VIBE_CUDA(cudaMemcpyAsync(X_d, X_h, (size_t)T * d * 2, cudaMemcpyHostToDevice, hp->in));
+    VIBE_CUDA(cudaEventRecord(hp->t_in[slot], hp->in));
+    VIBE_CUDA(cudaStreamWaitEvent(st, hp->t_in[slot], 0));
+    s = vibe_moe_layer_forward(cfg, logits_d, X_d, expert_map, T, d, f, E_loc, W1, W3, W2, out_d, counts_d, nullptr, nullptr,
+                               arena, inner, stream);
+    if (s != VIBE_OK) {
+      cudaStreamSynchronize(hp->in);
+      cudaStreamSynchronize(st);
+      return s;
+    }
+    VIBE_CUDA(cudaEventRecord(hp->t_comp[slot], st));
+    VIBE_CUDA(cudaStreamWaitEvent(hp->out, hp->t_comp[slot], 0));
+    VIBE_CUDA(cudaMemcpyAsync(out_h, out_d, (size_t)T * d * 2, cudaMemcpyDeviceToHost, hp->out));
+    VIBE_CUDA(cudaMemcpyAsync(counts_h, counts_d, (size_t)E * 4, cudaMemcpyDeviceToHost, hp->out));
+    VIBE_CUDA(cudaEventRecord(hp->t_done[slot], hp->out));
+    hp->t_busy[slot] = true;
+  }
+  *ticket = dev * kMaxTickets + slot;
+  return VIBE_OK;
+}
+
+extern "C" vibe_status vibe_host_wait(int32_t ticket) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(ticket >= 0 && ticket < kMaxDevices * kMaxTickets, VIBE_ERR_INVALID_ARG, "vibe_host_wait: bad ticket %d", ticket);
+  const int dev = ticket / kMaxTickets, slot = ticket % kMaxTickets;
+  int cur = 0;
+  VIBE_CUDA(cudaGetDevice(&cur));
+  HostPipe* hp = nullptr;
+  if (cur != dev) VIBE_CUDA(cudaSetDevice(dev));
+  vibe_status s = host_pipe(&hp);
+  if (s == VIBE_OK) {
+    bool busy;
+    {
+      std::lock_guard<std::mutex> lk(hp->in_use);
+      busy = hp->t_busy[slot];
+    }
+    if (!busy) {
+      set_error("vibe_host_wait: ticket %d is not outstanding", ticket);
+      s = VIBE_ERR_INVALID_ARG;
+    } else {
+      const cudaError_t e = cudaEventSynchronize(hp->t_done[slot]);
+      std::lock_guard<std::mutex> lk(hp->in_use);
+      hp->t_busy[slot] = false;
+      if (e != cudaSuccess) {
+        set_error("vibe_host_wait: %s", cudaGetErrorString(e));
+        s = VIBE_ERR_CUDA;
+      }
+    }
+  }
+  if (cur != dev) cudaSetDevice(cur);
+  return s;
 }
 
 extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, const float* logits, const void* X,

@@ -373,6 +373,7 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
 #pragma unroll
     for (int v = 0; v < VPL; ++v) insert(uk[v], v);
     // ---- group-limited routing (R6), one group per lane: score = sum of the lane's two largest keys ----
+    bool masked = false;
     if (p.n_group > 1) {
       const float k0 = unordered(h0);
       const float k1 = unordered(h1);
@@ -384,10 +385,10 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
         rank += (s2 > score || (s2 == score && g2 < sub)) ? 1 : 0;
       }
       if (rank >= p.topk_group) {
-        const uint32_t ninf = ordered_u32(NEG_INF);
-#pragma unroll
-        for (int v = 0; v < VPL; ++v) uk[v] = ninf;
-        h0 = h1 = h2 = h3 = ninf;      // indices 0..3 in order: still the lane's first four in pick order
+        // the lane's keys count as -inf in the selection; uk[] keeps the logits' images (the softmax denominator
+        // without renormalisation runs over ALL experts)
+        masked = true;
+        h0 = h1 = h2 = h3 = ordered_u32(NEG_INF);      // indices 0..3 in order: the lane's first four in pick order
         i0 = 0; i1 = 1; i2 = 2; i3 = 3;
       }
     }
@@ -413,7 +414,7 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
         i0 = i1 = i2 = i3 = 0;
 #pragma unroll
         for (int v = 0; v < VPL; ++v) {
-          const uint32_t c0 = uk[v];
+          const uint32_t c0 = masked ? ordered_u32(NEG_INF) : uk[v];
           const bool elig = (c0 < lk) || (c0 == lk && v > lv);
           insert(elig ? c0 : kTaken, v);
         }

@@ -670,3 +670,35 @@ def test_ffn_split_k_few_active_experts(shape, rows):
         assert mh["mean_rel_err"] <= FFN_MEAN, mh
         m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_ref)
         assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
+
+
+# ================================================================== asynchronous host entry
+def test_host_async_entry_same_bits_and_overlapping_steps():
+    """vibe_moe_layer_forward_host_async / vibe_host_wait: several steps in flight on two arenas give, step by step,
+    the bits of the synchronous host entry; a ticket can be waited for once only."""
+    cfg = I.scaled(I.C2, T=700, d=256, f=256, E=16, E_loc=16, k=4)
+    Ls = [I.make_layer(cfg, 30 + i) for i in range(4)]
+    rc, _, _, emap, W1, W3, W2 = layer_device_inputs(cfg, Ls[0])
+    need = B.workspace_bytes(B.WS_LAYER_HOST, cfg.T, cfg.k, cfg.E, cfg.E_loc, cfg.d, cfg.f)
+    arenas = [torch.empty((need,), dtype=torch.uint8, device="cuda") for _ in range(2)]
+    lg = [torch.from_numpy(L["logits"]).pin_memory() for L in Ls]
+    Xh = [torch.from_numpy(L["X"].view(np.int16)).view(torch.bfloat16).pin_memory() for L in Ls]
+    outs = [torch.empty((cfg.T, cfg.d), dtype=torch.bfloat16).pin_memory() for _ in Ls]
+    cnts = [torch.empty((cfg.E,), dtype=torch.int32).pin_memory() for _ in Ls]
+    tickets = []
+    for i in range(4):
+        if i >= 2:
+            B.host_wait(tickets[i - 2])                       # the arena of step i-2 is free again
+        tickets.append(B.moe_layer_forward_host_async(rc, lg[i], Xh[i], emap, W1, W3, W2, outs[i], cnts[i], arenas[i % 2]))
+    B.host_wait(tickets[2])
+    B.host_wait(tickets[3])
+    with pytest.raises(B.VibeError):
+        B.host_wait(tickets[3])
+    ref = torch.empty((cfg.T, cfg.d), dtype=torch.bfloat16).pin_memory()
+    refc = torch.empty((cfg.E,), dtype=torch.int32).pin_memory()
+    for i in range(4):
+        B.moe_layer_forward_host(rc, lg[i], Xh[i], emap, W1, W3, W2, ref, refc, arenas[0], n_chunks=1)
+        assert torch.equal(ref.view(torch.int16), outs[i].view(torch.int16)), i
+        assert torch.equal(refc, cnts[i]), i
+        _, _, c_o = O.route_topk(Ls[i]["logits"], select_bias=Ls[i]["select_bias"], **I.route_kwargs(cfg))
+        assert np.array_equal(cnts[i].numpy(), c_o)
