@@ -92,7 +92,8 @@ struct SmemTail {
   uint64_t tempty[2];             // leader CTA: all 8 epilogue warps of the pair drained it
   uint32_t tmem_base;
   int32_t total_t_tiles;
-  int32_t split;                  // K slices per tile (1 = no split-K)
+  int32_t split;                  // K slices of a split tile (1 = no split-K)
+  int32_t split_from;             // first split tile: tiles [split_from, total) are cut into `split` K slices
   int32_t off[MAX_SLOTS + 1];     // segment starts (rows)
   int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
   int32_t tsz[MAX_SLOTS];         // rows per token tile of the slot (multiple of 16, <= TN)
@@ -252,10 +253,21 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       tail->cum[E_loc] = carry;
       tail->off[E_loc] = offsets[E_loc];
       tail->total_t_tiles = carry;
+      // Split-K covers the LAST, partly filled round of tiles: with total = q * pairs + r tiles, the r tiles of
+      // the last round would occupy r pairs for a whole tile time while the others idle (r = 34 of 74 at 8 x 512
+      // rows of the C1 down projection: 14 % of the kernel).  When r <= pairs / 2 each of them is cut into
+      // S = pairs / r K slices (q = 0 is the few-active-experts case above).
       int S = 1;
       const int total = carry * NB;
-      if (split_part != nullptr && total > 0 && 2 * total <= num_pairs && num_pairs <= SPLIT_MAX_UNITS)
-        S = max(1, min(min(num_pairs / total, SPLIT_MAX), KB / SPLIT_MIN_STEPS));
+      int from = total;
+      const int r = total % num_pairs;
+      // (only when the last round is a material share of the kernel: at most 7 rounds -- beyond that the dump /
+      // fence / re-read of a split tile costs about what the idle pairs would; measured, same-box A/B)
+      if (split_part != nullptr && r > 0 && 2 * r <= num_pairs && total / num_pairs <= 6 && num_pairs <= SPLIT_MAX_UNITS) {
+        S = max(1, min(min(num_pairs / r, SPLIT_MAX), KB / SPLIT_MIN_STEPS));
+        if (S > 1) from = total - r;
+      }
+      tail->split_from = from;
       tail->split = S;
     }
   }
@@ -266,8 +278,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
   ptx::tc_fence_after();
 
   const uint32_t tmem_base = tail->tmem_base;
-  const int S = tail->split;                               // K slices per tile
-  const int total_units = tail->total_t_tiles * NB * S;    // a unit = (tile, K slice); S = 1: a unit is a tile
+  const int S = tail->split;                               // K slices of a split tile
+  const int split_from = tail->split_from;                 // tiles below are whole units, tiles from here on S units each
+  const int total_units = split_from + (tail->total_t_tiles * NB - split_from) * S;    // a unit = (tile, K slice)
 
   if (warp == 0) {
     // ================================================================ TMA producer (both CTAs)
@@ -288,8 +301,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       uint32_t phase = 0;
       for (int rnd = 0, unit = pair; unit < total_units; ++rnd, unit = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
-        const int tile = unit / S, slice = unit - tile * S;
-        const int kb_lo = slice * KB / S, kb_hi = (slice + 1) * KB / S;
+        const bool is_split = unit >= split_from;
+        const int tile = is_split ? split_from + (unit - split_from) / S : unit;
+        const int slice = is_split ? (unit - split_from) % S : 0, nsl = is_split ? S : 1;
+        const int kb_lo = slice * KB / nsl, kb_hi = (slice + 1) * KB / nsl;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
         const int tsz = tail->tsz[e];
@@ -341,8 +356,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       int it = 0;
       for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
         int f_blk, t_blk;
-        const int tile = unit / S, slice = unit - tile * S;
-        const int kb_lo = slice * KB / S, kb_hi = (slice + 1) * KB / S;
+        const bool is_split = unit >= split_from;
+        const int tile = is_split ? split_from + (unit - split_from) / S : unit;
+        const int slice = is_split ? (unit - split_from) % S : 0, nsl = is_split ? S : 1;
+        const int kb_lo = slice * KB / nsl, kb_hi = (slice + 1) * KB / nsl;
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
         const int tsz = tail->tsz[e];
@@ -385,7 +402,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     int it = 0;
     for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
       int f_blk, t_blk;
-      const int tile = unit / S;
+      const bool is_split = unit >= split_from;
+      const int tile = is_split ? split_from + (unit - split_from) / S : unit;
       cur.decode(tail, tile, NB, f_blk, t_blk);
       const int e = cur.e;
       const int tsz = tail->tsz[e];
@@ -411,10 +429,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
-      if (S > 1) {
+      if (is_split) {
         // ------------------------------------------------------------ split-K unit
         // (1) dump this warp's part of the fp32 accumulator: part[unit][column][rank * 128 + TMEM lane]
-        float* mypart = split_part + ((size_t)unit * TN) * 256 + rank * 128 + q * 32 + lane;
+        float* mypart = split_part + ((size_t)(unit - split_from) * TN) * 256 + rank * 128 + q * 32 + lane;
         for (int c0 = kGateUp ? 0 : blk_par * 32; c0 < n_rows; c0 += kGateUp ? 32 : 64) {
           uint32_t a[32];
           ptx::tmem_ld_32x32(taddr + c0, a);
@@ -428,7 +446,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa_u32(ptx::smem_u32(&tail->tempty[acc]), 0));
         // (2) arrive on the counter of this tile portion; the last of its S (x 2: gate and up warp) arrivals finishes it
         const int role = kGateUp ? (q & 1) : (warp - 2);
-        int* cnt = split_cnt + (tile * 2 + (int)rank) * 8 + role;
+        int* cnt = split_cnt + ((tile - split_from) * 2 + (int)rank) * 8 + role;
         const int expect = kGateUp ? 2 * S : S;
         __threadfence();
         int last = 0;
@@ -440,7 +458,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         if (last) {
           __threadfence();
           // (3) sum the S partials in slice order, then the normal epilogue on the sum
-          const float* p0 = split_part + ((size_t)tile * S * TN) * 256 + rank * 128;
+          const float* p0 = split_part + ((size_t)(tile - split_from) * S * TN) * 256 + rank * 128;
           if (kGateUp) {
             const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
             const bool feat_ok = feat < n_total;
