@@ -18,7 +18,7 @@ CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(os.path.dirname(PKG), "include")
 LIB = os.path.join(PKG, "libvibe.so")
 STAMP = os.path.join(PKG, "build", "libvibe.stamp")
-SOURCES = ["api.cu", "route.cu", "permute.cu", "combine.cu", "ffn.cu", "ffn_fp8.cu", "fp8_quant.cu", "profile.cu", "layer.cu", "placement.cpp"]
+SOURCES = ["api.cu", "route.cu", "permute.cu", "combine.cu", "ffn.cu", "fp8_quant.cu", "profile.cu", "layer.cu", "placement.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",

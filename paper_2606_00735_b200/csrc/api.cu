@@ -85,6 +85,7 @@ LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f) {
   a.Hq = take((size_t)a.R_cap * f);
   a.Y = take((size_t)a.R_cap * d * 2);
   a.perm_ws = take(permute_ws_bytes(T, k, E_loc));
+  a.ffn_ws = take(grouped_ffn_ws_bytes());
   a.total = o;
   return a;
 }
@@ -114,6 +115,7 @@ LayerArenaMx layer_arena_mx(int T, int k, int E_loc, int d, int f) {
   a.hsf = take((size_t)(f / 128) * 32 * Rb * 4);
   a.Y = take((size_t)a.R_cap * d * 2);
   a.perm_ws = take(permute_ws_bytes(T, k, E_loc));
+  a.ffn_ws = take(grouped_ffn_ws_bytes());
   a.total = o;
   return a;
 }

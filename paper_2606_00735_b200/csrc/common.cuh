@@ -65,10 +65,11 @@ vibe_status grouped_ffn_zero_counters(void* ws, cudaStream_t st);   // what ws_z
 vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const int32_t* offsets, int E_loc, int R_cap,
                                  int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
                                  const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
-                                 cudaStream_t st);
+                                 cudaStream_t st, void* ws = nullptr, size_t ws_bytes = 0, bool ws_zeroed = false);
 vibe_status grouped_ffn_mxfp8_impl(const void* Xq, const void* xsf, const int32_t* offsets, int E_loc, int R_cap, int d,
                                    int f, const void* W1q, const void* W3q, const void* sf13, const void* W2q,
-                                   const void* sf2, void* Hq, void* hsf, void* Y, cudaStream_t st);
+                                   const void* sf2, void* Hq, void* hsf, void* Y, cudaStream_t st, void* ws = nullptr,
+                                   size_t ws_bytes = 0, bool ws_zeroed = false);
 // words per (K stage, lane) row of a token-scale array [K/128][32][Rb]: the 32-row blocks of R_cap rows, rounded up to
 // a 16-byte row pitch (a TMA global stride; the kernel only fetches boxes of 4 row blocks that start on a multiple of 4,
 // so a box is entirely inside or entirely outside the tensor)
@@ -103,12 +104,12 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 }
 
 struct LayerArenaFp8 {
-  size_t ids, w, offsets, r2a, a2r, Xq, tok_scale, Xpq, row_scale, Hq, Y, perm_ws, total;
+  size_t ids, w, offsets, r2a, a2r, Xq, tok_scale, Xpq, row_scale, Hq, Y, perm_ws, ffn_ws, total;
   int64_t R_cap;
 };
 LayerArenaFp8 layer_arena_fp8(int T, int k, int E_loc, int d, int f);
 struct LayerArenaMx {
-  size_t ids, w, offsets, r2a, a2r, Xq, tok_sf, Xpq, xsf, Hq, hsf, Y, perm_ws, total;
+  size_t ids, w, offsets, r2a, a2r, Xq, tok_sf, Xpq, xsf, Hq, hsf, Y, perm_ws, ffn_ws, total;
   int64_t R_cap;
 };
 LayerArenaMx layer_arena_mx(int T, int k, int E_loc, int d, int f);

@@ -47,7 +47,25 @@
 // order, so the result does not depend on which unit came last -- and runs the normal epilogue on the sum.
 // S is derived on the device from `offsets`, like everything else.
 //
-// Semantics: include/vibe.h (vibe_grouped_ffn); F1-F4.
+// ONE kernel, three operand kinds (template parameter kKind) -- producer, MMA issuer, tile scheduler, split-K and
+// the epilogue skeleton are shared; a kind changes only what is listed here:
+//   KIND_BF16  bf16 x bf16 (kind::f16), K = 16 per MMA, 64 K elements per 128-byte smem row; the weights are consumed in
+//              place, [E_loc,K,N] N-contiguous: MN-major A descriptors, TMA coordinates (n, k, e)
+//   KIND_F8    e4m3 x e4m3 (kind::f8f6f4), K = 32 per MMA, 128 K elements per row; weights pre-quantised and
+//              pre-transposed to [E_loc,N,K] (vibe_fp8_pack_weights): K-major A, TMA coordinates (k, n, e); per-row,
+//              per-expert and static H scales multiply the accumulators in the epilogue; GEMM-1 writes H as e4m3
+//              (readings Q1-Q4)
+//   KIND_MXF8  e4m3 BLOCK-SCALED (kind::mxf8f6f4.block_scale; readings Q5-Q8): one UE8M0 scale per operand row and 32
+//              K elements, applied by the tensor core.  The scales of a K = 128 stage travel with the stage (weights:
+//              one 512-byte chunk already in TMEM order; tokens: aligned {4 row blocks x 32 rows} boxes of the
+//              [K/128][32][Rb] word array, which land in TMEM order; a tile that starts on a 64-row boundary reads
+//              them from column 0 or 2 of its chunk), are copied to TMEM by tcgen05.cp ahead of the stage's four MMAs
+//              (same issuing thread: ordered with them), and the instruction descriptor's scale-factor ids pick the
+//              K-block's byte.  Token tiles are multiples of 64 rows and at most 192 (2 x 192 accumulator columns + 12
+//              scale columns fit the 512 TMEM columns); no scale arithmetic is left in the epilogues; GEMM-1
+//              block-quantises H per row and 32 features (one warp = one block: redux.sync max).
+//
+// Semantics: include/vibe.h (vibe_grouped_ffn, vibe_grouped_ffn_fp8, vibe_grouped_ffn_mxfp8); F1-F4, Q1-Q8.
 #include <mutex>
 #include <unordered_map>
 #include <string>
@@ -59,16 +77,27 @@
 namespace vibe {
 namespace {
 
-constexpr int BK = 64;                  // K per smem stage (one 128-byte swizzle atom of bf16)
-constexpr int TN = 256;                 // tokens per tile = max UMMA N
-constexpr int UMMA_K = 16;
+enum { KIND_BF16 = 0, KIND_F8 = 1, KIND_MXF8 = 2 };
+__host__ __device__ constexpr int bk_of(int kind) { return kind == KIND_BF16 ? 64 : 128; }      // K elements per smem stage (128 bytes)
+__host__ __device__ constexpr int umma_k_of(int kind) { return kind == KIND_BF16 ? 16 : 32; }  // K per MMA instruction (32 bytes)
+__host__ __device__ constexpr int tn_of(int kind) { return kind == KIND_MXF8 ? 192 : 256; }    // tokens per tile = TMEM columns per accumulator
+__host__ __device__ constexpr int talign_of(int kind) { return kind == KIND_MXF8 ? 64 : 16; }  // token tiles are multiples of this
+
+constexpr int TN = 256;                 // largest token tile = max UMMA N
 constexpr int STAGES = 6;
-constexpr int ATOM_BYTES = 64 * BK * 2;         // 8 KB : 64 features x 64 K (MN-major, SW128)
+constexpr int ATOM_BYTES = 64 * 128;            // 8 KB : 64 features x 128 bytes of K (or 64 K-rows x 128 bytes of features), SW128
 constexpr int A_BYTES = 2 * ATOM_BYTES;         // 16 KB: this CTA's 128 accumulator lanes
-constexpr int B_BYTES = (TN / 2) * BK * 2;      // 16 KB: this CTA's half of the token tile
+constexpr int B_BYTES = (TN / 2) * 128;         // 16 KB: this CTA's half of the token tile
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;  // 32 KB
 constexpr int NARROW_ROWS = 32;                 // rows of the small activation box (per CTA)
 constexpr int XCHG_BYTES = 16384;               // gate/up swap: 2 warp pairs x 2 directions x 4 KB
+constexpr int SX_BYTES = 4 * TN * 4;            // KIND_F8 GEMM-1: the tile's row scales, one 1 KB slice per epilogue warp
+// block-scaled kind: per-CTA activation bytes of a stage, and where the stage keeps its scale factors
+constexpr int B_BYTES_MX = (tn_of(KIND_MXF8) / 2) * 128;   // 12 KB
+constexpr int SFA_OFF = A_BYTES + B_BYTES_MX;   // 512 B : this CTA's 128 weight rows x 4 K-blocks
+constexpr int SFB_OFF = SFA_OFF + 512;          // 1 KB  : up to two 128-row chunks of token scales x 4 K-blocks
+static_assert(SFB_OFF + 1024 <= STAGE_BYTES, "scale factors must fit behind the narrower activation tile");
+constexpr uint32_t SF_TMEM_COL = 2 * tn_of(KIND_MXF8);     // columns 384.. : SFA (4) then SFB (8)
 // warps: 0 = TMA producer, 1 = MMA issuer, 2.. = epilogue.  GEMM-1 has 4 epilogue warps (its SwiGLU
 // epilogue needs ~200 registers per thread); the down projection has 8 -- two per TMEM lane quarter,
 // alternating 32-column blocks -- because with a short K loop (f = 768: 12 K steps per tile) one warp
@@ -85,6 +114,19 @@ constexpr size_t SPLIT_PART_BYTES = (size_t)SPLIT_MAX_UNITS * TN * 256 * sizeof(
 constexpr int SPLIT_COUNTERS = SPLIT_MAX_UNITS * 16;     // per tile: 2 CTA ranks x 8 epilogue-warp roles
 constexpr size_t SPLIT_WS_BYTES = SPLIT_PART_BYTES + 2 * (size_t)SPLIT_COUNTERS * sizeof(int);   // counters of GEMM-1, of GEMM-2
 
+// what the e4m3 kinds need beyond the bf16 kernel's arguments
+struct FfnAux {
+  CUtensorMap tmSFB;          // KIND_MXF8 token scales : u32 [K/128][32][Rb]
+  CUtensorMap tmSFW;          // KIND_MXF8 weight scales: u32 [chunks][128 words], one 512-byte chunk per (expert, K stage, CTA feature tile)
+  const float* row_scale;     // KIND_F8 GEMM-1: sx [R_cap]
+  const float* sw0;           // KIND_F8: per-expert weight scale (W1 | W2)
+  const float* sw1;           // KIND_F8 GEMM-1: W3's
+  const float* h_scale;       // KIND_F8: static per-expert scale of H
+  uint8_t* hsf;               // KIND_MXF8 GEMM-1: scales of H, written in the token-scale layout (K = f)
+  int Rb;                     // KIND_MXF8: words per (K stage, lane) row of the token-scale arrays
+  int wchunks;                // KIND_MXF8: weight chunks per (expert, K stage)
+};
+
 struct SmemTail {
   uint64_t full[STAGES];          // leader CTA: both CTAs' TMA bytes of a stage have landed
   uint64_t empty[STAGES];         // each CTA: the MMAs reading the stage have retired
@@ -98,7 +140,7 @@ struct SmemTail {
   int32_t cum[MAX_SLOTS + 1];     // exclusive prefix of token tiles per slot
   int32_t tsz[MAX_SLOTS];         // rows per token tile of the slot (multiple of 16, <= TN)
 };
-constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + sizeof(SmemTail);
+constexpr size_t SMEM_BYTES = 1024 + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + SX_BYTES + sizeof(SmemTail);
 static_assert(SMEM_BYTES <= 232448, "exceeds the 227 KB dynamic shared memory of sm_100");
 
 struct TileCursor {
@@ -179,22 +221,50 @@ __device__ __forceinline__ void store_block_T_scatter(const float (&v)[32], __nv
   }
 }
 
+// The same transposed store for an e4m3 output (GEMM-1 writes Hq): every lane packs its own two tokens
+// of its feature into an e4m3x2 halfword; one shuffle + byte permute give {token: features f, f+1}.
+__device__ __forceinline__ void store_block_T_e4m3(const float (&v)[32], uint8_t* __restrict__ out, size_t ld, int row0,
+                                                   int n_rows, int feat, bool feat_ok, int lane) {
+  const int odd = lane & 1;
+  const uint32_t sel = odd ? 0x0015u : 0x0040u;   // even: (own.b0, got.b0) = token i;  odd: (got.b1, own.b1) = token i+1
+  uint8_t* p = out + (size_t)(row0 + odd) * ld + (feat - odd);
+  const size_t step = 2 * ld;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    const uint32_t own = ptx::pack2_e4m3(v[i], v[i + 1]);
+    const uint32_t got = __shfl_xor_sync(0xffffffffu, own, 1);
+    const uint32_t pk = __byte_perm(own, got, sel);
+    if (feat_ok && i + odd < n_rows) *reinterpret_cast<uint16_t*>(p) = (uint16_t)pk;
+    p += step;
+  }
+}
+
+
 // kMode: 0 = gate|up + SwiGLU (GEMM-1), 1 = down (GEMM-2), 2 = down with the gate-weighted
-// scatter fused into the epilogue (vibe_grouped_ffn_scatter).
-template <int kMode>
+// scatter fused into the epilogue (vibe_grouped_ffn_scatter; KIND_BF16 only).  kKind: the operand kind (above).
+template <int kMode, int kKind>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(num_threads(kMode), 1)
 ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant__ CUtensorMap tmActN,
                 const __grid_constant__ CUtensorMap tmW0, const __grid_constant__ CUtensorMap tmW1, const int32_t* __restrict__ offsets, int E_loc,
-                int n_total, int k_total, __nv_bfloat16* __restrict__ out, int ld_out,
+                int n_total, int k_total, void* __restrict__ out_v, int ld_out,
                 const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w,
-                float* __restrict__ split_part /*NULL: no split-K*/, int* __restrict__ split_cnt) {
+                float* __restrict__ split_part /*NULL: no split-K*/, int* __restrict__ split_cnt,
+                const __grid_constant__ FfnAux aux) {
+  static_assert(kMode != 2 || kKind == KIND_BF16, "the fused scatter epilogue exists for the bf16 kind only");
   constexpr bool kGateUp = (kMode == 0);
+  constexpr bool kMx = (kKind == KIND_MXF8);
+  constexpr bool kF8 = (kKind == KIND_F8);
+  constexpr int BK = bk_of(kKind);          // K elements per smem stage
+  constexpr int UMMA_K = umma_k_of(kKind);
+  constexpr int TNk = tn_of(kKind);         // tokens per tile / TMEM columns per accumulator stage
+  constexpr int TALIGN = talign_of(kKind);  // block-scaled: token tiles start on an even scale-factor row block
   constexpr int FB = kGateUp ? 128 : 256;   // output features per pair tile
   constexpr int FC = FB / 2;                // ... per CTA
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   float* xchg = reinterpret_cast<float*>(smem + (size_t)STAGES * STAGE_BYTES);
-  SmemTail* tail = reinterpret_cast<SmemTail*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES);
+  float* sx_all = reinterpret_cast<float*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES);
+  SmemTail* tail = reinterpret_cast<SmemTail*>(smem + (size_t)STAGES * STAGE_BYTES + XCHG_BYTES + SX_BYTES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = ptx::cluster_ctarank();      // 0 = leader (issues the MMAs)
   const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
@@ -209,6 +279,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     ptx::prefetch_tensormap(&tmActN);
     ptx::prefetch_tensormap(&tmW0);
     if (kGateUp) ptx::prefetch_tensormap(&tmW1);
+    if (kMx) {
+      ptx::prefetch_tensormap(&aux.tmSFW);
+      ptx::prefetch_tensormap(&aux.tmSFB);
+    }
     for (int s = 0; s < STAGES; ++s) {
       ptx::mbar_init(ptx::smem_u32(&tail->full[s]), 1);
       ptx::mbar_init(ptx::smem_u32(&tail->empty[s]), 1);
@@ -238,8 +312,8 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       // (same token tile, other feature blocks) then run K steps of the same length and stay in
       // step, which is what lets L2 serve the second reader.  With a short last tile the readers
       // drift apart by more than L2 holds and DRAM traffic doubles (measured, profiles/).
-      const int nt = (hi - lo + TN - 1) / TN;
-      if (e < E_loc) tail->tsz[e] = nt > 0 ? ((((hi - lo + nt - 1) / nt) + 15) & ~15) : TN;
+      const int nt = (hi - lo + TNk - 1) / TNk;
+      if (e < E_loc) tail->tsz[e] = nt > 0 ? ((((hi - lo + nt - 1) / nt) + TALIGN - 1) & ~(TALIGN - 1)) : TNk;
       int inc = nt;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -316,7 +390,15 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         // a tile of at most 2 * NARROW_ROWS tokens loads the small activation box (4 KB instead of 16 KB a stage)
         const bool narrow = half <= NARROW_ROWS;
         const CUtensorMap* tm_b = narrow ? &tmActN : &tmAct;
-        const uint32_t tx_bytes = narrow ? 2u * (A_BYTES + NARROW_ROWS * BK * 2) : 2u * STAGE_BYTES;
+        // Block-scaled kind: the tile's token scales.  A TMA box must start on a 16-byte boundary of global
+        // memory (measured: a start at 4 or 8 bytes faults), i.e. on a multiple of 4 row blocks, while a tile starts
+        // on any EVEN row block: fetch the aligned {4 row blocks x 32 rows} chunks that cover the tile (at most 2)
+        // and point the MMA (rb0 & 3) = 0 or 2 columns into them (measured: the scale-factor TMEM address of the
+        // MMA and the destination of tcgen05.cp must be even columns -- an odd one raises "misaligned address").
+        const int rb0 = row0 >> 5;
+        const int sf_chunks = ((rb0 & 3) + ((half + 15) >> 4) + 3) >> 2;
+        const uint32_t tx_bytes = 2u * ((uint32_t)A_BYTES + (uint32_t)(narrow ? NARROW_ROWS * 128 : (kMx ? B_BYTES_MX : B_BYTES)) +
+                                        (kMx ? 512u + 512u * (uint32_t)sf_chunks : 0u));
         for (int kb = kb_lo; kb < kb_hi; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->empty[stage]), phase ^ 1u);
           if (ptx::elect_one()) {
@@ -325,31 +407,49 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
             const uint32_t a_s = smem_base + (uint32_t)stage * STAGE_BYTES;
             const uint32_t b_s = a_s + A_BYTES;
             const int k0 = kb * BK;
+            // weights: the bf16 tensors are [E_loc, K, N] (N innermost), the packed e4m3 ones [E_loc, N, K] (K innermost)
+            const int c0 = (kKind == KIND_BF16) ? n0 : k0, c1 = (kKind == KIND_BF16) ? k0 : n0;
+            const int d0 = (kKind == KIND_BF16) ? 64 : 0, d1 = (kKind == KIND_BF16) ? 0 : 64;     // the second 64-feature atom
             if (kGateUp) {
-              ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);                 // gate -> lanes 0..63
-              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, n0, k0, e, pol_w);    // up   -> lanes 64..127
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, c0, c1, e, pol_w);                 // gate -> lanes 0..63
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW1, full, c0, c1, e, pol_w);    // up   -> lanes 64..127
             } else {
-              ptx::tma_load_3d_2sm(a_s, &tmW0, full, n0, k0, e, pol_w);
-              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, n0 + 64, k0, e, pol_w);
+              ptx::tma_load_3d_2sm(a_s, &tmW0, full, c0, c1, e, pol_w);
+              ptx::tma_load_3d_2sm(a_s + ATOM_BYTES, &tmW0, full, c0 + d0, c1 + d1, e, pol_w);
             }
             ptx::tma_load_2d_2sm(b_s, tm_b, full, k0, row_b, pol_act);
+            if (kMx) {
+              const int wchunk = (e * KB + kb) * aux.wchunks + n0 / FC;
+              ptx::tma_load_2d_2sm(a_s + SFA_OFF, &aux.tmSFW, full, 0, wchunk, pol_w);
+              for (int c = 0; c < sf_chunks; ++c)
+                ptx::tma_load_3d_2sm(a_s + SFB_OFF + c * 512, &aux.tmSFB, full, (rb0 & ~3) + 4 * c, 0, kb, pol_act);
+            }
           }
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
-  } else if (warp == 1) {
+  }
+  else if (warp == 1) {
     // ================================================================ UMMA issuer (leader CTA)
     // The whole warp runs the loop; one elected lane issues the MMAs and the commits (always the
     // same lane: tcgen05.commit tracks the MMAs of the issuing thread).
     if (rank == 0) {
-      constexpr uint32_t idesc0 = ptx::make_idesc_bf16_f32(256, 0, /*a_mn=*/true, /*b_mn=*/false);
+      constexpr uint32_t idesc0 = kKind == KIND_BF16 ? ptx::make_idesc_bf16_f32(256, 0, /*a_mn=*/true, /*b_mn=*/false)
+                                  : kMx            ? ptx::make_idesc_mxe4m3(256, 0)
+                                                   : ptx::make_idesc_e4m3_f32(256, 0);
       // descriptor = constant high word | low word (start address >> 4 in bits [0,14), LBO in [16,30))
       constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+      // A: bf16 weights are MN-major SW128 (LBO = one 8 KB atom; a K step of 16 rows = 2 swizzle atoms of 1024 B),
+      //    packed e4m3 weights K-major SW128 (a K step of 32 elements = 32 bytes inside the 128-byte row);
+      // B: K-major SW128 for every kind (a K step = 32 bytes inside the row)
+      constexpr uint32_t A_LBO = (kKind == KIND_BF16) ? (uint32_t)(ATOM_BYTES >> 4) : (16u >> 4);
+      constexpr uint32_t A_KSTEP = (kKind == KIND_BF16) ? (uint32_t)(UMMA_K * 128 / 16) : 2u;
       const uint32_t smem_base = ptx::smem_u32(smem);
-      const uint32_t a_lo0 = ((smem_base >> 4) & 0x3fffu) | ((uint32_t)(ATOM_BYTES >> 4) << 16);
+      const uint32_t a_lo0 = ((smem_base >> 4) & 0x3fffu) | (A_LBO << 16);
       const uint32_t b_lo0 = (((smem_base + A_BYTES) >> 4) & 0x3fffu) | ((16u >> 4) << 16);
+      const uint32_t sfa_t = tmem_base + SF_TMEM_COL, sfb_t = tmem_base + SF_TMEM_COL + 4;
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
@@ -363,27 +463,41 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         cur.decode(tail, tile, NB, f_blk, t_blk);
         const int e = cur.e;
         const int tsz = tail->tsz[e];
-        const int n_rows = min(tsz, tail->off[e + 1] - (tail->off[e] + t_blk * tsz));
+        const int row0 = tail->off[e] + t_blk * tsz;
+        const int n_rows = min(tsz, tail->off[e + 1] - row0);
         const uint32_t n_mma = (uint32_t)((n_rows + 15) >> 4) << 4;
         const uint32_t idesc = idesc0 | ((n_mma >> 3) << 17);
+        const uint32_t sf_shift = (uint32_t)(row0 >> 5) & 3u;                    // columns into the aligned scale chunks
+        const int sf_chunks = (int)((sf_shift + ((n_mma + 31) >> 5) + 3) >> 2);
         const int acc = it & 1;
         const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
         ptx::mbar_wait(ptx::smem_u32(&tail->tempty[acc]), acc_phase ^ 1u);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)acc * TN;
+        const uint32_t d_tmem = tmem_base + (uint32_t)acc * TNk;
         for (int kb = kb_lo; kb < kb_hi; ++kb) {
           ptx::mbar_wait(ptx::smem_u32(&tail->full[stage]), phase);
           ptx::tc_fence_after();
           if (ptx::elect_one()) {
-            // A: MN-major SW128 -> 16 K-rows = 2 swizzle atoms of 1024 B (+128 in units of 16 B);
-            // B: K-major SW128 -> 16 elements = 32 bytes inside the 128-byte row (+2)
+            if (kMx) {
+              // this stage's scale factors: shared memory -> TMEM of both CTAs, ahead of (and ordered with) its MMAs
+              const uint32_t sf_s = smem_base + (uint32_t)stage * STAGE_BYTES;
+              ptx::tmem_cp_32x128b_warpx4_2sm(sfa_t, ptx::make_smem_desc_rows16(sf_s + SFA_OFF));
+              for (int c = 0; c < sf_chunks; ++c)
+                ptx::tmem_cp_32x128b_warpx4_2sm(sfb_t + 4u * (uint32_t)c, ptx::make_smem_desc_rows16(sf_s + SFB_OFF + 512u * (uint32_t)c));
+            }
             const uint32_t a_lo = a_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
             const uint32_t b_lo = b_lo0 + (uint32_t)stage * (STAGE_BYTES >> 4);
 #pragma unroll
             for (int k = 0; k < BK / UMMA_K; ++k) {
-              const uint64_t da = ((uint64_t)DESC_HI << 32) | (uint64_t)(a_lo + (uint32_t)k * (UMMA_K * 128 / 16));
-              const uint64_t db = ((uint64_t)DESC_HI << 32) | (uint64_t)(b_lo + (uint32_t)k * (UMMA_K * 2 / 16));
-              ptx::umma_bf16_2sm(d_tmem, da, db, idesc, (uint32_t)((kb > kb_lo) | (k != 0)));
+              const uint64_t da = ((uint64_t)DESC_HI << 32) | (uint64_t)(a_lo + (uint32_t)k * A_KSTEP);
+              const uint64_t db = ((uint64_t)DESC_HI << 32) | (uint64_t)(b_lo + (uint32_t)k * 2u);
+              const uint32_t accum = (uint32_t)((kb > kb_lo) | (k != 0));
+              if (kKind == KIND_BF16)
+                ptx::umma_bf16_2sm(d_tmem, da, db, idesc, accum);
+              else if (kMx)
+                ptx::umma_mxf8_2sm(d_tmem, da, db, idesc | ((uint32_t)k << 29) | ((uint32_t)k << 4), accum, sfa_t, sfb_t + sf_shift);
+              else
+                ptx::umma_f8_2sm(d_tmem, da, db, idesc, accum);
             }
             ptx::umma_commit_2sm_mc(ptx::smem_u32(&tail->empty[stage]), 3);   // frees the stage in both CTAs
             if (kb == kb_hi - 1)
@@ -394,8 +508,9 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         }
       }
     }
-  } else {
-    // ================================================================ epilogue (warps 2..5, both CTAs)
+  }
+  else {
+    // ================================================================ epilogue (warps 2.., both CTAs)
     const int q = warp & 3;  // TMEM lane quarter this warp may access
     const int blk_par = (warp - 2) >> 2;   // down projection: which 32-column blocks (even / odd) are mine
     TileCursor cur;
@@ -426,9 +541,75 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
         }
         __syncwarp();
       }
+      // KIND_F8 GEMM-1: the tile's row scales sx go to this warp's slice while the MMAs of the tile still run
+      float* sx = sx_all + (warp - 2) * TN;
+      if (kF8 && kGateUp) {
+        __syncwarp();
+#pragma unroll
+        for (int b = 0; b < TN / 32; ++b) {
+          const int c = b * 32 + lane;
+          sx[c] = (c < n_rows) ? __ldg(aux.row_scale + row0 + c) : 0.0f;
+        }
+        __syncwarp();
+      }
+      const float se0 = kF8 ? __ldg(aux.sw0 + e) : 1.0f;
+      const float se1 = (kF8 && kGateUp) ? __ldg(aux.sw1 + e) : 1.0f;
+      const float she = kF8 ? __ldg(aux.h_scale + e) : 1.0f;
+      const float inv_sh = kF8 ? 1.0f / she : 1.0f;
+      // lanes 0..63 gate (q = 0,1), lanes 64..127 up (q = 2,3) of the same 64 features (GEMM-1); 128 features (GEMM-2)
+      const int feat = kGateUp ? f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane : f_blk * FB + (int)rank * FC + q * 32 + lane;
+      const bool feat_ok = feat < n_total;
+
+      // ---- what a kind does with finished accumulator values -------------------------------------------------
+      // GEMM-1, one element: the accumulators (gate, up) of token column `col` -> the value stored for H
+      auto h_of = [&](float g, float u, int col) -> float {
+        if (kF8) {
+          const float sxi = sx[col];
+          return swiglu(g * (sxi * se0), u * (sxi * se1)) * inv_sh;
+        }
+        return swiglu(g, u);       // KIND_MXF8: the block scales were applied by the tensor core
+      };
+      // GEMM-1, a finished 32-feature x 32-token block of H (h[i] = token column cbase + i of this lane's feature)
+      auto store_h = [&](float (&h)[32], int cbase) {
+        if (kMx) {
+          // Q7: this warp's 32 lanes are the 32 features of ONE scale block of H.  Per token column: the block's
+          // absmax (non-negative floats order like their bit patterns: one redux.sync), e = smallest exponent
+          // with amax <= 448 * 2^e (448 = 1.75 * 2^8: e = x - 8, +1 if the mantissa exceeds 1.75), the exact
+          // division by 2^e as a multiplication, and lane i keeps the byte of column i.
+          uint32_t my_byte = 127u;
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const uint32_t bits = __reduce_max_sync(0xffffffffu, __float_as_uint(fabsf(h[i])));
+            int ex = (int)(bits >> 23) - 127 - 8 + ((bits & 0x7fffffu) > 0x600000u ? 1 : 0);
+            ex = bits == 0u ? 0 : max(ex, -127);
+            h[i] *= __uint_as_float((uint32_t)(127 - ex) << 23);
+            if (lane == i) my_byte = (uint32_t)(ex + 127);
+          }
+          const int r = row0 + cbase + lane;
+          const int fb = feat >> 5;      // warp-uniform
+          if (feat_ok && cbase + lane < n_rows)
+            aux.hsf[((size_t)((fb >> 2) * 32 + (r & 31)) * (size_t)aux.Rb + (size_t)(r >> 5)) * 4 + (size_t)(fb & 3)] = (uint8_t)my_byte;
+        }
+        if (kKind == KIND_BF16)
+          store_block_T(h, reinterpret_cast<__nv_bfloat16*>(out_v), (size_t)ld_out, row0 + cbase, n_rows - cbase, feat, feat_ok, lane);
+        else
+          store_block_T_e4m3(h, reinterpret_cast<uint8_t*>(out_v), (size_t)ld_out, row0 + cbase, n_rows - cbase, feat, feat_ok, lane);
+      };
+      // GEMM-2, a finished 32-feature x 32-token block of Y
+      auto store_y = [&](float (&v)[32], int c0) {
+        if (kF8) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) v[i] *= she * se0;
+        }
+        if (kMode == 2)
+          store_block_T_scatter(v, reinterpret_cast<__nv_bfloat16*>(out_v), (size_t)ld_out, feat, feat_ok, lane, sc_wt + c0, sc_asg + c0);
+        else
+          store_block_T(v, reinterpret_cast<__nv_bfloat16*>(out_v), (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+      };
+
       ptx::mbar_wait(ptx::smem_u32(&tail->tfull[acc]), acc_phase);
       ptx::tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TN;
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)acc * TNk;
       if (is_split) {
         // ------------------------------------------------------------ split-K unit
         // (1) dump this warp's part of the fp32 accumulator: part[unit][column][rank * 128 + TMEM lane]
@@ -460,8 +641,6 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
           // (3) sum the S partials in slice order, then the normal epilogue on the sum
           const float* p0 = split_part + ((size_t)(tile - split_from) * S * TN) * 256 + rank * 128;
           if (kGateUp) {
-            const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
-            const bool feat_ok = feat < n_total;
             const float* pg = p0 + (q & 1) * 32 + lane;        // gate: TMEM lanes 0..63, up: the same feature + 64
             for (int c0 = 0; c0 < n_rows; c0 += 32) {
               // slice loop OUTSIDE, the 32 columns unrolled inside: 64 independent L2 loads in flight per slice
@@ -477,12 +656,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
                 }
               }
 #pragma unroll
-              for (int i = 0; i < 32; ++i) g[i] = swiglu(g[i], u[i]);
-              store_block_T(g, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+              for (int i = 0; i < 32; ++i) g[i] = h_of(g[i], u[i], c0 + i);
+              store_h(g, c0);
             }
           } else {
-            const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
-            const bool feat_ok = feat < n_total;
             const float* pv = p0 + q * 32 + lane;
             for (int c0 = blk_par * 32; c0 < n_rows; c0 += 64) {
               float v[32];
@@ -493,22 +670,16 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 #pragma unroll
                 for (int i = 0; i < 32; ++i) v[i] += __ldcg(pc + (size_t)i * 256);
               }
-              if (kMode == 2)
-                store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_wt + c0, sc_asg + c0);
-              else
-                store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+              store_y(v, c0);
             }
           }
         }
         continue;
       }
       if (kGateUp) {
-        // lanes 0..63 gate (q = 0,1), lanes 64..127 up (q = 2,3) of the same 64 features.
         // Per 64 columns: the gate warp finishes columns 0..31 (needs the partner's up block),
         // the up warp finishes columns 32..63 (needs the partner's gate block).
         const bool is_up = q >= 2;
-        const int feat = f_blk * FB + (int)rank * FC + (q & 1) * 32 + lane;
-        const bool feat_ok = feat < n_total;
         float* mine = xchg + ((q & 1) * 2 + (is_up ? 1 : 0)) * 1024;      // block I publish  [col][lane]
         float* theirs = xchg + ((q & 1) * 2 + (is_up ? 0 : 1)) * 1024;    // block my partner publishes
         const uint32_t bar_id = 1 + (q & 1);
@@ -521,21 +692,19 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 #pragma unroll
           for (int i = 0; i < 32; ++i) mine[i * 32 + lane] = __uint_as_float(is_up ? a[i] : b[i]);
           ptx::named_bar_sync(bar_id, 64);
+          const int cbase = c0 + (is_up ? 32 : 0);
           float h[32];
 #pragma unroll
           for (int i = 0; i < 32; ++i) {
             const float o = theirs[i * 32 + lane];
-            h[i] = is_up ? swiglu(o, __uint_as_float(b[i])) : swiglu(__uint_as_float(a[i]), o);
+            h[i] = is_up ? h_of(o, __uint_as_float(b[i]), cbase + i) : h_of(__uint_as_float(a[i]), o, cbase + i);
           }
           ptx::named_bar_sync(bar_id, 64);     // both blocks consumed before the next publish
-          const int cbase = c0 + (is_up ? 32 : 0);
-          store_block_T(h, out, (size_t)ld_out, row0 + cbase, n_rows - cbase, feat, feat_ok, lane);
+          store_h(h, cbase);
         }
       } else {
-        const int feat = f_blk * FB + (int)rank * FC + q * 32 + lane;
-        const bool feat_ok = feat < n_total;
 #pragma unroll
-        for (int b = 0; b < TN / 32; ++b) {
+        for (int b = 0; b < TNk / 32; ++b) {
           const int c0 = b * 32;
           if (c0 >= n_rows) break;
           if ((b & 1) != blk_par) continue;
@@ -545,10 +714,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
           float v[32];
 #pragma unroll
           for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(a[i]);
-          if (kMode == 2)
-            store_block_T_scatter(v, out, (size_t)ld_out, feat, feat_ok, lane, sc_wt + c0, sc_asg + c0);
-          else
-            store_block_T(v, out, (size_t)ld_out, row0 + c0, n_rows - c0, feat, feat_ok, lane);
+          store_y(v, c0);
         }
       }
       ptx::tc_fence_before();
@@ -571,7 +737,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
 // ---------------------------------------------------------------------------------------
 // TMA tensor maps (host).  cuTensorMapEncodeTiled is a driver entry point fetched through
 // the runtime, so libvibe.so does not link libcuda.  Maps are cached for the process
-// lifetime, keyed by (pointer, shape): weights and workspaces are long-lived in serving.
+// lifetime, keyed by (pointer, shape, element type): weights and workspaces are long-lived in serving.
 // ---------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -590,12 +756,17 @@ EncodeTiledFn get_encode_fn() {
   return fn;
 }
 
+// element types of the maps: bf16 and one-byte operands with the 128-byte swizzle; 32-bit words without
+// swizzle (the scale-factor arrays of the block-scaled kind)
+enum MapElem { ELEM_BF16 = 0, ELEM_U8 = 1, ELEM_WORDS = 2 };
+
 struct MapKey {
   const void* ptr;
   uint64_t d0, d1, d2;
   uint32_t b0, b1;
+  int elem;
   bool operator==(const MapKey& o) const {
-    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1;
+    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && d2 == o.d2 && b0 == o.b0 && b1 == o.b1 && elem == o.elem;
   }
 };
 struct MapKeyHash {
@@ -605,16 +776,17 @@ struct MapKeyHash {
     h = h * 1315423911u ^ k.d1;
     h = h * 1315423911u ^ k.d2;
     h = h * 1315423911u ^ ((uint64_t)k.b0 << 32 | k.b1);
+    h = h * 1315423911u ^ (size_t)k.elem;
     return h;
   }
 };
 std::mutex g_map_mu;
 std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
 
-// rank 2: dims (d0 inner, d1); rank 3: dims (d0 inner, d1, d2).  bf16, 128-byte swizzle.
-vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t box0, uint32_t box1,
+// rank 2: dims (d0 inner, d1); rank 3: dims (d0 inner, d1, d2)
+vibe_status get_tensor_map(MapElem elem, const void* ptr, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t box0, uint32_t box1,
                            CUtensorMap* out) {
-  MapKey key{ptr, d0, d1, d2, box0, box1};
+  MapKey key{ptr, d0, d1, d2, box0, box1, (int)elem};
   {
     std::lock_guard<std::mutex> lk(g_map_mu);
     auto it = g_maps.find(key);
@@ -626,14 +798,18 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
   EncodeTiledFn enc = get_encode_fn();
   VIBE_REQUIRE(enc != nullptr, VIBE_ERR_CUDA, "cuTensorMapEncodeTiled entry point unavailable (no CUDA driver?)");
   const bool r3 = d2 > 0;
+  const uint64_t esz = elem == ELEM_BF16 ? 2 : elem == ELEM_U8 ? 1 : 4;
   cuuint64_t dims[3] = {d0, d1, r3 ? d2 : 1};
-  cuuint64_t strides[2] = {d0 * 2, d0 * d1 * 2};
+  cuuint64_t strides[2] = {d0 * esz, d0 * d1 * esz};
   cuuint32_t box[3] = {box0, box1, 1};
   cuuint32_t estr[3] = {1, 1, 1};
   CUtensorMap m;
-  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, r3 ? 3 : 2, const_cast<void*>(ptr), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  const CUtensorMapDataType dt = elem == ELEM_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                 : elem == ELEM_U8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8
+                                                   : CU_TENSOR_MAP_DATA_TYPE_UINT32;
+  CUresult r = enc(&m, dt, r3 ? 3 : 2, const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   elem == ELEM_WORDS ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   VIBE_REQUIRE(r == CUDA_SUCCESS, VIBE_ERR_CUDA,
                "cuTensorMapEncodeTiled failed (CUresult %d) ptr=%p dims=(%llu,%llu,%llu) box=(%u,%u)", (int)r, ptr,
                (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2, box0, box1);
@@ -646,6 +822,64 @@ vibe_status get_tensor_map(const void* ptr, uint64_t d0, uint64_t d1, uint64_t d
   return VIBE_OK;
 }
 
+// the opt-in to > 48 KB of dynamic shared memory is per device: once for each device this process uses
+vibe_status set_smem_attrs() {
+  static std::mutex mu;
+  static bool done[kMaxDevices] = {};
+  const int dev = current_device();
+  std::lock_guard<std::mutex> lk(mu);
+  if (done[dev]) return VIBE_OK;
+  const int b = (int)SMEM_BYTES;
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<0, KIND_BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<1, KIND_BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<2, KIND_BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<0, KIND_F8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<1, KIND_F8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<0, KIND_MXF8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<1, KIND_MXF8>, cudaFuncAttributeMaxDynamicSharedMemorySize, b));
+  done[dev] = true;
+  return VIBE_OK;
+}
+
+// split-K workspace of a call: partial buffer + the counters of the two launches (NULL pointers: split-K off)
+struct SplitWs {
+  float* part = nullptr;
+  int* cnt1 = nullptr;
+  int* cnt2 = nullptr;
+};
+vibe_status split_ws(void* ws, size_t ws_bytes, bool ws_zeroed, cudaStream_t st, SplitWs* out) {
+  if (ws != nullptr && ws_bytes >= SPLIT_WS_BYTES && (reinterpret_cast<uintptr_t>(ws) & 15u) == 0) {
+    out->part = reinterpret_cast<float*>(ws);
+    out->cnt1 = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES);
+    out->cnt2 = out->cnt1 + SPLIT_COUNTERS;
+    if (!ws_zeroed) VIBE_CUDA(cudaMemsetAsync(out->cnt1, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
+  }
+  return VIBE_OK;
+}
+
+// the two launches of one FFN: gate|up + SwiGLU, then down (kDownMode = 1, or 2 with the fused scatter)
+template <int kKind, int kDownMode>
+vibe_status launch_pair(const CUtensorMap& tmX, const CUtensorMap& tmXN, const CUtensorMap& tmW1, const CUtensorMap& tmW3,
+                        const CUtensorMap& tmH, const CUtensorMap& tmHN, const CUtensorMap& tmW2, const int32_t* offsets,
+                        int E_loc, int d, int f, void* H, void* Y, const int32_t* row_to_assign, const float* topk_w,
+                        const SplitWs& sw, const FfnAux& aux1, const FfnAux& aux2, cudaStream_t st) {
+  vibe_status sa = set_smem_attrs();
+  if (sa != VIBE_OK) return sa;
+  const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
+  // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
+  const int32_t* no_map = nullptr;
+  const float* no_w = nullptr;
+  cudaError_t le = launch_pdl(ffn_gemm_kernel<0, kKind>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
+                              offsets, E_loc, f, d, H, f, no_map, no_w, sw.part, sw.cnt1, aux1);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
+  VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
+  le = launch_pdl(ffn_gemm_kernel<kDownMode, kKind>, dim3(grid), dim3(num_threads(kDownMode)), SMEM_BYTES, st, tmH, tmHN, tmW2,
+                  tmW2, offsets, E_loc, d, f, Y, d, row_to_assign, topk_w, sw.part, sw.cnt2, aux2);
+  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
+  VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
+  return VIBE_OK;
+}
+
 }  // namespace
 
 size_t grouped_ffn_ws_bytes() { return SPLIT_WS_BYTES; }
@@ -655,60 +889,90 @@ vibe_status grouped_ffn_zero_counters(void* ws, cudaStream_t st) {
 }
 
 // ws (may be NULL or short: split-K is then off): SPLIT_WS_BYTES bytes; ws_zeroed: the caller has already zeroed the
-// counters behind the partial buffer on this stream (the layer entry does it before the route kernel so that no
+// counters behind the partial buffer on this stream (the layer entries do it before the route kernel so that no
 // memset sits between the permutation and the FFN kernels, which are chained by programmatic dependent launch)
 vibe_status grouped_ffn_impl(const void* Xp, const int32_t* offsets, int E_loc, int R_cap, int d, int f,
                              const void* W1, const void* W3, const void* W2, void* H_ws, void* Y,
                              cudaStream_t st, const int32_t* row_to_assign, const float* topk_w, void* ws,
                              size_t ws_bytes, bool ws_zeroed) {
+  constexpr int BK = bk_of(KIND_BF16);
   CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
   vibe_status s;
-  if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(Xp, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(H_ws, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(W1, f, d, E_loc, 64, BK, &tmW1)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(W3, f, d, E_loc, 64, BK, &tmW3)) != VIBE_OK) return s;
-  if ((s = get_tensor_map(W2, d, f, E_loc, 64, BK, &tmW2)) != VIBE_OK) return s;
-  {
-    // the opt-in to > 48 KB of dynamic shared memory is per device: once for each device this process uses
-    static std::mutex mu;
-    static bool done[kMaxDevices] = {};
-    const int dev = current_device();
-    std::lock_guard<std::mutex> lk(mu);
-    if (!done[dev]) {
-      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-      VIBE_CUDA(cudaFuncSetAttribute(ffn_gemm_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-      done[dev] = true;
-    }
-  }
-  const int grid = num_sms() & ~1;   // CTA pairs (clusters of 2)
-  // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
-  const int32_t* no_map = nullptr;
-  const float* no_w = nullptr;
-  float* part = nullptr;
-  int* cnt1 = nullptr;
-  int* cnt2 = nullptr;
-  if (ws != nullptr && ws_bytes >= SPLIT_WS_BYTES && (reinterpret_cast<uintptr_t>(ws) & 15u) == 0) {
-    part = reinterpret_cast<float*>(ws);
-    cnt1 = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES);
-    cnt2 = cnt1 + SPLIT_COUNTERS;
-    if (!ws_zeroed) VIBE_CUDA(cudaMemsetAsync(cnt1, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
-  }
-  cudaError_t le = launch_pdl(ffn_gemm_kernel<0>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
-                              offsets, E_loc, f, d, reinterpret_cast<__nv_bfloat16*>(H_ws), f, no_map, no_w, part, cnt1);
-  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
-  VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
+  // activations [R_cap, K] K innermost: boxes of 64 K x (128 | 32) rows; weights [E_loc, K, N] N innermost: 64 N x 64 K
+  if ((s = get_tensor_map(ELEM_BF16, Xp, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, H_ws, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, Xp, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, H_ws, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, W1, f, d, E_loc, 64, BK, &tmW1)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, W3, f, d, E_loc, 64, BK, &tmW3)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_BF16, W2, d, f, E_loc, 64, BK, &tmW2)) != VIBE_OK) return s;
+  SplitWs sw;
+  if ((s = split_ws(ws, ws_bytes, ws_zeroed, st, &sw)) != VIBE_OK) return s;
+  const FfnAux none{};
   if (row_to_assign != nullptr)
-    le = launch_pdl(ffn_gemm_kernel<2>, dim3(grid), dim3(num_threads(2)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
-                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, row_to_assign, topk_w, part, cnt2);
-  else
-    le = launch_pdl(ffn_gemm_kernel<1>, dim3(grid), dim3(num_threads(1)), SMEM_BYTES, st, tmH, tmHN, tmW2, tmW2, offsets,
-                    E_loc, d, f, reinterpret_cast<__nv_bfloat16*>(Y), d, no_map, no_w, part, cnt2);
-  VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
-  VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
-  return VIBE_OK;
+    return launch_pair<KIND_BF16, 2>(tmX, tmXN, tmW1, tmW3, tmH, tmHN, tmW2, offsets, E_loc, d, f, H_ws, Y, row_to_assign, topk_w,
+                                     sw, none, none, st);
+  return launch_pair<KIND_BF16, 1>(tmX, tmXN, tmW1, tmW3, tmH, tmHN, tmW2, offsets, E_loc, d, f, H_ws, Y, nullptr, nullptr, sw,
+                                   none, none, st);
+}
+
+// KIND_F8 (readings Q1-Q4): packed weights [E_loc, N, K] (K innermost), per-row / per-expert / static H scales
+vibe_status grouped_ffn_fp8_impl(const void* Xq, const float* row_scale, const int32_t* offsets, int E_loc, int R_cap,
+                                 int d, int f, const void* W1q, const float* s1, const void* W3q, const float* s3,
+                                 const void* W2q, const float* s2, const float* h_scale, void* Hq, void* Y,
+                                 cudaStream_t st, void* ws, size_t ws_bytes, bool ws_zeroed) {
+  constexpr int BK = bk_of(KIND_F8);
+  CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
+  vibe_status s;
+  if ((s = get_tensor_map(ELEM_U8, Xq, d, R_cap, 0, BK, TN / 2, &tmX)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Hq, f, R_cap, 0, BK, TN / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Xq, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Hq, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W1q, d, f, E_loc, BK, 64, &tmW1)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W3q, d, f, E_loc, BK, 64, &tmW3)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W2q, f, d, E_loc, BK, 64, &tmW2)) != VIBE_OK) return s;
+  SplitWs sw;
+  if ((s = split_ws(ws, ws_bytes, ws_zeroed, st, &sw)) != VIBE_OK) return s;
+  FfnAux a1{}, a2{};
+  a1.row_scale = row_scale;
+  a1.sw0 = s1;
+  a1.sw1 = s3;
+  a1.h_scale = a2.h_scale = h_scale;
+  a2.sw0 = s2;
+  return launch_pair<KIND_F8, 1>(tmX, tmXN, tmW1, tmW3, tmH, tmHN, tmW2, offsets, E_loc, d, f, Hq, Y, nullptr, nullptr, sw, a1, a2, st);
+}
+
+// KIND_MXF8 (readings Q5-Q8).  sf13: joint gate|up weight scales (one 512-byte chunk per expert, K stage and 64
+// features: TMEM rows 0..63 = W1's, 64..127 = W3's); sf2: down-projection weight scales (chunk per 128 features);
+// xsf / hsf: token scales [K/128][32][Rb] words (hsf is written by GEMM-1 and read by GEMM-2).
+vibe_status grouped_ffn_mxfp8_impl(const void* Xq, const void* xsf, const int32_t* offsets, int E_loc, int R_cap, int d,
+                                   int f, const void* W1q, const void* W3q, const void* sf13, const void* W2q,
+                                   const void* sf2, void* Hq, void* hsf, void* Y, cudaStream_t st, void* ws,
+                                   size_t ws_bytes, bool ws_zeroed) {
+  constexpr int BK = bk_of(KIND_MXF8);
+  constexpr int TNM = tn_of(KIND_MXF8);
+  CUtensorMap tmX, tmH, tmXN, tmHN, tmW1, tmW3, tmW2;
+  FfnAux a1{}, a2{};
+  vibe_status s;
+  const int Rb = mx_row_blocks(R_cap);
+  if ((s = get_tensor_map(ELEM_U8, Xq, d, R_cap, 0, BK, TNM / 2, &tmX)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Hq, f, R_cap, 0, BK, TNM / 2, &tmH)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Xq, d, R_cap, 0, BK, NARROW_ROWS, &tmXN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, Hq, f, R_cap, 0, BK, NARROW_ROWS, &tmHN)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W1q, d, f, E_loc, BK, 64, &tmW1)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W3q, d, f, E_loc, BK, 64, &tmW3)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_U8, W2q, f, d, E_loc, BK, 64, &tmW2)) != VIBE_OK) return s;
+  a1.wchunks = f / 64;
+  a2.wchunks = d / 128;
+  if ((s = get_tensor_map(ELEM_WORDS, sf13, 128, (uint64_t)E_loc * (d / BK) * a1.wchunks, 0, 128, 1, &a1.tmSFW)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_WORDS, sf2, 128, (uint64_t)E_loc * (f / BK) * a2.wchunks, 0, 128, 1, &a2.tmSFW)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_WORDS, xsf, Rb, 32, d / BK, 4, 32, &a1.tmSFB)) != VIBE_OK) return s;
+  if ((s = get_tensor_map(ELEM_WORDS, hsf, Rb, 32, f / BK, 4, 32, &a2.tmSFB)) != VIBE_OK) return s;
+  a1.hsf = reinterpret_cast<uint8_t*>(hsf);
+  a1.Rb = a2.Rb = Rb;
+  SplitWs sw;
+  if ((s = split_ws(ws, ws_bytes, ws_zeroed, st, &sw)) != VIBE_OK) return s;
+  return launch_pair<KIND_MXF8, 1>(tmX, tmXN, tmW1, tmW3, tmH, tmHN, tmW2, offsets, E_loc, d, f, Hq, Y, nullptr, nullptr, sw, a1, a2, st);
 }
 
 // the shape / alignment limits of the FFN kernels, checkable before anything is enqueued (the layer entry points
@@ -758,4 +1022,44 @@ extern "C" vibe_status vibe_grouped_ffn_scatter(const void* Xp, const int32_t* o
   VIBE_REQUIRE(row_to_assign && topk_w, VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_scatter: NULL row_to_assign / topk_w");
   return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H_ws, Yw,
                           reinterpret_cast<cudaStream_t>(stream), row_to_assign, topk_w, ws, ws_bytes, false);
+}
+
+extern "C" vibe_status vibe_grouped_ffn_fp8(const void* Xq, const float* row_scale, const int32_t* offsets,
+                                            int32_t E_loc, int32_t R_cap, int32_t d, int32_t f, const void* W1q,
+                                            const float* s1, const void* W3q, const float* s3, const void* W2q,
+                                            const float* s2, const float* h_scale, void* Hq_ws, void* Y,
+                                            void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(E_loc >= 1 && R_cap >= 1 && d >= 1 && f >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_grouped_ffn_fp8: bad sizes E_loc=%d R_cap=%d d=%d f=%d", E_loc, R_cap, d, f);
+  VIBE_REQUIRE(Xq && row_scale && offsets && W1q && s1 && W3q && s3 && W2q && s2 && h_scale && Hq_ws && Y,
+               VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_fp8: NULL argument");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0, VIBE_ERR_UNSUPPORTED,
+               "vibe_grouped_ffn_fp8: d and f must be multiples of 128 (d=%d f=%d)", d, f);
+  VIBE_REQUIRE(E_loc <= MAX_SLOTS, VIBE_ERR_UNSUPPORTED, "vibe_grouped_ffn_fp8: E_loc > %d not implemented", MAX_SLOTS);
+  VIBE_REQUIRE(aligned16(Xq) && aligned16(W1q) && aligned16(W3q) && aligned16(W2q) && aligned16(Hq_ws) && aligned16(Y),
+               VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_fp8: all tensors must be 16-byte aligned");
+  return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq_ws, Y,
+                              reinterpret_cast<cudaStream_t>(stream), nullptr, 0, false);
+}
+
+extern "C" vibe_status vibe_grouped_ffn_mxfp8(const void* Xq, const void* Xsf, const int32_t* offsets, int32_t E_loc,
+                                              int32_t R_cap, int32_t d, int32_t f, const void* W1q, const void* W3q,
+                                              const void* sf13, const void* W2q, const void* sf2, void* Hq_ws,
+                                              void* Hsf_ws, void* Y, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(E_loc >= 1 && R_cap >= 1 && d >= 1 && f >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_grouped_ffn_mxfp8: bad sizes E_loc=%d R_cap=%d d=%d f=%d", E_loc, R_cap, d, f);
+  VIBE_REQUIRE(Xq && Xsf && offsets && W1q && W3q && sf13 && W2q && sf2 && Hq_ws && Hsf_ws && Y, VIBE_ERR_INVALID_ARG,
+               "vibe_grouped_ffn_mxfp8: NULL argument");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0, VIBE_ERR_UNSUPPORTED,
+               "vibe_grouped_ffn_mxfp8: d and f must be multiples of 128 (d=%d f=%d)", d, f);
+  VIBE_REQUIRE(E_loc <= MAX_SLOTS, VIBE_ERR_UNSUPPORTED, "vibe_grouped_ffn_mxfp8: E_loc > %d not implemented", MAX_SLOTS);
+  VIBE_REQUIRE(aligned16(Xq) && aligned16(Xsf) && aligned16(W1q) && aligned16(W3q) && aligned16(sf13) && aligned16(W2q) &&
+                   aligned16(sf2) && aligned16(Hq_ws) && aligned16(Hsf_ws) && aligned16(Y),
+               VIBE_ERR_INVALID_ARG, "vibe_grouped_ffn_mxfp8: all tensors must be 16-byte aligned");
+  return grouped_ffn_mxfp8_impl(Xq, Xsf, offsets, E_loc, R_cap, d, f, W1q, W3q, sf13, W2q, sf2, Hq_ws, Hsf_ws, Y,
+                                reinterpret_cast<cudaStream_t>(stream), nullptr, 0, false);
 }

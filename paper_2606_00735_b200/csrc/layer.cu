@@ -363,6 +363,7 @@ extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, con
   float* tok_scale = reinterpret_cast<float*>(base + a.tok_scale);
   float* row_scale = reinterpret_cast<float*>(base + a.row_scale);
   vibe_status s;
+  if (T > 0 && (s = grouped_ffn_zero_counters(base + a.ffn_ws, reinterpret_cast<cudaStream_t>(stream))) != VIBE_OK) return s;
   if ((s = vibe_route_topk(cfg, logits, T, ids, w, counts, stream)) != VIBE_OK) return s;
   // tokens are quantised BEFORE the permutation (T rows instead of T*k), and the permutation then moves
   // one-byte elements: to vibe_permute an e4m3 row of d bytes is a bf16 row of d/2 elements
@@ -378,8 +379,9 @@ extern "C" vibe_status vibe_moe_layer_forward_fp8(const vibe_route_cfg* cfg, con
   if ((s = fp8_gather_row_scales(tok_scale, r2a, offsets, E_loc, k, (int)a.R_cap, row_scale,
                                  reinterpret_cast<cudaStream_t>(stream))) != VIBE_OK)
     return s;
-  if ((s = vibe_grouped_ffn_fp8(base + a.Xpq, row_scale, offsets, E_loc, (int32_t)a.R_cap, d, f, W1q, s1, W3q, s3, W2q,
-                                s2, h_scale, base + a.Hq, base + a.Y, stream)) != VIBE_OK)
+  if ((s = grouped_ffn_fp8_impl(base + a.Xpq, row_scale, offsets, E_loc, (int)a.R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale,
+                                base + a.Hq, base + a.Y, reinterpret_cast<cudaStream_t>(stream), base + a.ffn_ws,
+                                grouped_ffn_ws_bytes(), true)) != VIBE_OK)
     return s;
   return vibe_combine(base + a.Y, a2r, w, T, k, d, out, stream);
 }
@@ -415,6 +417,7 @@ extern "C" vibe_status vibe_moe_layer_forward_mxfp8(const vibe_route_cfg* cfg, c
   int32_t* a2r = reinterpret_cast<int32_t*>(base + a.a2r);
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   vibe_status s;
+  if (T > 0 && (s = grouped_ffn_zero_counters(base + a.ffn_ws, st)) != VIBE_OK) return s;
   if ((s = vibe_route_topk(cfg, logits, T, ids, w, counts, stream)) != VIBE_OK) return s;
   // tokens are quantised BEFORE the permutation (T rows instead of T*k); the permutation then moves one-byte rows
   if ((s = mx_quantize_rows(X, T, d, 32, base + a.Xq, base + a.tok_sf, VIBE_MX_SF_ROWMAJOR, T,
@@ -426,7 +429,7 @@ extern "C" vibe_status vibe_moe_layer_forward_mxfp8(const vibe_route_cfg* cfg, c
   if (T == 0) return VIBE_OK;
   if ((s = mx_gather_row_sf(base + a.tok_sf, r2a, offsets, E_loc, k, (int)a.R_cap, d, base + a.xsf, st)) != VIBE_OK) return s;
   if ((s = grouped_ffn_mxfp8_impl(base + a.Xpq, base + a.xsf, offsets, E_loc, (int)a.R_cap, d, f, W1q, W3q, sf13, W2q, sf2,
-                                  base + a.Hq, base + a.hsf, base + a.Y, st)) != VIBE_OK)
+                                  base + a.Hq, base + a.hsf, base + a.Y, st, base + a.ffn_ws, grouped_ffn_ws_bytes(), true)) != VIBE_OK)
     return s;
   return vibe_combine(base + a.Y, a2r, w, T, k, d, out, stream);
 }
