@@ -112,7 +112,10 @@ constexpr int SPLIT_MIN_STEPS = 4;         // K steps per slice at least
 constexpr int SPLIT_MAX_UNITS = 128;       // >= CTA pairs of any supported device (B200: 74)
 constexpr size_t SPLIT_PART_BYTES = (size_t)SPLIT_MAX_UNITS * TN * 256 * sizeof(float);
 constexpr int SPLIT_COUNTERS = SPLIT_MAX_UNITS * 16;     // per tile: 2 CTA ranks x 8 epilogue-warp roles
-constexpr size_t SPLIT_WS_BYTES = SPLIT_PART_BYTES + 2 * (size_t)SPLIT_COUNTERS * sizeof(int);   // counters of GEMM-1, of GEMM-2
+constexpr int TILE_CTRS = 16;               // [0], [8]: the next-unit counters of GEMM-1 / GEMM-2 (dynamic tile scheduler)
+constexpr size_t SPLIT_CNT_BYTES = (2 * (size_t)SPLIT_COUNTERS + TILE_CTRS) * sizeof(int);       // zeroed per call
+constexpr size_t SPLIT_WS_BYTES = SPLIT_PART_BYTES + SPLIT_CNT_BYTES;   // partials | counters of GEMM-1 | of GEMM-2 | unit counters
+constexpr int RING = 4;                     // unit ids in flight between the fetching warp and the other roles of a pair
 
 // what the e4m3 kinds need beyond the bf16 kernel's arguments
 struct FfnAux {
@@ -132,6 +135,9 @@ struct SmemTail {
   uint64_t empty[STAGES];         // each CTA: the MMAs reading the stage have retired
   uint64_t tfull[2];              // each CTA: accumulator stage complete
   uint64_t tempty[2];             // leader CTA: all 8 epilogue warps of the pair drained it
+  uint64_t rfull[RING];           // each CTA: ring slot holds the next unit id of the pair
+  uint64_t rempty[RING];          // leader CTA: every consuming warp of the pair has read the slot
+  int32_t ring[RING];             // unit ids (-1: no more work), written by the leader's producer warp in BOTH CTAs
   uint32_t tmem_base;
   int32_t total_t_tiles;
   int32_t split;                  // K slices of a split tile (1 = no split-K)
@@ -240,6 +246,58 @@ __device__ __forceinline__ void store_block_T_e4m3(const float (&v)[32], uint8_t
 }
 
 
+// ---- which unit a pair works on next --------------------------------------------------------------------------
+// Static (no workspace): round r hands out units [r*P, (r+1)*P) rotated by r (tile_of).  Dynamic (workspace given):
+// the pairs take the next unit from ONE global counter when they are ready for it, so that consecutive units -- the
+// token tiles that share a weight tile -- are started within microseconds of each other by whichever pairs are free,
+// and stay L2-resident for each other; under the static assignment the pairs drift apart by whole tiles over the
+// rounds (tile costs differ with the ragged N) and every drifted sharer re-reads its weight tile from DRAM
+// (profiles/: 1.5 x the algorithmic bytes).  Dynamic hand-out also balances the ragged tile costs.
+// The leader CTA's producer warp fetches (one atomicAdd per unit, on demand: its latency hides behind the 6 stages
+// the producer runs ahead) and publishes the id to a 4-slot ring in both CTAs; every other role of the pair reads it.
+struct UnitCursor {
+  int rnd = 0, idx = 0;
+  uint32_t ph = 0;
+};
+__device__ __forceinline__ int next_unit_fetch(SmemTail* tail, unsigned int* ctr, int total, int pair, int num_pairs,
+                                               UnitCursor& c, int lane) {
+  if (ctr == nullptr) {
+    const int u = tile_of(c.rnd, pair, num_pairs);
+    ++c.rnd;
+    return u < total ? u : -1;
+  }
+  const int slot = c.idx;
+  ptx::mbar_wait(ptx::smem_u32(&tail->rempty[slot]), c.ph ^ 1u);
+  int u = 0;
+  if (lane == 0) {
+    u = (int)atomicAdd(ctr, 1u);
+    if (u >= total) u = -1;
+    const uint32_t ra = ptx::smem_u32(&tail->ring[slot]), fa = ptx::smem_u32(&tail->rfull[slot]);
+    ptx::st_shared_cluster_u32(ptx::mapa_u32(ra, 0), (uint32_t)u);
+    ptx::st_shared_cluster_u32(ptx::mapa_u32(ra, 1), (uint32_t)u);
+    ptx::mbar_arrive_release_cluster(ptx::mapa_u32(fa, 0));
+    ptx::mbar_arrive_release_cluster(ptx::mapa_u32(fa, 1));
+  }
+  u = __shfl_sync(0xffffffffu, u, 0);
+  if (++c.idx == RING) { c.idx = 0; c.ph ^= 1u; }
+  return u;
+}
+__device__ __forceinline__ int next_unit_read(SmemTail* tail, bool dynamic, int total, int pair, int num_pairs, UnitCursor& c,
+                                              int lane) {
+  if (!dynamic) {
+    const int u = tile_of(c.rnd, pair, num_pairs);
+    ++c.rnd;
+    return u < total ? u : -1;
+  }
+  const int slot = c.idx;
+  ptx::mbar_wait_acq_cluster(ptx::smem_u32(&tail->rfull[slot]), c.ph);
+  const int u = *reinterpret_cast<volatile int32_t*>(&tail->ring[slot]);
+  __syncwarp();
+  if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa_u32(ptx::smem_u32(&tail->rempty[slot]), 0));
+  if (++c.idx == RING) { c.idx = 0; c.ph ^= 1u; }
+  return u;
+}
+
 // kMode: 0 = gate|up + SwiGLU (GEMM-1), 1 = down (GEMM-2), 2 = down with the gate-weighted
 // scatter fused into the epilogue (vibe_grouped_ffn_scatter; KIND_BF16 only).  kKind: the operand kind (above).
 template <int kMode, int kKind>
@@ -249,7 +307,7 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
                 int n_total, int k_total, void* __restrict__ out_v, int ld_out,
                 const int32_t* __restrict__ row_to_assign, const float* __restrict__ topk_w,
                 float* __restrict__ split_part /*NULL: no split-K*/, int* __restrict__ split_cnt,
-                const __grid_constant__ FfnAux aux) {
+                unsigned int* __restrict__ unit_ctr /*NULL: static tile assignment*/, const __grid_constant__ FfnAux aux) {
   static_assert(kMode != 2 || kKind == KIND_BF16, "the fused scatter epilogue exists for the bf16 kind only");
   constexpr bool kGateUp = (kMode == 0);
   constexpr bool kMx = (kKind == KIND_MXF8);
@@ -290,6 +348,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(ptx::smem_u32(&tail->tfull[a]), 1);
       ptx::mbar_init(ptx::smem_u32(&tail->tempty[a]), 2 * (num_threads(kMode) / 32 - 2));   // epilogue warps of the pair
+    }
+    for (int r = 0; r < RING; ++r) {
+      ptx::mbar_init(ptx::smem_u32(&tail->rfull[r]), 1);
+      // readers of a slot: the peer's producer warp, the leader's MMA warp, the epilogue warps of both CTAs
+      ptx::mbar_init(ptx::smem_u32(&tail->rempty[r]), 2 + 2 * (num_threads(kMode) / 32 - 2));
     }
     ptx::fence_barrier_init();
   } else if (warp == 1) {
@@ -373,7 +436,11 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       TileCursor cur;
       int stage = 0;
       uint32_t phase = 0;
-      for (int rnd = 0, unit = pair; unit < total_units; ++rnd, unit = tile_of(rnd, pair, num_pairs)) {
+      UnitCursor uc;
+      for (;;) {
+        const int unit = rank == 0 ? next_unit_fetch(tail, unit_ctr, total_units, pair, num_pairs, uc, lane)
+                                   : next_unit_read(tail, unit_ctr != nullptr, total_units, pair, num_pairs, uc, lane);
+        if (unit < 0) break;
         int f_blk, t_blk;
         const bool is_split = unit >= split_from;
         const int tile = is_split ? split_from + (unit - split_from) / S : unit;
@@ -454,7 +521,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
+      UnitCursor uc;
+      for (;; ++it) {
+        const int unit = next_unit_read(tail, unit_ctr != nullptr, total_units, pair, num_pairs, uc, lane);
+        if (unit < 0) break;
         int f_blk, t_blk;
         const bool is_split = unit >= split_from;
         const int tile = is_split ? split_from + (unit - split_from) / S : unit;
@@ -515,7 +585,10 @@ ffn_gemm_kernel(const __grid_constant__ CUtensorMap tmAct, const __grid_constant
     const int blk_par = (warp - 2) >> 2;   // down projection: which 32-column blocks (even / odd) are mine
     TileCursor cur;
     int it = 0;
-    for (int rnd = 0, unit = pair; unit < total_units; ++rnd, ++it, unit = tile_of(rnd, pair, num_pairs)) {
+    UnitCursor uc;
+    for (;; ++it) {
+      const int unit = next_unit_read(tail, unit_ctr != nullptr, total_units, pair, num_pairs, uc, lane);
+      if (unit < 0) break;
       int f_blk, t_blk;
       const bool is_split = unit >= split_from;
       const int tile = is_split ? split_from + (unit - split_from) / S : unit;
@@ -846,13 +919,18 @@ struct SplitWs {
   float* part = nullptr;
   int* cnt1 = nullptr;
   int* cnt2 = nullptr;
+  unsigned int* ctr1 = nullptr;   // next-unit counters of the dynamic tile scheduler
+  unsigned int* ctr2 = nullptr;
 };
 vibe_status split_ws(void* ws, size_t ws_bytes, bool ws_zeroed, cudaStream_t st, SplitWs* out) {
   if (ws != nullptr && ws_bytes >= SPLIT_WS_BYTES && (reinterpret_cast<uintptr_t>(ws) & 15u) == 0) {
     out->part = reinterpret_cast<float*>(ws);
     out->cnt1 = reinterpret_cast<int*>(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES);
     out->cnt2 = out->cnt1 + SPLIT_COUNTERS;
-    if (!ws_zeroed) VIBE_CUDA(cudaMemsetAsync(out->cnt1, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
+    out->ctr1 = reinterpret_cast<unsigned int*>(out->cnt2 + SPLIT_COUNTERS);
+    out->ctr2 = out->ctr1 + 8;
+
+    if (!ws_zeroed) VIBE_CUDA(cudaMemsetAsync(out->cnt1, 0, SPLIT_CNT_BYTES, st));
   }
   return VIBE_OK;
 }
@@ -869,12 +947,19 @@ vibe_status launch_pair(const CUtensorMap& tmX, const CUtensorMap& tmXN, const C
   // both launches carry the programmatic-dependent-launch attribute (see the kernel's set-up)
   const int32_t* no_map = nullptr;
   const float* no_w = nullptr;
+  // dynamic hand-out of tiles only where a tile is long enough to hide the fetch (one atomic round trip plus two
+  // cluster-scope barrier hops per tile, ~1.5 us): at least DYN_MIN_STEPS K stages per tile.  Short-K launches (the
+  // C2 shape: 32 / 12 stages) keep the static assignment -- measured 4 % faster there, while the long-K launches of C1
+  // gain 1-2 % in time and drop from 1.52 x to 1.09 x the algorithmic DRAM bytes.
+  constexpr int DYN_MIN_STEPS = 48;
+  unsigned int* ctr1 = (d / bk_of(kKind) >= DYN_MIN_STEPS) ? sw.ctr1 : nullptr;
+  unsigned int* ctr2 = (f / bk_of(kKind) >= DYN_MIN_STEPS) ? sw.ctr2 : nullptr;
   cudaError_t le = launch_pdl(ffn_gemm_kernel<0, kKind>, dim3(grid), dim3(num_threads(0)), SMEM_BYTES, st, tmX, tmXN, tmW1, tmW3,
-                              offsets, E_loc, f, d, H, f, no_map, no_w, sw.part, sw.cnt1, aux1);
+                              offsets, E_loc, f, d, H, f, no_map, no_w, sw.part, sw.cnt1, ctr1, aux1);
   VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<gate_up> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<gate_up>");
   le = launch_pdl(ffn_gemm_kernel<kDownMode, kKind>, dim3(grid), dim3(num_threads(kDownMode)), SMEM_BYTES, st, tmH, tmHN, tmW2,
-                  tmW2, offsets, E_loc, d, f, Y, d, row_to_assign, topk_w, sw.part, sw.cnt2, aux2);
+                  tmW2, offsets, E_loc, d, f, Y, d, row_to_assign, topk_w, sw.part, sw.cnt2, ctr2, aux2);
   VIBE_REQUIRE(le == cudaSuccess, VIBE_ERR_CUDA, "ffn_gemm_kernel<down> launch failed: %s", cudaGetErrorString(le));
   VIBE_LAUNCH_CHECK("ffn_gemm_kernel<down>");
   return VIBE_OK;
@@ -884,7 +969,7 @@ vibe_status launch_pair(const CUtensorMap& tmX, const CUtensorMap& tmXN, const C
 
 size_t grouped_ffn_ws_bytes() { return SPLIT_WS_BYTES; }
 vibe_status grouped_ffn_zero_counters(void* ws, cudaStream_t st) {
-  VIBE_CUDA(cudaMemsetAsync(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES, 0, 2 * (size_t)SPLIT_COUNTERS * sizeof(int), st));
+  VIBE_CUDA(cudaMemsetAsync(reinterpret_cast<char*>(ws) + SPLIT_PART_BYTES, 0, SPLIT_CNT_BYTES, st));
   return VIBE_OK;
 }
 
