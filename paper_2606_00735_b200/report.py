@@ -349,6 +349,32 @@ def section_ffn_fp8(peaks, quick):
     return out
 
 
+def section_fp8_probe(peaks, quick):
+    """A fixed, short launch sequence for ncu captures of the two FP8 kinds: C1 shape, 8 experts x 1024 rows; three
+    calls of the block-scaled FFN, then three of the per-tensor one (launches 1-6 and 7-12 of ffn_gemm_kernel)."""
+    cfg = I.C1
+    E, d, f, n = cfg.E_loc, cfg.d, cfg.f, 1024
+    W1, W3, W2 = _weights(E, d, f)
+    R = E * n
+    Xp = torch.randn((R, d), device="cuda").to(torch.bfloat16)
+    off = (torch.arange(E + 1, device="cuda", dtype=torch.int32) * n).contiguous()
+    W1m, sf13 = B.mxfp8_pack_weights(W1, B.MX_ROLE_GATE)
+    W3m, sf13 = B.mxfp8_pack_weights(W3, B.MX_ROLE_UP, sf=sf13)
+    W2m, sf2 = B.mxfp8_pack_weights(W2, B.MX_ROLE_DOWN)
+    Xm, xsf = B.mxfp8_quantize_rows(Xp, 32, B.MX_SF_TOKENS, R_cap=R)
+    for _ in range(3):
+        B.grouped_ffn_mxfp8(Xm, xsf, off, W1m, W3m, sf13, W2m, sf2)
+    torch.cuda.synchronize()
+    del W1m, W3m, W2m
+    (W1q, s1), (W3q, s3), (W2q, s2) = (B.fp8_pack_weights(w) for w in (W1, W3, W2))
+    Xq, rs = B.fp8_quantize_rows(Xp)
+    hs = torch.full((E,), 8.0 / 448.0, dtype=torch.float32, device="cuda")
+    for _ in range(3):
+        B.grouped_ffn_fp8(Xq, rs, off, W1q, s1, W3q, s3, W2q, s2, hs)
+    torch.cuda.synchronize()
+    return {"shape": cfg.name, "rows_per_expert": n, "calls": "3 x vibe_grouped_ffn_mxfp8, then 3 x vibe_grouped_ffn_fp8"}
+
+
 def _weights(E, d, f):
     W1 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
     W3 = (torch.randn((E, d, f), device="cuda") * d ** -0.5).to(torch.bfloat16)
@@ -762,6 +788,8 @@ def main():
         rep["fused_scatter"] = section_fused(peaks, args.quick)
         for r in rep["fused_scatter"]:
             print(r, flush=True)
+    if "fp8_probe" in want:
+        rep["fp8_probe"] = section_fp8_probe(peaks, args.quick)
     if "fp8" in want:
         rep["ffn_fp8"] = section_ffn_fp8(peaks, args.quick)
         for r in rep["ffn_fp8"]:
