@@ -16,8 +16,10 @@ Citations:  P:L<n> = /root/reference/PAPER.md line n;  R*/P*/F*/C*/M*/L* = DESIG
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): every function below is pinned to
 something other than itself -- brute force, closed forms, library routines
 (scipy.special.softmax/expit, np.argsort(kind='stable'), torch CPU fp64 matmul+silu),
-hand-worked golden fixtures in tests/golden/.  The only unpinned item is the latency
-*profile* (a measurement; nothing to pin numerically) -- its *model* (O5) is pinned.
+hand-worked golden fixtures in tests/golden/; the FP8 parts (O11, O12) additionally to torch's own
+float8_e4m3fn / float8_e8m0fnu casts and to golden rows worked in exact rational arithmetic.
+parity unpinned: only the latency *profile* (a measurement; nothing to pin numerically) -- its *model*
+(O5) is pinned.
 """
 from __future__ import annotations
 
