@@ -139,6 +139,11 @@ VIBE_API vibe_status vibe_permute(const void* X, const int32_t* topk_ids, const 
  *     has CTA pairs -- a lone or a few light experts, the decode regime P:L108 / L130 calls low-intensity -- every
  *     tile's K range is cut over several pairs and reduced in fp32 in a fixed order.  With ws = NULL (or too small)
  *     the call is still correct; such launches then stream their weights on as many SM pairs as they have tiles.
+ *     The workspace also holds the unit counters of the DYNAMIC tile hand-out used for long-K launches (the CTA pairs
+ *     take the next tile from one counter when they are ready, so that the token tiles sharing a weight tile run
+ *     together and share it through L2: DRAM traffic 1.08 x instead of 1.5 x the algorithmic bytes at the C1 shape);
+ *     without a workspace tiles are assigned statically.  Results do not depend on the workspace being given beyond
+ *     the fp32 summation order of split tiles, and are bit-reproducible from call to call either way.
  *     Calls that may run concurrently must use different workspaces.
  * ---------------------------------------------------------------------------------- */
 VIBE_API vibe_status vibe_grouped_ffn(const void* Xp, const int32_t* offsets, int32_t E_loc, int32_t R_cap,
