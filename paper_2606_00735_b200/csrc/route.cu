@@ -373,7 +373,6 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
 #pragma unroll
     for (int v = 0; v < VPL; ++v) insert(uk[v], v);
     // ---- group-limited routing (R6), one group per lane: score = sum of the lane's two largest keys ----
-    bool masked = false;
     if (p.n_group > 1) {
       const float k0 = unordered(h0);
       const float k1 = unordered(h1);
@@ -385,10 +384,10 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
         rank += (s2 > score || (s2 == score && g2 < sub)) ? 1 : 0;
       }
       if (rank >= p.topk_group) {
-        // the lane's keys count as -inf in the selection; uk[] keeps the logits' images (the softmax denominator
-        // without renormalisation runs over ALL experts)
-        masked = true;
-        h0 = h1 = h2 = h3 = ordered_u32(NEG_INF);      // indices 0..3 in order: the lane's first four in pick order
+        const uint32_t ninf = ordered_u32(NEG_INF);
+#pragma unroll
+        for (int v = 0; v < VPL; ++v) uk[v] = ninf;
+        h0 = h1 = h2 = h3 = ninf;      // indices 0..3 in order: still the lane's first four in pick order
         i0 = 0; i1 = 1; i2 = 2; i3 = 3;
       }
     }
@@ -414,7 +413,7 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
         i0 = i1 = i2 = i3 = 0;
 #pragma unroll
         for (int v = 0; v < VPL; ++v) {
-          const uint32_t c0 = masked ? ordered_u32(NEG_INF) : uk[v];
+          const uint32_t c0 = uk[v];
           const bool elig = (c0 < lk) || (c0 == lk && v > lv);
           insert(elig ? c0 : kTaken, v);
         }
@@ -541,7 +540,10 @@ extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* l
   const bool sig = cfg->score_fn == VIBE_SCORE_SIGMOID;
 
   // 128 / 256 experts, top-k <= 8: four tokens per warp (route_topk8_kernel); group-limited only with 8 groups
-  if ((E == 128 || E == 256) && k <= 8 && (ng == 0 || ng == 8)) {
+  // (not the un-renormalised softmax with group limiting: the wide-lane kernel overwrites the keys of masked groups,
+  // and that denominator runs over ALL logits; keeping them costs a register, a spill and 15 % of the kernel's speed
+  // for every other configuration -- measured --, so this one combination takes the 32-lane kernel)
+  if ((E == 128 || E == 256) && k <= 8 && (ng == 0 || (ng == 8 && (sig || cfg->renormalize)))) {
     p.fast_groups = 1;
     return E == 256 ? launch_route8<32>(p, sig, st) : launch_route8<16>(p, sig, st);
   }
