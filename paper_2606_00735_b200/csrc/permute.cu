@@ -258,19 +258,19 @@ __global__ void __launch_bounds__(256) perm_rows_kernel(const __nv_bfloat16* __r
   const int vpr = d >> 3;
   const int per_row = vpr / VPT;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the FFN's CTAs may become resident
-  asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
   const long long g = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (g >= (long long)T * per_row) return;
-  const int t = (int)(g / per_row);
-  const int v0 = (int)(g - (long long)t * per_row);
-  const int32_t* a2r = assign_to_row + (size_t)t * k;
-  bool any = false;
-  for (int j = 0; j < k; ++j) any |= (__ldg(a2r + j) >= 0);
-  if (!any) return;
+  const bool live = g < (long long)T * per_row;
+  const int t = live ? (int)(g / per_row) : 0;
+  const int v0 = live ? (int)(g - (long long)t * per_row) : 0;
+  // X is an INPUT of the permutation (not written by the index kernel): the CTAs that are resident while K1 still
+  // runs issue their row loads before they wait for the index
   const uint4* src = reinterpret_cast<const uint4*>(X + (size_t)t * d) + v0;
   uint4 val[VPT];
 #pragma unroll
-  for (int q = 0; q < VPT; ++q) val[q] = ld_nc_v4(src + q * per_row);
+  for (int q = 0; q < VPT; ++q) val[q] = live ? ld_nc_v4(src + q * per_row) : make_uint4(0, 0, 0, 0);
+  asm volatile("griddepcontrol.wait;" ::: "memory");     // K1's index is complete and visible
+  if (!live) return;
+  const int32_t* a2r = assign_to_row + (size_t)t * k;
   for (int j = 0; j < k; ++j) {
     const int r = __ldg(a2r + j);
     if (r < 0) continue;
