@@ -298,6 +298,19 @@ VIBE_API vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, i
                                                      float* latency_us /*host*/, float* samples_us /*host|NULL*/,
                                                      void* ws, size_t ws_bytes, void* stream);
 
+/* a6 for the BLOCK-SCALED FP8 FFN (packed weights / scales as vibe_grouped_ffn_mxfp8).  Segments start on multiples of
+ * 64 rows and are roundup(n, 64) rows long -- what vibe_permute with align = 64 hands that kernel -- so l(n) is a step
+ * function of n with steps of 64.  ws: with n' = max(roundup(max tokens_per_expert, 64), 64) and R' = E_loc * n':
+ * vibe_workspace_bytes(VIBE_WS_PROFILE, T = n', ...) rounded up to 256, plus vibe_mxfp8_sf_bytes(TOKENS, R', d) and
+ * vibe_mxfp8_sf_bytes(TOKENS, R', f), each rounded up to 256 bytes. */
+VIBE_API vibe_status vibe_profile_expert_latency_mxfp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
+                                                       const void* W3q, const void* sf13, const void* W2q,
+                                                       const void* sf2, const int32_t* tokens_per_expert /*host*/,
+                                                       int32_t n_points, int32_t mode, int32_t warmup, int32_t iters,
+                                                       float* latency_us /*host*/, float* samples_us /*host|NULL*/,
+                                                       void* ws, size_t ws_bytes, void* stream);
+
+
 /* ------------------------------------------------------------------------------------
  * The whole layer (a1..a5) as one call: enqueues route -> permute -> grouped FFN ->
  * combine on `stream` using one caller-provided device arena.

@@ -41,7 +41,7 @@ EXPORTED_SYMBOLS = (
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
     "vibe_fp8_quantize_rows", "vibe_fp8_pack_weights", "vibe_grouped_ffn_fp8", "vibe_moe_layer_forward_fp8",
     "vibe_profile_expert_latency_fp8", "vibe_moe_layer_forward_host_chunked",
-    "vibe_l2_flush", "vibe_moe_layer_forward_host_async", "vibe_host_wait", "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
+    "vibe_profile_expert_latency_mxfp8", "vibe_l2_flush", "vibe_moe_layer_forward_host_async", "vibe_host_wait", "vibe_mxfp8_sf_bytes", "vibe_mxfp8_quantize_rows", "vibe_mxfp8_pack_weights", "vibe_grouped_ffn_mxfp8",
     "vibe_moe_layer_forward_mxfp8",
     "vibe_drift_cosine", "vibe_drift_monitor_create", "vibe_drift_monitor_destroy",
     "vibe_drift_monitor_set_reference", "vibe_drift_monitor_push", "vibe_drift_monitor_rearranged",
@@ -124,6 +124,9 @@ def load() -> C.CDLL:
                                                         vp, vp, vp, i32, vp, sz, vp]
     lib.vibe_moe_layer_forward_fp8.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp,
                                                vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_profile_expert_latency_mxfp8.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, C.POINTER(i32), i32, i32, i32, i32,
+                                                      C.POINTER(C.c_float), C.POINTER(C.c_float), vp, sz, vp]
+    lib.vibe_profile_expert_latency_mxfp8.restype = C.c_int
     lib.vibe_moe_layer_forward_host_async.argtypes = [C.POINTER(_RouteCfg), vp, vp, vp, i32, i32, i32, i32, vp, vp, vp,
                                                       vp, vp, vp, sz, vp, C.POINTER(i32)]
     lib.vibe_moe_layer_forward_host_async.restype = C.c_int
@@ -555,6 +558,25 @@ def profile_expert_latency_fp8(W1q, s1, W3q, s3, W2q, s2, h_scale, tokens_per_ex
                                             W2q.data_ptr(), s2.data_ptr(), h_scale.data_ptr(), toks, npts, mode, warmup,
                                             iters, lat, None, ws.data_ptr(), ws.numel(), _stream(stream)),
         "vibe_profile_expert_latency_fp8")
+    return np.array(lat[:], dtype=np.float64)
+
+
+def profile_expert_latency_mxfp8(W1q, W3q, sf13, W2q, sf2, tokens_per_expert: Sequence[int] = DEFAULT_SWEEP, mode: int = 0,
+                                 warmup: int = 10, iters: int = 100, stream=None):
+    """vibe_profile_expert_latency for the block-scaled FP8 FFN (median latency [us] per sweep point)."""
+    lib = load()
+    E_loc, f, d = W1q.shape
+    toks = (C.c_int32 * len(tokens_per_expert))(*[int(x) for x in tokens_per_expert])
+    npts = len(tokens_per_expert)
+    lat = (C.c_float * npts)()
+    n_pad = max((max(tokens_per_expert) + MX_ROW_ALIGN - 1) // MX_ROW_ALIGN * MX_ROW_ALIGN, MX_ROW_ALIGN)
+    r256 = lambda x: (x + 255) // 256 * 256
+    need = r256(workspace_bytes(WS_PROFILE, n_pad, 1, E_loc, E_loc, d, f, 1)) + \
+        r256(mxfp8_sf_bytes(MX_SF_TOKENS, E_loc * n_pad, d)) + r256(mxfp8_sf_bytes(MX_SF_TOKENS, E_loc * n_pad, f))
+    ws = _scratch(need, W1q.device, stream)
+    _ok(lib.vibe_profile_expert_latency_mxfp8(E_loc, d, f, W1q.data_ptr(), W3q.data_ptr(), sf13.data_ptr(), W2q.data_ptr(),
+                                              sf2.data_ptr(), toks, npts, mode, warmup, iters, lat, None, ws.data_ptr(),
+                                              ws.numel(), _stream(stream)), "vibe_profile_expert_latency_mxfp8")
     return np.array(lat[:], dtype=np.float64)
 
 

@@ -55,7 +55,8 @@ namespace {
 // read faster than it ever does inside a model, where the other layers' traffic has evicted them.
 template <class Run>
 vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_points, int mode, int warmup, int iters,
-                          float* latency_us, float* samples_us, int32_t* offsets, void* flush, cudaStream_t caller, Run run) {
+                          float* latency_us, float* samples_us, int32_t* offsets, void* flush, cudaStream_t caller, Run run,
+                          int seg_align = 1) {
   VIBE_CUDA(cudaStreamSynchronize(caller));
   cudaStream_t st = nullptr;
   VIBE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
@@ -69,7 +70,8 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
   for (int p = 0; p < n_points && rc == VIBE_OK; ++p) {
     const int n = tokens_per_expert[p];
     off[0] = 0;
-    for (int e = 0; e < E_loc; ++e) off[e + 1] = off[e] + ((mode == 0 || e == 0) ? n : 0);
+    // (seg_align > 1: segments start on multiples of it and are that long -- what vibe_permute with that align produces)
+    for (int e = 0; e < E_loc; ++e) off[e + 1] = off[e] + ((mode == 0 || e == 0) ? (n + seg_align - 1) / seg_align * seg_align : 0);
     cudaError_t ce = cudaMemcpyAsync(offsets, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
     if (ce != cudaSuccess) {
@@ -224,6 +226,62 @@ extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d,
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st, [&](cudaStream_t ps) {
     return grouped_ffn_fp8_impl(Xq, row_scale, offsets, E_loc, R_cap, d, f, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq, Y, ps);
   });
+}
+
+extern "C" vibe_status vibe_profile_expert_latency_mxfp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
+                                                         const void* W3q, const void* sf13, const void* W2q,
+                                                         const void* sf2, const int32_t* tokens_per_expert,
+                                                         int32_t n_points, int32_t mode, int32_t warmup, int32_t iters,
+                                                         float* latency_us, float* samples_us, void* ws, size_t ws_bytes,
+                                                         void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(tokens_per_expert && latency_us && n_points >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_mxfp8: need tokens_per_expert, latency_us, n_points >= 1");
+  VIBE_REQUIRE(mode == 0 || mode == 1, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency_mxfp8: mode must be 0 or 1");
+  VIBE_REQUIRE(warmup >= 0 && iters >= 1 && iters <= 100000, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_mxfp8: need warmup >= 0, 1 <= iters <= 100000");
+  VIBE_REQUIRE(W1q && W3q && sf13 && W2q && sf2, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency_mxfp8: NULL weights / scales");
+  VIBE_REQUIRE(d % 128 == 0 && f % 128 == 0 && E_loc >= 1 && E_loc <= 512, VIBE_ERR_UNSUPPORTED,
+               "vibe_profile_expert_latency_mxfp8: d and f must be multiples of 128, E_loc <= 512");
+  int n_max = 0;
+  for (int p = 0; p < n_points; ++p) {
+    VIBE_REQUIRE(tokens_per_expert[p] >= 0, VIBE_ERR_INVALID_ARG, "vibe_profile_expert_latency_mxfp8: negative token count");
+    n_max = std::max(n_max, tokens_per_expert[p]);
+  }
+  const int n_pad = std::max((n_max + kMxRowAlign - 1) / kMxRowAlign * kMxRowAlign, kMxRowAlign);
+  VIBE_REQUIRE((int64_t)E_loc * n_pad < (int64_t)INT32_MAX, VIBE_ERR_INVALID_ARG,
+               "vibe_profile_expert_latency_mxfp8: E_loc * max tokens >= 2^31");
+  const int R_cap = E_loc * n_pad;
+  const size_t base_need = round_up(vibe_workspace_bytes(VIBE_WS_PROFILE, n_pad, 1, E_loc, E_loc, d, f, 1), 256);
+  const size_t xsf_b = round_up(vibe_mxfp8_sf_bytes(VIBE_MX_SF_TOKENS, R_cap, d, 1), 256);
+  const size_t hsf_b = round_up(vibe_mxfp8_sf_bytes(VIBE_MX_SF_TOKENS, R_cap, f, 1), 256);
+  const size_t need = base_need + xsf_b + hsf_b;
+  VIBE_REQUIRE(ws != nullptr && ws_bytes >= need && (reinterpret_cast<uintptr_t>(ws) & 255u) == 0, VIBE_ERR_WORKSPACE,
+               "vibe_profile_expert_latency_mxfp8: workspace needs %zu bytes, 256-byte aligned (got %zu)", need, ws_bytes);
+  // the bf16 profile's workspace layout with one-byte activations (Xq | Y | Hq | offsets | FFN ws | flush), scales appended
+  char* base = reinterpret_cast<char*>(ws);
+  void* Xq = base;
+  void* Y = base + round_up((size_t)R_cap * d * 2, 256);
+  char* Hreg = base + 2 * round_up((size_t)R_cap * d * 2, 256);
+  void* Hq = Hreg;
+  int32_t* offsets = reinterpret_cast<int32_t*>(Hreg + round_up((size_t)R_cap * f * 2, 256));
+  void* flush = base + base_need - kProfileFlushBytes;
+  void* ffn_ws = base + base_need - kProfileFlushBytes - round_up(grouped_ffn_ws_bytes(), 256);
+  void* xsf = base + base_need;
+  void* hsf = base + base_need + xsf_b;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  // arbitrary finite codes (0x38 = 1.0) and unit scales (byte 127): latency does not depend on the values
+  VIBE_CUDA(cudaMemsetAsync(Xq, 0x38, (size_t)R_cap * d, st));
+  VIBE_CUDA(cudaMemsetAsync(xsf, 127, xsf_b, st));
+  VIBE_CUDA(cudaMemsetAsync(hsf, 127, hsf_b, st));
+  VIBE_CUDA(cudaMemsetAsync(flush, 0, kProfileFlushBytes, st));
+  return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st,
+                       [&](cudaStream_t ps) {
+                         return grouped_ffn_mxfp8_impl(Xq, xsf, offsets, E_loc, R_cap, d, f, W1q, W3q, sf13, W2q, sf2, Hq, hsf, Y, ps,
+                                                       ffn_ws, grouped_ffn_ws_bytes(), false);
+                       },
+                       kMxRowAlign);
 }
 
 // Measurement utility: evict the L2 (evict_last read sweep, see l2_flush_kernel) before a timed region.

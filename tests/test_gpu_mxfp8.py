@@ -204,3 +204,21 @@ def test_layer_forward_mxfp8_against_oracle(which):
     assert m["mean_rel_err"] <= FFN_MEAN, m
     bound = 1e-2 * m["rms_ref"] + BF16_U * ref_abs + BF16_U * np.abs(ref)
     assert np.all(np.abs(got - ref) <= bound), (np.max(np.abs(got - ref) / bound), m)
+
+
+def test_profile_expert_latency_mxfp8_sanity():
+    """a6 for the block-scaled FFN: positive, finite, a step function of n with steps of 64 rows (segments are
+    padded to the scale-factor row alignment), growing with n, not faster than the nominal dense FP8 peak."""
+    cfg = I.scaled(I.C2, E=16, E_loc=16)
+    Wb = [dev_bf16(x) for x in I.make_weights(cfg.E_loc, cfg.d, cfg.f, 0)]
+    W1m, sf13 = B.mxfp8_pack_weights(Wb[0], B.MX_ROLE_GATE)
+    W3m, sf13 = B.mxfp8_pack_weights(Wb[1], B.MX_ROLE_UP, sf=sf13)
+    W2m, sf2 = B.mxfp8_pack_weights(Wb[2], B.MX_ROLE_DOWN)
+    sweep = [1, 64, 128, 2048]
+    lat = B.profile_expert_latency_mxfp8(W1m, W3m, sf13, W2m, sf2, sweep, mode=0, warmup=3, iters=21)
+    assert lat.shape == (4,) and np.all(lat > 0) and np.all(np.isfinite(lat))
+    assert abs(lat[0] - lat[1]) <= 0.15 * lat[1], lat            # 1 row and 64 rows are the same launch
+    assert lat[3] > lat[2] >= lat[1] * 0.9, lat
+    assert lat[3] * 1e-6 >= 6.0 * 2048 * cfg.d * cfg.f / 4.5e15
+    solo = B.profile_expert_latency_mxfp8(W1m, W3m, sf13, W2m, sf2, [128], mode=1, warmup=2, iters=5)
+    assert solo[0] > 0
