@@ -9,7 +9,10 @@
 // Gate weights are evaluated in fp64 for the k picked experts only.
 //
 // Semantics: include/vibe.h (vibe_route_topk), readings R1-R8.
+#include <mutex>
+
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace vibe {
 namespace {
@@ -339,7 +342,10 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
 
   // the trip count is WARP-uniform (full-mask collectives inside): a group past the last token works on a copy of
   // token T-1 and stores nothing
-  for (int tw = blockIdx.x * 32 + (gidx & ~3); tw < p.T; tw += gridDim.x * 32) {
+  // (tiles of four tokens, interleaved over (warp, block): a last, partial round of tiles is spread over all blocks)
+  const int n_tiles = (p.T + 3) >> 2;
+  for (int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < n_tiles; tile += 8 * gridDim.x) {
+    const int tw = tile * 4;
     const bool valid = tw + (gidx & 3) < p.T;
     const int t = valid ? tw + (gidx & 3) : p.T - 1;
     // a lane's VPL * 4 bytes are contiguous: both 16-byte halves of every 32-byte sector are this lane's, read by
@@ -463,12 +469,358 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
   }
 }
 
+
+// ------------------------------------------------------------------------------------------------------------
+// Packed-key variant of the wide-lane kernel (no group limiting; sigmoid, or softmax with renormalisation: the
+// two cases whose gate weights need the picked logits only).  ncu of route_topk8_kernel at 64K x 256 (profiles/
+// r2_route_ncu.md): 390 warp-instructions per token, three quarters of them on the ALU pipe (ISETP/SEL/LOP3/VIMNMX:
+// one warp-instruction per two cycles), most of them the (key, index) pairs dragged through the per-lane sorted
+// insertion and the five-instruction order-preserving map.  Here a key is ONE register: the order-preserving u32
+// image of the f32 key with its low 8 bits replaced by 255 - expert index, so keys are unique, ties go to the
+// lowest index by construction, a lane's first four are found by min/max sorting networks (5.1 VIMNMX per element
+// instead of 13 compare/select), a selection round is a group max and one compare (no ballot / find-first /
+// indexed shuffle), and the winner's index comes out of the key.
+// The packed order differs from the exact one only between keys that agree in their upper 24 bits without being
+// equal.  After the k rounds the k picks and the best remaining key are in packed order; if all adjacent pairs
+// differ in the upper 24 bits, every pick is strictly above every other key of the token in exact order too and
+// the result is exact.  Otherwise (about 3 tokens in 1000 on continuous f32 logits) the warp reloads the exact
+// keys: if the low bytes of ALL keys of the token are zero (bf16- or fp16-valued logits, where exact ties are
+// common), equal upper bits mean equal keys and the packed tie-break is the exact one; else the token is redone
+// by the exact selection below (k rounds of a full rescan; slow and rare).
+// ------------------------------------------------------------------------------------------------------------
+#define VIBE_CSWAP(a, b)                     \
+  {                                          \
+    const uint32_t hi_ = max(a, b);          \
+    const uint32_t lo_ = min(a, b);          \
+    a = hi_;                                 \
+    b = lo_;                                 \
+  }
+
+// (h0..h3) sorted descending <- the four largest of (h0..h3) sorted and (a, b, c, d) in any order
+__device__ __forceinline__ void merge_quad(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t a, uint32_t b,
+                                           uint32_t c, uint32_t d) {
+  VIBE_CSWAP(a, b);
+  VIBE_CSWAP(c, d);
+  VIBE_CSWAP(a, c);
+  VIBE_CSWAP(b, d);
+  VIBE_CSWAP(b, c);          // a >= b >= c >= d
+  h0 = max(h0, d);           // half-cleaner of the bitonic sequence h0 h1 h2 h3 d c b a: the four largest, bitonic
+  h1 = max(h1, c);
+  h2 = max(h2, b);
+  h3 = max(h3, a);
+  VIBE_CSWAP(h0, h2);
+  VIBE_CSWAP(h1, h3);
+  VIBE_CSWAP(h0, h1);
+  VIBE_CSWAP(h2, h3);
+}
+
+// One token by one warp on the EXACT keys (32 lanes x E/32 consecutive experts, k rounds of {lane best, redux max,
+// ballot, lowest lane wins}): the packed-key kernel calls it for the few tokens whose packed order is not provably the
+// exact one.  Writes the token's ids / weights and counts it in the block histogram.  No group limiting; sigmoid, or
+// softmax with renormalisation (the configurations of the packed-key kernel).
+template <int VPL, bool SIGMOID>
+__device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids, float* w, int k, int renorm, float scale,
+                                               int t, int* s_hist, const float* s_bias) {
+  constexpr int E = 8 * VPL;
+  constexpr int V = E / 32;
+  constexpr unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const float* row = logits + (size_t)t * E;
+  uint32_t uk[V];
+#pragma unroll
+  for (int q = 0; q < V / 4; ++q) {
+    const uint4 u = __ldg(reinterpret_cast<const uint4*>(row + lane * V) + q);
+    const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const int e = lane * V + 4 * q + c;
+      const float key = SIGMOID ? __fadd_rn(vsig(xv[c]), s_bias[(e / VPL) * (VPL + 1) + e % VPL]) : xv[c];
+      uk[4 * q + c] = ordered_u32(key);
+    }
+  }
+  int my_id = 0;
+  for (int j = 0; j < k; ++j) {
+    uint32_t best = kTaken;
+    int bv = 0;
+#pragma unroll
+    for (int v = 0; v < V; ++v)
+      if (uk[v] > best) { best = uk[v]; bv = v; }
+    const uint32_t gm = __reduce_max_sync(FULL, best);
+    const int win = __ffs(__ballot_sync(FULL, best == gm)) - 1;
+    const int id = __shfl_sync(FULL, lane * V + bv, win);
+    if (lane == j) my_id = id;
+    if (lane == win) {
+#pragma unroll
+      for (int v = 0; v < V; ++v)
+        if (v == bv) uk[v] = kTaken;
+    }
+  }
+  auto wsum_f64 = [&](double v) {
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+    return v;
+  };
+  const float my_x = (lane < k) ? __ldg(row + my_id) : 0.0f;
+  double wj;
+  if (SIGMOID) {
+    const double sj = (lane < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
+    wj = sj;
+    if (renorm) wj = sj / wsum_f64(sj);
+  } else {
+    const float mx = __shfl_sync(FULL, my_x, 0);
+    const double ej = (lane < k) ? exp((double)my_x - (double)mx) : 0.0;
+    wj = ej / wsum_f64(ej);
+  }
+  wj *= (double)scale;
+  if (lane < k) {
+    ids[(size_t)t * k + lane] = my_id;
+    w[(size_t)t * k + lane] = __double2float_rn(wj);
+    atomicAdd(&s_hist[my_id], 1);
+  }
+}
+
+// shared memory of route_topk8p_kernel: histogram, padded bias, then (128-byte aligned) one 4-token staging buffer and
+// one mbarrier per warp, then the block's tile counter
+constexpr int ROUTE8P_WARPS = 32;      // ONE block of 32 warps per SM (64 registers per thread: the whole register file)
 template <int VPL>
-vibe_status launch_route8(const RouteParams& p, bool sigmoid, cudaStream_t st) {
-  int blocks = (p.T + 31) / 32;
-  const int cap = num_sms() * 8;
+__host__ __device__ constexpr size_t route8p_stage_off(bool sigmoid) {
+  return ((size_t)8 * VPL * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0) + 127) & ~(size_t)127;
+}
+template <int VPL>
+__host__ __device__ constexpr size_t route8p_smem_bytes(bool sigmoid) {
+  return route8p_stage_off<VPL>(sigmoid) + (size_t)ROUTE8P_WARPS * 4 * 8 * VPL * sizeof(float) +
+         ROUTE8P_WARPS * sizeof(uint64_t) + 16;
+}
+
+template <int VPL, bool SIGMOID>
+__global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(const RouteParams p) {
+  constexpr int NW = ROUTE8P_WARPS;
+  extern __shared__ __align__(128) int s_mem[];
+  constexpr int E = 8 * VPL;
+  constexpr uint32_t TILE_BYTES = 4u * E * sizeof(float);
+  int* s_hist = s_mem;
+  float* s_bias = reinterpret_cast<float*>(s_mem + E);        // [8][VPL + 1]: lane-major, padded (conflict-free)
+  char* s_stage = reinterpret_cast<char*>(s_mem) + route8p_stage_off<VPL>(SIGMOID);
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const uint32_t my_stage = ptx::smem_u32(s_stage + (size_t)warp * TILE_BYTES);
+  const uint32_t my_bar = ptx::smem_u32(s_stage + (size_t)NW * TILE_BYTES + (size_t)warp * sizeof(uint64_t));
+  // The logits of a warp's NEXT tile (four consecutive tokens: 4 KB / 2 KB contiguous) are fetched by one bulk copy
+  // into the warp's staging buffer while the warp works on the current tile from registers: the DRAM latency, which
+  // the 64-register / 8-warps-per-scheduler budget cannot hide with loads into registers, is off the critical path.
+  const int n_tiles = (p.T + 3) >> 2;
+  auto fetch = [&](int tile) {
+    const int ntok = min(4, p.T - tile * 4);
+    const uint32_t bytes = (uint32_t)ntok * E * (uint32_t)sizeof(float);
+    ptx::mbar_arrive_expect_tx(my_bar, bytes);
+    ptx::bulk_load_1d(my_stage, p.logits + (size_t)tile * 4 * E, bytes, my_bar);
+  };
+  // Tiles of four tokens; block b (one per SM) owns tiles b, b + G, b + 2G, ... (G = grid size) and hands them to its
+  // 32 warps on demand (shared counter): a warp that took the exact-selection or the head-rebuild path, or that the
+  // scheduler served less often, simply takes fewer tiles, and all warps of the SM end together.  With a static
+  // assignment to four blocks of 8 warps per SM the blocks of one SM ended between 12 and 27 us of a 30 us kernel
+  // (64K tokens x 256 experts, in-kernel timestamps).
+  int* s_next = reinterpret_cast<int*>(s_stage + (size_t)NW * TILE_BYTES + NW * sizeof(uint64_t));
+  if (threadIdx.x == 0) *s_next = NW;
+  int tile = warp * gridDim.x + blockIdx.x;
+#ifdef ROUTE_TRACE
+  unsigned long long tr0, tr1 = 0, tr2;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr0));
+#endif
+  if (lane == 0) {
+    ptx::mbar_init(my_bar, 1);
+    ptx::fence_barrier_init();
+    if (tile < n_tiles) fetch(tile);
+  }
+  for (int i = threadIdx.x; i < E; i += blockDim.x) {
+    s_hist[i] = 0;
+    if (SIGMOID) s_bias[(i / VPL) * (VPL + 1) + i % VPL] = p.bias != nullptr ? p.bias[i] : 0.0f;
+  }
+  __syncthreads();
+  constexpr unsigned FULL = 0xffffffffu;       // full-mask collectives that stay inside the 8-lane groups (see above)
+  const int sub = lane & 7;
+  const int gbase = lane & ~7;
+  auto gmax_u32 = [&](uint32_t v) {
+    v = max(v, __shfl_xor_sync(FULL, v, 1));
+    v = max(v, __shfl_xor_sync(FULL, v, 2));
+    return max(v, __shfl_xor_sync(FULL, v, 4));
+  };
+  auto gsum_f64 = [&](double v) {
+    v += __shfl_xor_sync(FULL, v, 4);
+    v += __shfl_xor_sync(FULL, v, 2);
+    return v + __shfl_xor_sync(FULL, v, 1);
+  };
+  const uint32_t e0 = (uint32_t)(sub * VPL);
+  const int k = p.k;
+  const float* my_bias = s_bias + sub * (VPL + 1);
+  // f32 key -> order-preserving u32 with the low byte set (the caller subtracts the index): -0 -> +0 first
+  auto packed_hi = [](float key) {
+    const uint32_t b = __float_as_uint(__fadd_rn(key, 0.0f));
+    const uint32_t t = (uint32_t)((int32_t)b >> 31) | 0x80000000u;
+    return (b ^ t) | 0xffu;
+  };
+  // a lane's VPL consecutive experts are CH 16-byte chunks of the staged row; the lanes of a quarter-warp read them
+  // in rotated order (chunk (q + rot) mod CH at step q), which spreads the 8 lanes over all 32 banks
+  constexpr int CH = VPL / 4;
+  const int rot = sub / (8 / CH);
+  const uint4* my_row4 = reinterpret_cast<const uint4*>(s_stage + (size_t)warp * TILE_BYTES) + (lane >> 3) * (E / 4) + sub * CH;
+
+  uint32_t phase = 0;
+  while (tile < n_tiles) {
+    const int tbase = tile * 4;
+    const int tt = tbase + (lane >> 3);
+    const bool valid = tt < p.T;
+    const int t = valid ? tt : p.T - 1;
+    const float* row = p.logits + (size_t)t * E;
+    uint32_t pk[VPL];                          // packed keys with the IN-LANE index (low byte 255 - v)
+    uint32_t lowor = 0;                        // OR of the raw key bits (its low byte: are all low bytes zero?)
+    ptx::mbar_wait(my_bar, phase);
+#ifdef ROUTE_TRACE
+    if (phase == 0 && tr1 == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr1));
+#endif
+    phase ^= 1u;
+#pragma unroll
+    for (int q = 0; q < CH; ++q) {
+      const int ch = (q + rot) & (CH - 1);
+      const uint4 u = my_row4[ch];
+      const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const float key = SIGMOID ? __fadd_rn(vsig(xv[c]), my_bias[4 * ch + c]) : xv[c];
+        lowor |= __float_as_uint(key);
+        pk[4 * q + c] = packed_hi(key) - (uint32_t)(4 * ch) - (uint32_t)c;
+      }
+    }
+    // every lane has consumed its part of the buffer: the next tile's copy may overwrite it
+    __syncwarp();
+    {
+      int nxt = 0;
+      if (lane == 0) {
+        nxt = atomicAdd(s_next, 1) * (int)gridDim.x + (int)blockIdx.x;
+        if (nxt < n_tiles) fetch(nxt);
+      }
+      tile = __shfl_sync(FULL, nxt, 0);      // (the rest of this iteration addresses its tile through t / row only)
+    }
+    // ---- the lane's four largest, sorted; then the lane's first expert goes into the index byte ----
+    uint32_t h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+#pragma unroll
+    for (int q = 0; q < VPL / 4; ++q) merge_quad(h0, h1, h2, h3, pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+    h0 -= e0; h1 -= e0; h2 -= e0; h3 -= e0;
+    // ---- k rounds: group max; the one lane that holds it pops ----
+    uint32_t lk = 0xffffffffu, my_p = 0;
+    bool dry = false;
+    for (int j = 0; j < k; ++j) {
+      const uint32_t gm = gmax_u32(h0);
+      if (sub == j) my_p = gm;
+      if (h0 == gm) { lk = h0; h0 = h1; h1 = h2; h2 = h3; h3 = 0u; }
+      const bool need = (h0 == 0u) && !dry;
+      if (__any_sync(FULL, need)) {            // rare: a lane gave away all four heads -> its next four below lk
+        const uint32_t lim = need ? lk + e0 : 0u;
+        uint32_t r0 = 0, r1 = 0, r2 = 0, r3 = 0;
+#pragma unroll
+        for (int q = 0; q < VPL / 4; ++q) {
+          uint32_t c4[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) c4[c] = pk[4 * q + c] < lim ? pk[4 * q + c] : 0u;
+          merge_quad(r0, r1, r2, r3, c4[0], c4[1], c4[2], c4[3]);
+        }
+        if (need) {
+          h0 = r0 ? r0 - e0 : 0u; h1 = r1 ? r1 - e0 : 0u; h2 = r2 ? r2 - e0 : 0u; h3 = r3 ? r3 - e0 : 0u;
+          dry = (h0 == 0u);
+        }
+      }
+    }
+    int my_id = 255 - (int)(my_p & 0xffu);
+    bool redo = false;
+    // ---- is the packed order the exact one?  picks and the best remaining key must differ in their upper 24 bits ----
+    {
+      const uint32_t p9 = gmax_u32(h0);
+      uint32_t nxt = __shfl_down_sync(FULL, my_p, 1);
+      if (sub == k - 1) nxt = p9;
+      const bool collide = (sub < k) && ((my_p ^ nxt) < 256u);
+      const unsigned cb = __ballot_sync(FULL, collide);
+      if (cb != 0u) {
+        // equal upper bits: exact ties if the low bytes of all keys of the token are zero, else the token is redone
+        uint32_t lo = lowor;
+        lo |= __shfl_xor_sync(FULL, lo, 1);
+        lo |= __shfl_xor_sync(FULL, lo, 2);
+        lo |= __shfl_xor_sync(FULL, lo, 4);
+        redo = ((cb >> gbase) & 0xffu) != 0u && (lo & 0xffu) != 0u && valid;
+        const unsigned rb = __ballot_sync(FULL, redo);
+        for (int g = 0; g < 4; ++g)
+          if ((rb >> (8 * g)) & 1u) route_exact_token<VPL, SIGMOID>(p.logits, p.ids, p.w, k, p.renorm, p.scale, tbase + g, s_hist, s_bias);
+      }
+    }
+    // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
+    const float my_x = (sub < k) ? __ldg(row + my_id) : 0.0f;
+    double wj;
+    if (SIGMOID) {
+      const double sj = (sub < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
+      wj = sj;
+      if (p.renorm) wj = sj / gsum_f64(sj);
+    } else {
+      const float mx = __shfl_sync(FULL, my_x, gbase);      // the first pick is the row maximum
+      const double ej = (sub < k) ? exp((double)my_x - (double)mx) : 0.0;
+      wj = ej / gsum_f64(ej);                               // renormalised: the denominator over all experts cancels
+    }
+    wj *= (double)p.scale;
+    if (sub < k && valid && !redo) {
+      p.ids[(size_t)t * k + sub] = my_id;
+      p.w[(size_t)t * k + sub] = __double2float_rn(wj);
+      atomicAdd(&s_hist[my_id], 1);
+    }
+  }
+#ifdef ROUTE_TRACE
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr2));
+#endif
+  __syncthreads();
+  for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
+    const int c = s_hist[i];
+    if (c) atomicAdd(&p.counts[i], c);
+  }
+#ifdef ROUTE_TRACE
+  if (lane == 0) {          // debug build only: the trace overwrites the first gate weights
+    unsigned long long tr3;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr3));
+    unsigned long long* o = reinterpret_cast<unsigned long long*>(p.w) + (size_t)(blockIdx.x * NW + warp) * 5;
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    o[0] = tr0; o[1] = tr1; o[2] = tr2; o[3] = tr3; o[4] = smid;
+  }
+#endif
+}
+
+template <int VPL>
+vibe_status launch_route8(const RouteParams& p, bool sigmoid, bool packed, cudaStream_t st) {
+  // one resident wave (4 blocks of 8 warps per SM), tiles of four tokens interleaved over warps and blocks
+  int blocks = ((p.T + 3) / 4 + 7) / 8;
+  const int cap = num_sms() * ROUTE8_MIN_BLOCKS;
   if (blocks > cap) blocks = cap;
   const size_t smem = (size_t)p.E * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0);
+  if (packed) {
+    const size_t psmem = route8p_smem_bytes<VPL>(sigmoid);
+    static std::mutex mu;
+    static bool done[kMaxDevices] = {};
+    {
+      std::lock_guard<std::mutex> lk(mu);
+      const int dev = current_device();
+      if (!done[dev]) {      // the opt-in to > 48 KB of dynamic shared memory is per device
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)route8p_smem_bytes<VPL>(true)));
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)route8p_smem_bytes<VPL>(false)));
+        done[dev] = true;
+      }
+    }
+    int pblocks = ((p.T + 3) / 4 + ROUTE8P_WARPS - 1) / ROUTE8P_WARPS;
+    if (pblocks > num_sms()) pblocks = num_sms();
+    if (sigmoid)
+      route_topk8p_kernel<VPL, true><<<pblocks, ROUTE8P_WARPS * 32, psmem, st>>>(p);
+    else
+      route_topk8p_kernel<VPL, false><<<pblocks, ROUTE8P_WARPS * 32, psmem, st>>>(p);
+    VIBE_LAUNCH_CHECK("route_topk8p_kernel");
+    return VIBE_OK;
+  }
   if (sigmoid)
     route_topk8_kernel<VPL, true><<<blocks, 256, smem, st>>>(p);
   else
@@ -545,7 +897,9 @@ extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* l
   // for every other configuration -- measured --, so this one combination takes the 32-lane kernel)
   if ((E == 128 || E == 256) && k <= 8 && (ng == 0 || (ng == 8 && (sig || cfg->renormalize)))) {
     p.fast_groups = 1;
-    return E == 256 ? launch_route8<32>(p, sig, st) : launch_route8<16>(p, sig, st);
+    // packed one-register keys where the gate weights need the picked logits only and there is no group score
+    const bool packed = ng == 0 && (sig || cfg->renormalize);
+    return E == 256 ? launch_route8<32>(p, sig, packed, st) : launch_route8<16>(p, sig, packed, st);
   }
   int lanes, vpl;
   if (E <= 64 && k <= 8) {

@@ -496,6 +496,15 @@ def section_profile(peaks, quick):
         for j, r in enumerate(m0):
             r["fp8_latency_us"] = round(float(lat8[j]), 3)
         del W1q, W3q, W2q
+        # ... and for the BLOCK-SCALED FP8 FFN (segments padded to 64 rows: l(n) is a step function of n)
+        W1m, sf13 = B.mxfp8_pack_weights(W1, B.MX_ROLE_GATE)
+        W3m, sf13 = B.mxfp8_pack_weights(W3, B.MX_ROLE_UP, sf=sf13)
+        W2m, sf2 = B.mxfp8_pack_weights(W2, B.MX_ROLE_DOWN)
+        latm = B.profile_expert_latency_mxfp8(W1m, W3m, sf13, W2m, sf2, B.DEFAULT_SWEEP[::-1], mode=0,
+                                              warmup=10 if quick else 30, iters=20 if quick else 100)[::-1]
+        for j, r in enumerate(m0):
+            r["mxfp8_latency_us"] = round(float(latm[j]), 3)
+        del W1m, W3m, W2m
         out[cfg.name] = {"E_loc": E, "d": d, "f": f, "rows": rows}
         del W1, W3, W2
         torch.cuda.empty_cache()
@@ -706,12 +715,12 @@ def write_markdown(r, path, command):
         o.append("\n## profile: per-expert latency l(n) [us], median of 100 calls per point (p10..p90), modes 0 (all experts n rows; time / E_loc) and 1 (one expert n rows)\n")
         for name,p in r['profile'].items():
             o.append(f"### {name}: E_loc={p['E_loc']} d={p['d']} f={p['f']}\n")
-            o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 | FP8 mode 0 us |\n|---|---|---|---|---|---|---|---|---|")
+            o.append("| n | mode 0 us | p10 | p90 | weight-stream floor us | mode 1 us | p10 | p90 | per-tensor FP8 mode 0 us | block-scaled FP8 mode 0 us |\n|---|---|---|---|---|---|---|---|---|---|")
             m0={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==0}
             m1={x['tokens_per_expert']:x for x in p['rows'] if x['mode']==1}
             for n in sorted(m0):
                 a,b=m0[n],m1[n]
-                o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} | {a.get('fp8_latency_us')} |")
+                o.append(f"| {n} | {a['latency_us']} | {a['p10_us']} | {a['p90_us']} | {a['weight_stream_floor_us']} | {b['latency_us']} | {b['p10_us']} | {b['p90_us']} | {a.get('fp8_latency_us')} | {a.get('mxfp8_latency_us')} |")
             o.append("")
     if "placement_stress" in r:
         o.append("## placement_stress (BASELINE.json configs[4]): 256 experts -> 8 virtual GPUs, sigma ~ U[0.78,1.0] (8 seeds), measured C3-shape profile\n")

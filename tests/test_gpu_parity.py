@@ -129,6 +129,42 @@ def test_route_adversarial_ties_and_degenerate():
     check_route(big, dict(num_experts=E, top_k=k, score_fn=1, renormalize=1))
 
 
+@pytest.mark.parametrize("E,k", [(256, 8), (128, 8), (256, 5), (128, 3)])
+def test_route_packed_keys_ties_and_near_ties(E, k):
+    """The packed-key kernel of the 128- / 256-expert configs (route.cu, route_topk8p_kernel): its keys keep the upper
+    24 bits of the f32 key, so exact ties, keys that differ in the low byte only, more than four picks from one
+    lane and a ragged last tile must all come out as the oracle's (key descending, index ascending) order."""
+    rng = np.random.default_rng(E * 10 + k)
+    T = 1027
+    kws = [dict(num_experts=E, top_k=k), dict(num_experts=E, top_k=k, score_fn=1),
+           dict(num_experts=E, top_k=k, score_fn=1, renormalize=0, routed_scale=2.5)]
+    # (a) all equal; (b) half-integer logits: exact ties with zero low bytes
+    same = np.full((T, E), -1.5, np.float32)
+    ids, _, _ = check_route(same, kws[0])
+    assert np.array_equal(ids, np.tile(np.arange(k), (T, 1)))
+    q = (np.round(I.make_logits(T, E, 1.0, 5) * 2) / 2).astype(np.float32)
+    # (c) the same values moved by a few ulps: equal upper 24 bits, different low bytes (both signs)
+    near = (q.view(np.int32) + rng.integers(0, 200, size=q.shape, dtype=np.int32)).view(np.float32)
+    # (d) zeros of both signs among small values
+    z = (rng.standard_normal((T, E)) * 1e-3).astype(np.float32)
+    z[rng.random((T, E)) < 0.3] = 0.0
+    z[rng.random((T, E)) < 0.3] = -0.0
+    # (e) one lane's experts (consecutive indices) hold all the large logits; with near-ties among them
+    vpl = E // 8
+    lane = I.make_logits(T, E, 0.0, 6).astype(np.float32)
+    lane[:, 3 * vpl:4 * vpl] += 50.0
+    lane2 = lane.copy()
+    lane2[:, 3 * vpl:4 * vpl] = (np.float32(40.0).view(np.int32)
+                                 + rng.integers(0, 3, size=(T, vpl), dtype=np.int32)).view(np.float32)
+    for kw in kws:
+        for x in (q, near, z, lane, lane2):
+            check_route(np.ascontiguousarray(x), kw)
+    # a select bias with near-ties of the biased sigmoid keys
+    bias = (rng.integers(0, 4, size=E) * 0.25).astype(np.float32)
+    check_route(q, kws[1], bias)
+    check_route(near, kws[1], bias)
+
+
 def test_route_empty_batch():
     rc = B.RouteConfig(num_experts=16, top_k=2)
     logits = torch.empty((0, 16), dtype=torch.float32, device="cuda")
