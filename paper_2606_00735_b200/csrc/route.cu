@@ -7,6 +7,10 @@
 // expert index" rule for free (lane-major element order).  The histogram is privatised in
 // shared memory per block and merged with one global atomic per non-empty bin.
 // Gate weights are evaluated in fp64 for the k picked experts only.
+// Three kernels: route_topk_kernel (any E <= 512, k <= 32, any grouping), route_topk8_kernel (E = 128 | 256, k <= 8,
+// four tokens per warp, (key, index) pairs) and route_topk8p_kernel (the same shapes without group limiting: packed
+// one-register keys, merge networks, staged logits -- the fast path of the 128- / 256-expert softmax configs).
+// The counts are zeroed by a one-block kernel that the route kernel overlaps (programmatic dependent launch).
 //
 // Semantics: include/vibe.h (vibe_route_topk), readings R1-R8.
 #include <mutex>
@@ -16,6 +20,13 @@
 
 namespace vibe {
 namespace {
+
+// counts <- 0.  The route kernels are launched with programmatic stream serialisation behind it: they start while it
+// runs (everything older in the stream is complete: it is an ordinary launch) and wait for it (griddepcontrol.wait)
+// only before they add their block histograms to the counts, so the zeroing costs no dependent launch latency.
+__global__ void route_zero_counts_kernel(int32_t* counts, int E) {
+  for (int i = threadIdx.x; i < E; i += blockDim.x) counts[i] = 0;
+}
 
 struct RouteParams {
   const float* logits;
@@ -281,6 +292,7 @@ __global__ void __launch_bounds__(256) route_topk_kernel(const RouteParams p) {
     }
   }
   __syncthreads();
+  ptx::griddep_wait();       // the kernel that zeroes the counts is the predecessor in the stream (see vibe_route_topk)
   for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
     const int c = s_hist[i];
     if (c) atomicAdd(&p.counts[i], c);
@@ -463,6 +475,7 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
     }
   }
   __syncthreads();
+  ptx::griddep_wait();       // the kernel that zeroes the counts is the predecessor in the stream (see vibe_route_topk)
   for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
     const int c = s_hist[i];
     if (c) atomicAdd(&p.counts[i], c);
@@ -475,18 +488,24 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
 // two cases whose gate weights need the picked logits only).  ncu of route_topk8_kernel at 64K x 256 (profiles/
 // r2_route_ncu.md): 390 warp-instructions per token, three quarters of them on the ALU pipe (ISETP/SEL/LOP3/VIMNMX:
 // one warp-instruction per two cycles), most of them the (key, index) pairs dragged through the per-lane sorted
-// insertion and the five-instruction order-preserving map.  Here a key is ONE register: the order-preserving u32
-// image of the f32 key with its low 8 bits replaced by 255 - expert index, so keys are unique, ties go to the
-// lowest index by construction, a lane's first four are found by min/max sorting networks (5.1 VIMNMX per element
-// instead of 13 compare/select), a selection round is a group max and one compare (no ballot / find-first /
-// indexed shuffle), and the winner's index comes out of the key.
+// insertion and the k selection rounds.  Here a key is ONE register: the order-preserving u32 image of the f32 key
+// with its low 8 bits replaced by 255 - expert index, so keys are unique and ties go to the lowest index by
+// construction.  A lane's first four (and its fifth) come out of min/max sorting networks, the group's first eight
+// out of a three-level bitonic merge tree over the 8 lanes (20 shuffles, no ballot / find-first / indexed shuffle,
+// no rounds), and the winners' indices out of the keys.
 // The packed order differs from the exact one only between keys that agree in their upper 24 bits without being
-// equal.  After the k rounds the k picks and the best remaining key are in packed order; if all adjacent pairs
-// differ in the upper 24 bits, every pick is strictly above every other key of the token in exact order too and
-// the result is exact.  Otherwise (about 3 tokens in 1000 on continuous f32 logits) the warp reloads the exact
-// keys: if the low bytes of ALL keys of the token are zero (bf16- or fp16-valued logits, where exact ties are
-// common), equal upper bits mean equal keys and the packed tie-break is the exact one; else the token is redone
-// by the exact selection below (k rounds of a full rescan; slow and rare).
+// equal.  The tree leaves the picks in packed order and a bound on every key that was not picked (what its
+// half-cleaners dropped and the lanes' fifths); if all adjacent pairs of {picks, bound} differ in the upper 24 bits,
+// every pick is strictly above every other key of the token in exact order too and the result is exact.  Otherwise
+// (about 3 tokens in 1000 on continuous f32 logits) the lanes OR the raw bits of the token's keys: if the low bytes
+// of ALL keys are zero (bf16- or fp16-valued logits, where exact ties are common), equal upper bits mean equal keys
+// and the packed tie-break is the exact one; else the token is redone by route_exact_token (one token per warp on
+// exact keys).  A token of which one lane holds five or more picks (its fifth is above the last pick: 1 in 100)
+// is redone the same way.
+// The kernel is bound by the ALU pipe (about 520 of its 800 warp-instructions per 4-token tile).  What surrounds the
+// arithmetic is arranged so that the pipe stays busy: the logits of a warp's next tile arrive by a bulk copy while it
+// works on the current one, one block per SM hands tiles to its warps on demand, and the zeroing of the counts
+// overlaps the kernel (programmatic dependent launch).  64K tokens x 256 experts, top-8: 44.0 -> 23 us.
 // ------------------------------------------------------------------------------------------------------------
 #define VIBE_CSWAP(a, b)                     \
   {                                          \
@@ -518,6 +537,49 @@ __device__ __forceinline__ void merge_quad(uint32_t& h0, uint32_t& h1, uint32_t&
 // ballot, lowest lane wins}): the packed-key kernel calls it for the few tokens whose packed order is not provably the
 // exact one.  Writes the token's ids / weights and counts it in the block histogram.  No group limiting; sigmoid, or
 // softmax with renormalisation (the configurations of the packed-key kernel).
+// merge_quad that also keeps r5, the fifth largest seen so far (the largest key the half-cleaner drops)
+__device__ __forceinline__ void merge_quad5(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t& r5, uint32_t a,
+                                            uint32_t b, uint32_t c, uint32_t d) {
+  VIBE_CSWAP(a, b);
+  VIBE_CSWAP(c, d);
+  VIBE_CSWAP(a, c);
+  VIBE_CSWAP(b, d);
+  VIBE_CSWAP(b, c);          // a >= b >= c >= d
+  r5 = __vimax3_u32(r5, min(h0, d), min(h1, c));
+  r5 = __vimax3_u32(r5, min(h2, b), min(h3, a));
+  h0 = max(h0, d);
+  h1 = max(h1, c);
+  h2 = max(h2, b);
+  h3 = max(h3, a);
+  VIBE_CSWAP(h0, h2);
+  VIBE_CSWAP(h1, h3);
+  VIBE_CSWAP(h0, h1);
+  VIBE_CSWAP(h2, h3);
+}
+// one step of the cross-lane merge tree: against the partner's (q0..q3) the lane keeps the larger (or, low = true, the
+// smaller) of every pair -- a bitonic four -- and sorts them
+__device__ __forceinline__ void tree_exchange(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t q0, uint32_t q1,
+                                              uint32_t q2, uint32_t q3, bool low) {
+  h0 = low ? min(h0, q0) : max(h0, q0);
+  h1 = low ? min(h1, q1) : max(h1, q1);
+  h2 = low ? min(h2, q2) : max(h2, q2);
+  h3 = low ? min(h3, q3) : max(h3, q3);
+  VIBE_CSWAP(h0, h2);
+  VIBE_CSWAP(h1, h3);
+  VIBE_CSWAP(h0, h1);
+  VIBE_CSWAP(h2, h3);
+}
+// half-cleaner against the partner's reversed four: keep the larger of every pair, remember the largest dropped key
+__device__ __forceinline__ void tree_halfclean(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t& dmax,
+                                               uint32_t q0, uint32_t q1, uint32_t q2, uint32_t q3) {
+  dmax = __vimax3_u32(dmax, min(h0, q0), min(h1, q1));
+  dmax = __vimax3_u32(dmax, min(h2, q2), min(h3, q3));
+  h0 = max(h0, q0);
+  h1 = max(h1, q1);
+  h2 = max(h2, q2);
+  h3 = max(h3, q3);
+}
+
 template <int VPL, bool SIGMOID>
 __device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids, float* w, int k, int renorm, float scale,
                                                int t, int* s_hist, const float* s_bias) {
@@ -581,20 +643,22 @@ __device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids
 
 // shared memory of route_topk8p_kernel: histogram, padded bias, then (128-byte aligned) one 4-token staging buffer and
 // one mbarrier per warp, then the block's tile counter
-constexpr int ROUTE8P_WARPS = 32;      // ONE block of 32 warps per SM (64 registers per thread: the whole register file)
+#ifndef ROUTE8P_WARPS_N
+#define ROUTE8P_WARPS_N 28
+#endif
+constexpr int ROUTE8P_WARPS = ROUTE8P_WARPS_N;      // ONE block of up to 28 warps per SM (72 registers per thread; with 32 warps of 64 registers the merge networks spill)
 template <int VPL>
 __host__ __device__ constexpr size_t route8p_stage_off(bool sigmoid) {
   return ((size_t)8 * VPL * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0) + 127) & ~(size_t)127;
 }
 template <int VPL>
-__host__ __device__ constexpr size_t route8p_smem_bytes(bool sigmoid) {
-  return route8p_stage_off<VPL>(sigmoid) + (size_t)ROUTE8P_WARPS * 4 * 8 * VPL * sizeof(float) +
-         ROUTE8P_WARPS * sizeof(uint64_t) + 16;
+__host__ __device__ constexpr size_t route8p_smem_bytes(bool sigmoid, int warps) {
+  return route8p_stage_off<VPL>(sigmoid) + (size_t)warps * 4 * 8 * VPL * sizeof(float) + warps * sizeof(uint64_t) + 16;
 }
 
 template <int VPL, bool SIGMOID>
 __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(const RouteParams p) {
-  constexpr int NW = ROUTE8P_WARPS;
+  const int NW = blockDim.x >> 5;
   extern __shared__ __align__(128) int s_mem[];
   constexpr int E = 8 * VPL;
   constexpr uint32_t TILE_BYTES = 4u * E * sizeof(float);
@@ -616,8 +680,8 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     ptx::bulk_load_1d(my_stage, p.logits + (size_t)tile * 4 * E, bytes, my_bar);
   };
   // Tiles of four tokens; block b (one per SM) owns tiles b, b + G, b + 2G, ... (G = grid size) and hands them to its
-  // 32 warps on demand (shared counter): a warp that took the exact-selection or the head-rebuild path, or that the
-  // scheduler served less often, simply takes fewer tiles, and all warps of the SM end together.  With a static
+  // warps on demand (shared counter): a warp that had to redo tokens on exact keys, or that the scheduler served
+  // less often, simply takes fewer tiles, and all warps of the SM end together.  With a static
   // assignment to four blocks of 8 warps per SM the blocks of one SM ended between 12 and 27 us of a 30 us kernel
   // (64K tokens x 256 experts, in-kernel timestamps).
   int* s_next = reinterpret_cast<int*>(s_stage + (size_t)NW * TILE_BYTES + NW * sizeof(uint64_t));
@@ -673,7 +737,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     const int t = valid ? tt : p.T - 1;
     const float* row = p.logits + (size_t)t * E;
     uint32_t pk[VPL];                          // packed keys with the IN-LANE index (low byte 255 - v)
-    uint32_t lowor = 0;                        // OR of the raw key bits (its low byte: are all low bytes zero?)
     ptx::mbar_wait(my_bar, phase);
 #ifdef ROUTE_TRACE
     if (phase == 0 && tr1 == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr1));
@@ -687,7 +750,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         const float key = SIGMOID ? __fadd_rn(vsig(xv[c]), my_bias[4 * ch + c]) : xv[c];
-        lowor |= __float_as_uint(key);
         pk[4 * q + c] = packed_hi(key) - (uint32_t)(4 * ch) - (uint32_t)c;
       }
     }
@@ -701,72 +763,94 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
       }
       tile = __shfl_sync(FULL, nxt, 0);      // (the rest of this iteration addresses its tile through t / row only)
     }
-    // ---- the lane's four largest, sorted; then the lane's first expert goes into the index byte ----
-    uint32_t h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+    // ---- the lane's four largest, sorted, and its fifth (r5); then the lane's first expert goes into the index byte ----
+    uint32_t h0 = 0, h1 = 0, h2 = 0, h3 = 0, r5 = 0;
 #pragma unroll
-    for (int q = 0; q < VPL / 4; ++q) merge_quad(h0, h1, h2, h3, pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
-    h0 -= e0; h1 -= e0; h2 -= e0; h3 -= e0;
-    // ---- k rounds: group max; the one lane that holds it pops ----
-    uint32_t lk = 0xffffffffu, my_p = 0;
-    bool dry = false;
-    for (int j = 0; j < k; ++j) {
-      const uint32_t gm = gmax_u32(h0);
-      if (sub == j) my_p = gm;
-      if (h0 == gm) { lk = h0; h0 = h1; h1 = h2; h2 = h3; h3 = 0u; }
-      const bool need = (h0 == 0u) && !dry;
-      if (__any_sync(FULL, need)) {            // rare: a lane gave away all four heads -> its next four below lk
-        const uint32_t lim = need ? lk + e0 : 0u;
-        uint32_t r0 = 0, r1 = 0, r2 = 0, r3 = 0;
-#pragma unroll
-        for (int q = 0; q < VPL / 4; ++q) {
-          uint32_t c4[4];
-#pragma unroll
-          for (int c = 0; c < 4; ++c) c4[c] = pk[4 * q + c] < lim ? pk[4 * q + c] : 0u;
-          merge_quad(r0, r1, r2, r3, c4[0], c4[1], c4[2], c4[3]);
-        }
-        if (need) {
-          h0 = r0 ? r0 - e0 : 0u; h1 = r1 ? r1 - e0 : 0u; h2 = r2 ? r2 - e0 : 0u; h3 = r3 ? r3 - e0 : 0u;
-          dry = (h0 == 0u);
-        }
-      }
+    for (int q = 0; q < VPL / 4; ++q)
+      merge_quad5(h0, h1, h2, h3, r5, pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+    h0 -= e0; h1 -= e0; h2 -= e0; h3 -= e0; r5 -= e0;
+    // ---- the group's eight largest heads by a bitonic merge tree over the 8 lanes (three levels) ----
+    // Level L merges the sorted 8 of two 2^(L-1)-lane halves: half-cleaner against the reversed partner list (all
+    // lanes keep the larger: both halves then hold the 8 largest, as mirrored copies), one exchange between the lane
+    // with the upper and the lane with the lower four, a local bitonic sort.  After level 3 the lanes of even parity
+    // (0, 3, 5, 6) hold picks 1..4 and those of odd parity (1, 2, 4, 7) picks 5..8, sorted, in h0..h3.  What the
+    // half-cleaners drop, and the lanes' fifths, bound everything that was not picked (dmax).
+    uint32_t dmax = r5;
+    {
+      const bool low1 = (sub & 1) != 0;
+      tree_exchange(h0, h1, h2, h3, __shfl_xor_sync(FULL, h3, 1), __shfl_xor_sync(FULL, h2, 1),
+                    __shfl_xor_sync(FULL, h1, 1), __shfl_xor_sync(FULL, h0, 1), low1);
+      const bool low2 = (__popc(sub & 3) & 1) != 0;
+      tree_halfclean(h0, h1, h2, h3, dmax, __shfl_xor_sync(FULL, h3, 3), __shfl_xor_sync(FULL, h2, 3),
+                     __shfl_xor_sync(FULL, h1, 3), __shfl_xor_sync(FULL, h0, 3));
+      tree_exchange(h0, h1, h2, h3, __shfl_xor_sync(FULL, h0, 1), __shfl_xor_sync(FULL, h1, 1),
+                    __shfl_xor_sync(FULL, h2, 1), __shfl_xor_sync(FULL, h3, 1), low2);
+      tree_halfclean(h0, h1, h2, h3, dmax, __shfl_xor_sync(FULL, h3, 5), __shfl_xor_sync(FULL, h2, 5),
+                     __shfl_xor_sync(FULL, h1, 5), __shfl_xor_sync(FULL, h0, 5));
     }
+    const bool low3 = (__popc(sub) & 1) != 0;
+    tree_exchange(h0, h1, h2, h3, __shfl_xor_sync(FULL, h0, 1), __shfl_xor_sync(FULL, h1, 1),
+                  __shfl_xor_sync(FULL, h2, 1), __shfl_xor_sync(FULL, h3, 1), low3);
+    // this lane's pick: number myj in the order of the picks
+    const int slot = sub >> 1;
+    const int myj = (low3 ? 4 : 0) + slot;
+    const uint32_t my_p = slot == 0 ? h0 : slot == 1 ? h1 : slot == 2 ? h2 : h3;
     int my_id = 255 - (int)(my_p & 0xffu);
     bool redo = false;
-    // ---- is the packed order the exact one?  picks and the best remaining key must differ in their upper 24 bits ----
+    // ---- is the packed order the exact one?  the picks and the best key that was not picked must differ in their
+    //      upper 24 bits; a key above the last pick that was not picked (a lane with five or more of the picks: its
+    //      heads ran out) sends the token to the exact routine too ----
     {
-      const uint32_t p9 = gmax_u32(h0);
-      uint32_t nxt = __shfl_down_sync(FULL, my_p, 1);
-      if (sub == k - 1) nxt = p9;
-      const bool collide = (sub < k) && ((my_p ^ nxt) < 256u);
+      const uint32_t rest = gmax_u32(dmax);
+      const uint32_t cross = __shfl_xor_sync(FULL, h0, 1);             // an upper lane reads pick 5 here
+      uint32_t nxt = slot == 0 ? h1 : slot == 1 ? h2 : slot == 2 ? h3 : (low3 ? 0u : cross);
+      if (myj == k - 1) nxt = max(nxt, rest);
+      const bool collide = (myj < k) && (((my_p ^ nxt) < 256u) || nxt > my_p);
       const unsigned cb = __ballot_sync(FULL, collide);
       if (cb != 0u) {
         // equal upper bits: exact ties if the low bytes of all keys of the token are zero, else the token is redone
-        uint32_t lo = lowor;
+        uint32_t lo = 0;                         // OR of the raw bits of the lane's keys (reloaded: L2 hits)
+        {
+          const uint4* grow4 = reinterpret_cast<const uint4*>(row + e0);
+#pragma unroll
+          for (int q = 0; q < CH; ++q) {
+            const uint4 u = __ldg(grow4 + q);
+            if (SIGMOID) {
+              const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+#pragma unroll
+              for (int c = 0; c < 4; ++c) lo |= __float_as_uint(__fadd_rn(vsig(xv[c]), my_bias[4 * q + c]));
+            } else {
+              lo |= u.x | u.y | u.z | u.w;
+            }
+          }
+        }
         lo |= __shfl_xor_sync(FULL, lo, 1);
         lo |= __shfl_xor_sync(FULL, lo, 2);
         lo |= __shfl_xor_sync(FULL, lo, 4);
-        redo = ((cb >> gbase) & 0xffu) != 0u && (lo & 0xffu) != 0u && valid;
+        const bool ran_out = (myj == k - 1) && nxt > my_p;
+        const unsigned ob = __ballot_sync(FULL, ran_out);
+        redo = ((((cb >> gbase) & 0xffu) != 0u && (lo & 0xffu) != 0u) || ((ob >> gbase) & 0xffu) != 0u) && valid;
         const unsigned rb = __ballot_sync(FULL, redo);
         for (int g = 0; g < 4; ++g)
           if ((rb >> (8 * g)) & 1u) route_exact_token<VPL, SIGMOID>(p.logits, p.ids, p.w, k, p.renorm, p.scale, tbase + g, s_hist, s_bias);
       }
     }
     // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
-    const float my_x = (sub < k) ? __ldg(row + my_id) : 0.0f;
+    const float my_x = (myj < k) ? __ldg(row + my_id) : 0.0f;
     double wj;
     if (SIGMOID) {
-      const double sj = (sub < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
+      const double sj = (myj < k) ? 1.0 / (1.0 + exp(-(double)my_x)) : 0.0;
       wj = sj;
       if (p.renorm) wj = sj / gsum_f64(sj);
     } else {
-      const float mx = __shfl_sync(FULL, my_x, gbase);      // the first pick is the row maximum
-      const double ej = (sub < k) ? exp((double)my_x - (double)mx) : 0.0;
+      const float mx = __shfl_sync(FULL, my_x, gbase);      // the first pick (lane 0 of the group) is the row maximum
+      const double ej = (myj < k) ? exp((double)my_x - (double)mx) : 0.0;
       wj = ej / gsum_f64(ej);                               // renormalised: the denominator over all experts cancels
     }
     wj *= (double)p.scale;
-    if (sub < k && valid && !redo) {
-      p.ids[(size_t)t * k + sub] = my_id;
-      p.w[(size_t)t * k + sub] = __double2float_rn(wj);
+    if (myj < k && valid && !redo) {
+      p.ids[(size_t)t * k + myj] = my_id;
+      p.w[(size_t)t * k + myj] = __double2float_rn(wj);
       atomicAdd(&s_hist[my_id], 1);
     }
   }
@@ -774,6 +858,7 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr2));
 #endif
   __syncthreads();
+  ptx::griddep_wait();       // the kernel that zeroes the counts is the predecessor in the stream (see vibe_route_topk)
   for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
     const int c = s_hist[i];
     if (c) atomicAdd(&p.counts[i], c);
@@ -798,7 +883,6 @@ vibe_status launch_route8(const RouteParams& p, bool sigmoid, bool packed, cudaS
   if (blocks > cap) blocks = cap;
   const size_t smem = (size_t)p.E * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0);
   if (packed) {
-    const size_t psmem = route8p_smem_bytes<VPL>(sigmoid);
     static std::mutex mu;
     static bool done[kMaxDevices] = {};
     {
@@ -806,25 +890,30 @@ vibe_status launch_route8(const RouteParams& p, bool sigmoid, bool packed, cudaS
       const int dev = current_device();
       if (!done[dev]) {      // the opt-in to > 48 KB of dynamic shared memory is per device
         VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)route8p_smem_bytes<VPL>(true)));
+                                       (int)route8p_smem_bytes<VPL>(true, ROUTE8P_WARPS)));
         VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)route8p_smem_bytes<VPL>(false)));
+                                       (int)route8p_smem_bytes<VPL>(false, ROUTE8P_WARPS)));
         done[dev] = true;
       }
     }
-    int pblocks = ((p.T + 3) / 4 + ROUTE8P_WARPS - 1) / ROUTE8P_WARPS;
+    // one block per SM; a small batch is spread over all SMs with fewer warps per block
+    const int n_tiles = (p.T + 3) / 4;
+    int warps = (n_tiles + num_sms() - 1) / num_sms();
+    warps = warps < 1 ? 1 : warps > ROUTE8P_WARPS ? ROUTE8P_WARPS : warps;
+    int pblocks = (n_tiles + warps - 1) / warps;
     if (pblocks > num_sms()) pblocks = num_sms();
+    const size_t psmem = route8p_smem_bytes<VPL>(sigmoid, warps);
     if (sigmoid)
-      route_topk8p_kernel<VPL, true><<<pblocks, ROUTE8P_WARPS * 32, psmem, st>>>(p);
+      (void)launch_pdl(route_topk8p_kernel<VPL, true>, dim3(pblocks), dim3(warps * 32), psmem, st, p);
     else
-      route_topk8p_kernel<VPL, false><<<pblocks, ROUTE8P_WARPS * 32, psmem, st>>>(p);
+      (void)launch_pdl(route_topk8p_kernel<VPL, false>, dim3(pblocks), dim3(warps * 32), psmem, st, p);
     VIBE_LAUNCH_CHECK("route_topk8p_kernel");
     return VIBE_OK;
   }
   if (sigmoid)
-    route_topk8_kernel<VPL, true><<<blocks, 256, smem, st>>>(p);
+    (void)launch_pdl(route_topk8_kernel<VPL, true>, dim3(blocks), dim3(256), smem, st, p);
   else
-    route_topk8_kernel<VPL, false><<<blocks, 256, smem, st>>>(p);
+    (void)launch_pdl(route_topk8_kernel<VPL, false>, dim3(blocks), dim3(256), smem, st, p);
   VIBE_LAUNCH_CHECK("route_topk8_kernel");
   return VIBE_OK;
 }
@@ -838,9 +927,9 @@ vibe_status launch_route(const RouteParams& p, bool sigmoid, cudaStream_t st) {
   size_t smem = (size_t)p.E * sizeof(int);
   if (p.n_group > 1 && !p.fast_groups) smem += (size_t)gpb * p.n_group * sizeof(float);
   if (sigmoid)
-    route_topk_kernel<LANES, VPL, true><<<blocks, 256, smem, st>>>(p);
+    (void)launch_pdl(route_topk_kernel<LANES, VPL, true>, dim3(blocks), dim3(256), smem, st, p);
   else
-    route_topk_kernel<LANES, VPL, false><<<blocks, 256, smem, st>>>(p);
+    (void)launch_pdl(route_topk_kernel<LANES, VPL, false>, dim3(blocks), dim3(256), smem, st, p);
   VIBE_LAUNCH_CHECK("route_topk_kernel");
   return VIBE_OK;
 }
@@ -873,7 +962,8 @@ extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* l
   VIBE_REQUIRE(E <= 512, VIBE_ERR_UNSUPPORTED, "vibe_route_topk: E > 512 not implemented");
   VIBE_REQUIRE(k <= 32, VIBE_ERR_UNSUPPORTED, "vibe_route_topk: k > 32 not implemented");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  VIBE_CUDA(cudaMemsetAsync(counts, 0, (size_t)E * sizeof(int32_t), st));
+  route_zero_counts_kernel<<<1, 256, 0, st>>>(counts, E);
+  VIBE_LAUNCH_CHECK("route_zero_counts_kernel");
   if (T == 0) return VIBE_OK;
 
   RouteParams p;
