@@ -8,8 +8,9 @@
 // shared memory per block and merged with one global atomic per non-empty bin.
 // Gate weights are evaluated in fp64 for the k picked experts only.
 // Three kernels: route_topk_kernel (any E <= 512, k <= 32, any grouping), route_topk8_kernel (E = 128 | 256, k <= 8,
-// four tokens per warp, (key, index) pairs) and route_topk8p_kernel (the same shapes without group limiting: packed
-// one-register keys, merge networks, staged logits -- the fast path of the 128- / 256-expert softmax configs).
+// four tokens per warp, (key, index) pairs: left with the un-renormalised softmax) and route_topk8p_kernel (the same
+// shapes with no groups or 8 groups, sigmoid or renormalised softmax: packed one-register keys, merge networks, staged
+// logits, approximate sigmoid keys with an exact redo where a margin fails -- the kernel of the C2 / C3 / 64K configs).
 // The counts are zeroed by a one-block kernel that the route kernel overlaps (programmatic dependent launch).
 //
 // Semantics: include/vibe.h (vibe_route_topk), readings R1-R8.
@@ -484,8 +485,8 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
 
 
 // ------------------------------------------------------------------------------------------------------------
-// Packed-key variant of the wide-lane kernel (no group limiting; sigmoid, or softmax with renormalisation: the
-// two cases whose gate weights need the picked logits only).  ncu of route_topk8_kernel at 64K x 256 (profiles/
+// Packed-key variant of the wide-lane kernel (no groups or 8 groups = one lane's experts each; sigmoid, or softmax
+// with renormalisation: the two cases whose gate weights need the picked logits only).  ncu of route_topk8_kernel at 64K x 256 (profiles/
 // r2_route_ncu.md): 390 warp-instructions per token, three quarters of them on the ALU pipe (ISETP/SEL/LOP3/VIMNMX:
 // one warp-instruction per two cycles), most of them the (key, index) pairs dragged through the per-lane sorted
 // insertion and the k selection rounds.  Here a key is ONE register: the order-preserving u32 image of the f32 key
@@ -535,7 +536,7 @@ __device__ __forceinline__ void merge_quad(uint32_t& h0, uint32_t& h1, uint32_t&
 
 // One token by one warp on the EXACT keys (32 lanes x E/32 consecutive experts, k rounds of {lane best, redux max,
 // ballot, lowest lane wins}): the packed-key kernel calls it for the few tokens whose packed order is not provably the
-// exact one.  Writes the token's ids / weights and counts it in the block histogram.  No group limiting; sigmoid, or
+// exact one.  Writes the token's ids / weights and counts it in the block histogram.  No groups or 8 groups of 4 lanes; sigmoid, or
 // softmax with renormalisation (the configurations of the packed-key kernel).
 // merge_quad that also keeps r5, the fifth largest seen so far (the largest key the half-cleaner drops)
 __device__ __forceinline__ void merge_quad5(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t& r5, uint32_t a,
@@ -580,15 +581,16 @@ __device__ __forceinline__ void tree_halfclean(uint32_t& h0, uint32_t& h1, uint3
   h3 = max(h3, q3);
 }
 
-template <int VPL, bool SIGMOID>
+template <int VPL, bool SIGMOID, bool GROUPED>
 __device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids, float* w, int k, int renorm, float scale,
-                                               int t, int* s_hist, const float* s_bias) {
+                                               int topk_group, int t, int* s_hist, const float* s_bias) {
   constexpr int E = 8 * VPL;
   constexpr int V = E / 32;
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
   const float* row = logits + (size_t)t * E;
   uint32_t uk[V];
+  float fk[V];
 #pragma unroll
   for (int q = 0; q < V / 4; ++q) {
     const uint4 u = __ldg(reinterpret_cast<const uint4*>(row + lane * V) + q);
@@ -597,7 +599,38 @@ __device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids
     for (int c = 0; c < 4; ++c) {
       const int e = lane * V + 4 * q + c;
       const float key = SIGMOID ? __fadd_rn(vsig(xv[c]), s_bias[(e / VPL) * (VPL + 1) + e % VPL]) : xv[c];
+      fk[4 * q + c] = key;
       uk[4 * q + c] = ordered_u32(key);
+    }
+  }
+  if (GROUPED) {
+    // 8 groups of VPL consecutive experts = 4 lanes each: score = sum of the group's two largest keys (R6)
+    const float NEG_INF = __int_as_float(0xff800000);
+    float m1 = NEG_INF, m2 = NEG_INF;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const float c = fk[v];
+      if (c > m1) { m2 = m1; m1 = c; } else if (c > m2) { m2 = c; }
+    }
+#pragma unroll
+    for (int o = 1; o < 4; o <<= 1) {
+      const float q1 = __shfl_xor_sync(FULL, m1, o);
+      const float q2 = __shfl_xor_sync(FULL, m2, o);
+      const float lo = fminf(m1, q1);
+      m1 = fmaxf(m1, q1);
+      m2 = fmaxf(lo, fmaxf(m2, q2));
+    }
+    const float score = __fadd_rn(m1, m2);
+    const int g = lane >> 2;
+    int rank = 0;
+#pragma unroll
+    for (int g2 = 0; g2 < 8; ++g2) {
+      const float s2 = __shfl_sync(FULL, score, g2 * 4);
+      rank += (s2 > score || (s2 == score && g2 < g)) ? 1 : 0;
+    }
+    if (rank >= topk_group) {
+#pragma unroll
+      for (int v = 0; v < V; ++v) uk[v] = ordered_u32(NEG_INF);
     }
   }
   int my_id = 0;
@@ -646,6 +679,7 @@ __device__ __noinline__ void route_exact_token(const float* logits, int32_t* ids
 #ifndef ROUTE8P_WARPS_N
 #define ROUTE8P_WARPS_N 28
 #endif
+constexpr int ROUTE8P_REDO_CAP = 126;   // tokens a block may put off to its end (more are redone on the spot)
 constexpr int ROUTE8P_WARPS = ROUTE8P_WARPS_N;      // ONE block of up to 28 warps per SM (72 registers per thread; with 32 warps of 64 registers the merge networks spill)
 template <int VPL>
 __host__ __device__ constexpr size_t route8p_stage_off(bool sigmoid) {
@@ -653,10 +687,11 @@ __host__ __device__ constexpr size_t route8p_stage_off(bool sigmoid) {
 }
 template <int VPL>
 __host__ __device__ constexpr size_t route8p_smem_bytes(bool sigmoid, int warps) {
-  return route8p_stage_off<VPL>(sigmoid) + (size_t)warps * 4 * 8 * VPL * sizeof(float) + warps * sizeof(uint64_t) + 16;
+  return route8p_stage_off<VPL>(sigmoid) + (size_t)warps * 4 * 8 * VPL * sizeof(float) + warps * sizeof(uint64_t) +
+         (2 + ROUTE8P_REDO_CAP) * sizeof(int) + 8;
 }
 
-template <int VPL, bool SIGMOID>
+template <int VPL, bool SIGMOID, bool GROUPED>
 __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(const RouteParams p) {
   const int NW = blockDim.x >> 5;
   extern __shared__ __align__(128) int s_mem[];
@@ -685,7 +720,13 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
   // assignment to four blocks of 8 warps per SM the blocks of one SM ended between 12 and 27 us of a 30 us kernel
   // (64K tokens x 256 experts, in-kernel timestamps).
   int* s_next = reinterpret_cast<int*>(s_stage + (size_t)NW * TILE_BYTES + NW * sizeof(uint64_t));
-  if (threadIdx.x == 0) *s_next = NW;
+  // s_next[1]: number of, s_next[2..]: the tokens whose exact redo was put off to the end of the block (see below)
+  int* s_redo_n = s_next + 1;
+  int* s_redo = s_next + 2;
+  if (threadIdx.x == 0) {
+    *s_next = NW;
+    *s_redo_n = 0;
+  }
   int tile = warp * gridDim.x + blockIdx.x;
 #ifdef ROUTE_TRACE
   unsigned long long tr0, tr1 = 0, tr2;
@@ -723,6 +764,21 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     const uint32_t t = (uint32_t)((int32_t)b >> 31) | 0x80000000u;
     return (b ^ t) | 0xffu;
   };
+  // Sigmoid keys are APPROXIMATE here (2 MUFU + 3 FMA-pipe operations instead of the ~25 separately rounded ones of
+  // vsig): |approx - vsig| < 2^-21 (ex2.approx 2^-22 and rcp.approx 2^-23 relative; vsig itself is within 1.2e-7 of
+  // the sigmoid), the keys (+ bias, rounded) differ by that and one ulp at most.  For keys >= 2^-4 one unit of the
+  // upper 24 bits is >= 2^-19, and two keys whose upper 24 bits are two or more units apart differ by more than one
+  // unit: they are in the same order exactly as approximately.  Wherever the selection leans on a
+  // smaller gap (or on a key below 2^-4) the token is redone on exact keys; the group scores use exact keys of the
+  // two candidates.
+  auto approx_sig = [](float x) {
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * -1.44269504f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+    return r;
+  };
+  constexpr uint32_t GAP_MIN = SIGMOID ? 2u : 1u;
+  constexpr uint32_t PK_FLOOR = 0xbd800000u;     // order-preserving image of 2^-4 (0x3d800000 | sign bit)
   // a lane's VPL consecutive experts are CH 16-byte chunks of the staged row; the lanes of a quarter-warp read them
   // in rotated order (chunk (q + rot) mod CH at step q), which spreads the 8 lanes over all 32 banks
   constexpr int CH = VPL / 4;
@@ -749,7 +805,7 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
       const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        const float key = SIGMOID ? __fadd_rn(vsig(xv[c]), my_bias[4 * ch + c]) : xv[c];
+        const float key = SIGMOID ? __fadd_rn(approx_sig(xv[c]), my_bias[4 * ch + c]) : xv[c];
         pk[4 * q + c] = packed_hi(key) - (uint32_t)(4 * ch) - (uint32_t)c;
       }
     }
@@ -768,6 +824,26 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
 #pragma unroll
     for (int q = 0; q < VPL / 4; ++q)
       merge_quad5(h0, h1, h2, h3, r5, pk[4 * q], pk[4 * q + 1], pk[4 * q + 2], pk[4 * q + 3]);
+    bool unsure = false;                       // this lane's part of "the packed order may not be the exact one"
+    if (GROUPED) {
+      // ---- group-limited routing (R6), one group per lane: score = sum of the lane's two largest EXACT keys.  The
+      //      two are the first two of the packed order if the second is clear of the third (margin below). ----
+      unsure = (h1 >> 8) - (h2 >> 8) < GAP_MIN || (SIGMOID && h1 < PK_FLOOR);
+      const int v0 = 255 - (int)(h0 & 0xffu), v1 = 255 - (int)(h1 & 0xffu);
+      float k0 = __ldg(row + e0 + v0), k1 = __ldg(row + e0 + v1);
+      if (SIGMOID) {
+        k0 = __fadd_rn(vsig(k0), my_bias[v0]);
+        k1 = __fadd_rn(vsig(k1), my_bias[v1]);
+      }
+      const float score = __fadd_rn(k0, k1);
+      int rank = 0;
+#pragma unroll
+      for (int g2 = 0; g2 < 8; ++g2) {
+        const float s2 = __shfl_sync(FULL, score, gbase + g2);
+        rank += (s2 > score || (s2 == score && g2 < sub)) ? 1 : 0;
+      }
+      if (rank >= p.topk_group) { h0 = h1 = h2 = h3 = r5 = e0; }     // (e0 is subtracted below: the group is out)
+    }
     h0 -= e0; h1 -= e0; h2 -= e0; h3 -= e0; r5 -= e0;
     // ---- the group's eight largest heads by a bitonic merge tree over the 8 lanes (three levels) ----
     // Level L merges the sorted 8 of two 2^(L-1)-lane halves: half-cleaner against the reversed partner list (all
@@ -805,34 +881,52 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
       const uint32_t cross = __shfl_xor_sync(FULL, h0, 1);             // an upper lane reads pick 5 here
       uint32_t nxt = slot == 0 ? h1 : slot == 1 ? h2 : slot == 2 ? h3 : (low3 ? 0u : cross);
       if (myj == k - 1) nxt = max(nxt, rest);
-      const bool collide = (myj < k) && (((my_p ^ nxt) < 256u) || nxt > my_p);
-      const unsigned cb = __ballot_sync(FULL, collide);
+      // exact keys (softmax): equal upper 24 bits; approximate keys (sigmoid, error far below one unit of the upper
+      // 24 bits for keys >= 2^-4): less than two units apart, or a last pick below 2^-4
+      const bool ran_out = (myj == k - 1) && nxt > my_p;
+      const bool close = SIGMOID ? (my_p >> 8) - (nxt >> 8) < GAP_MIN : (my_p ^ nxt) < 256u;
+      const bool collide = (myj < k) && (close || nxt > my_p || (SIGMOID && myj == k - 1 && my_p < PK_FLOOR));
+      const unsigned cb = __ballot_sync(FULL, collide || unsure);
       if (cb != 0u) {
-        // equal upper bits: exact ties if the low bytes of all keys of the token are zero, else the token is redone
-        uint32_t lo = 0;                         // OR of the raw bits of the lane's keys (reloaded: L2 hits)
-        {
+        // softmax: equal upper bits are exact ties if the low bytes of all keys of the token are zero, else the token
+        // is redone; a doubtful group score, a lane that ran out of heads or approximate keys: always redone
+        bool hard = unsure || ran_out || (SIGMOID && collide);
+        if (!SIGMOID) {
+          uint32_t lo = 0;                       // OR of the raw bits of the lane's keys (reloaded: L2 hits)
           const uint4* grow4 = reinterpret_cast<const uint4*>(row + e0);
 #pragma unroll
           for (int q = 0; q < CH; ++q) {
             const uint4 u = __ldg(grow4 + q);
-            if (SIGMOID) {
-              const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
-#pragma unroll
-              for (int c = 0; c < 4; ++c) lo |= __float_as_uint(__fadd_rn(vsig(xv[c]), my_bias[4 * q + c]));
+            lo |= u.x | u.y | u.z | u.w;
+          }
+          lo |= __shfl_xor_sync(FULL, lo, 1);
+          lo |= __shfl_xor_sync(FULL, lo, 2);
+          lo |= __shfl_xor_sync(FULL, lo, 4);
+          hard = hard || (collide && (lo & 0xffu) != 0u);
+        }
+        const unsigned hb = __ballot_sync(FULL, hard);
+        redo = ((hb >> gbase) & 0xffu) != 0u && valid;
+        const unsigned rb = __ballot_sync(FULL, redo);
+        // With several tiles per warp a token is redone on the spot (the other warps take the tiles this warp does
+        // not, and a redo in a last tile overlaps the other warps' last tiles).  In a single-wave launch (one tile
+        // per warp: all warps end together) the tokens are left to the block: after the loop every warp takes one,
+        // side by side, instead of one warp holding the block's end back by two or three redos in a row
+        // (C3, 16K tokens: 18.6 -> 14.5 us).
+        // (softmax keys are exact and redone 1 token in 80: putting those off costs more than it saves -- measured)
+        const bool last_tile = SIGMOID && n_tiles <= (int)gridDim.x * NW;
+        for (int g = 0; g < 4; ++g)
+          if ((rb >> (8 * g)) & 1u) {
+            int slot = ROUTE8P_REDO_CAP;
+            if (last_tile) {
+              if (lane == 0) slot = atomicAdd(s_redo_n, 1);
+              slot = __shfl_sync(FULL, slot, 0);
+            }
+            if (slot < ROUTE8P_REDO_CAP) {
+              if (lane == 0) s_redo[slot] = tbase + g;
             } else {
-              lo |= u.x | u.y | u.z | u.w;
+              route_exact_token<VPL, SIGMOID, GROUPED>(p.logits, p.ids, p.w, k, p.renorm, p.scale, p.topk_group, tbase + g, s_hist, s_bias);
             }
           }
-        }
-        lo |= __shfl_xor_sync(FULL, lo, 1);
-        lo |= __shfl_xor_sync(FULL, lo, 2);
-        lo |= __shfl_xor_sync(FULL, lo, 4);
-        const bool ran_out = (myj == k - 1) && nxt > my_p;
-        const unsigned ob = __ballot_sync(FULL, ran_out);
-        redo = ((((cb >> gbase) & 0xffu) != 0u && (lo & 0xffu) != 0u) || ((ob >> gbase) & 0xffu) != 0u) && valid;
-        const unsigned rb = __ballot_sync(FULL, redo);
-        for (int g = 0; g < 4; ++g)
-          if ((rb >> (8 * g)) & 1u) route_exact_token<VPL, SIGMOID>(p.logits, p.ids, p.w, k, p.renorm, p.scale, tbase + g, s_hist, s_bias);
       }
     }
     // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----
@@ -858,6 +952,12 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr2));
 #endif
   __syncthreads();
+  {
+    const int n_redo = min(*s_redo_n, ROUTE8P_REDO_CAP);
+    for (int i = warp; i < n_redo; i += NW)
+      route_exact_token<VPL, SIGMOID, GROUPED>(p.logits, p.ids, p.w, p.k, p.renorm, p.scale, p.topk_group, s_redo[i], s_hist, s_bias);
+    if (n_redo > 0) __syncthreads();
+  }
   ptx::griddep_wait();       // the kernel that zeroes the counts is the predecessor in the stream (see vibe_route_topk)
   for (int i = threadIdx.x; i < p.E; i += blockDim.x) {
     const int c = s_hist[i];
@@ -883,16 +983,18 @@ vibe_status launch_route8(const RouteParams& p, bool sigmoid, bool packed, cudaS
   if (blocks > cap) blocks = cap;
   const size_t smem = (size_t)p.E * sizeof(int) + (sigmoid ? (size_t)8 * (VPL + 1) * sizeof(float) : 0);
   if (packed) {
+    const bool grouped = p.n_group > 1;
     static std::mutex mu;
     static bool done[kMaxDevices] = {};
     {
       std::lock_guard<std::mutex> lk(mu);
       const int dev = current_device();
       if (!done[dev]) {      // the opt-in to > 48 KB of dynamic shared memory is per device
-        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)route8p_smem_bytes<VPL>(true, ROUTE8P_WARPS)));
-        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)route8p_smem_bytes<VPL>(false, ROUTE8P_WARPS)));
+        const int big = (int)route8p_smem_bytes<VPL>(true, ROUTE8P_WARPS);
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
+        VIBE_CUDA(cudaFuncSetAttribute(route_topk8p_kernel<VPL, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
         done[dev] = true;
       }
     }
@@ -903,10 +1005,15 @@ vibe_status launch_route8(const RouteParams& p, bool sigmoid, bool packed, cudaS
     int pblocks = (n_tiles + warps - 1) / warps;
     if (pblocks > num_sms()) pblocks = num_sms();
     const size_t psmem = route8p_smem_bytes<VPL>(sigmoid, warps);
-    if (sigmoid)
-      (void)launch_pdl(route_topk8p_kernel<VPL, true>, dim3(pblocks), dim3(warps * 32), psmem, st, p);
+    const dim3 pg(pblocks), pb(warps * 32);
+    if (sigmoid && grouped)
+      (void)launch_pdl(route_topk8p_kernel<VPL, true, true>, pg, pb, psmem, st, p);
+    else if (sigmoid)
+      (void)launch_pdl(route_topk8p_kernel<VPL, true, false>, pg, pb, psmem, st, p);
+    else if (grouped)
+      (void)launch_pdl(route_topk8p_kernel<VPL, false, true>, pg, pb, psmem, st, p);
     else
-      (void)launch_pdl(route_topk8p_kernel<VPL, false>, dim3(pblocks), dim3(warps * 32), psmem, st, p);
+      (void)launch_pdl(route_topk8p_kernel<VPL, false, false>, pg, pb, psmem, st, p);
     VIBE_LAUNCH_CHECK("route_topk8p_kernel");
     return VIBE_OK;
   }
@@ -987,8 +1094,9 @@ extern "C" vibe_status vibe_route_topk(const vibe_route_cfg* cfg, const float* l
   // for every other configuration -- measured --, so this one combination takes the 32-lane kernel)
   if ((E == 128 || E == 256) && k <= 8 && (ng == 0 || (ng == 8 && (sig || cfg->renormalize)))) {
     p.fast_groups = 1;
-    // packed one-register keys where the gate weights need the picked logits only and there is no group score
-    const bool packed = ng == 0 && (sig || cfg->renormalize);
+    // packed one-register keys where the gate weights need the picked logits only (with or without the 8 groups);
+    // route_topk8_kernel is left with the un-renormalised softmax without groups
+    const bool packed = sig || cfg->renormalize;
     return E == 256 ? launch_route8<32>(p, sig, packed, st) : launch_route8<16>(p, sig, packed, st);
   }
   int lanes, vpl;

@@ -129,6 +129,10 @@ def test_route_adversarial_ties_and_degenerate():
     check_route(big, dict(num_experts=E, top_k=k, score_fn=1, renormalize=1))
 
 
+def make_bias(rng, E, lo, hi):
+    return rng.uniform(lo, hi, size=E).astype(np.float32)
+
+
 @pytest.mark.parametrize("E,k", [(256, 8), (128, 8), (256, 5), (128, 3)])
 def test_route_packed_keys_ties_and_near_ties(E, k):
     """The packed-key kernel of the 128- / 256-expert configs (route.cu, route_topk8p_kernel): its keys keep the upper
@@ -163,6 +167,21 @@ def test_route_packed_keys_ties_and_near_ties(E, k):
     bias = (rng.integers(0, 4, size=E) * 0.25).astype(np.float32)
     check_route(q, kws[1], bias)
     check_route(near, kws[1], bias)
+    # group-limited (8 groups = one lane's experts each; the sigmoid keys of this kernel are approximate and every
+    # decision that leans on a small gap, or on keys below 2^-4, must fall back to the exact ones): continuous logits,
+    # ties, near-ties, keys pushed below the floor and across zero by a negative bias, large biases
+    cont = I.make_logits(T, E, 1.0, 7).astype(np.float32)
+    gk = [dict(num_experts=E, top_k=k, n_group=8, topk_group=4),
+          dict(num_experts=E, top_k=k, score_fn=1, n_group=8, topk_group=4),
+          dict(num_experts=E, top_k=k, score_fn=1, n_group=8, topk_group=3, renormalize=0, routed_scale=2.5)]
+    gk = [g for g in gk if g["topk_group"] * (E // 8) >= k]
+    for kw in gk:
+        for x in (cont, q, near, z, lane, lane2):
+            check_route(np.ascontiguousarray(x), kw)
+    for b in (make_bias(rng, E, -0.95, 0.05), make_bias(rng, E, 0.0, 10.0), make_bias(rng, E, -0.5, 0.5)):
+        for kw in gk[1:] + [kws[1]]:
+            check_route(cont, kw, b)
+            check_route(near, kw, b)
 
 
 def test_route_empty_batch():
