@@ -178,6 +178,14 @@ def test_route_packed_keys_ties_and_near_ties(E, k):
     for kw in gk:
         for x in (cont, q, near, z, lane, lane2):
             check_route(np.ascontiguousarray(x), kw)
+    # gaps of one to a few units of the keys' upper 24 bits between the leading sigmoid keys (the margin rule's edge):
+    # per token 14 experts at 2.0 + a ladder of steps of 1e-4 .. 8e-4 (sigmoid slope 0.105 there), in random positions
+    ladder = (I.make_logits(T, E, 0.0, 8) * 0.3).astype(np.float32)
+    for t in range(T):
+        pos = rng.choice(E, size=14, replace=False)
+        ladder[t, pos] = np.float32(2.0) + np.cumsum(rng.uniform(1e-4, 8e-4, size=14)).astype(np.float32)
+    for kw in gk + kws:
+        check_route(ladder, kw)
     for b in (make_bias(rng, E, -0.95, 0.05), make_bias(rng, E, 0.0, 10.0), make_bias(rng, E, -0.5, 0.5)):
         for kw in gk[1:] + [kws[1]]:
             check_route(cont, kw, b)
