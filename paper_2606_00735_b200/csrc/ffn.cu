@@ -255,9 +255,12 @@ __device__ __forceinline__ void store_block_T_e4m3(const float (&v)[32], uint8_t
 // (profiles/: 1.5 x the algorithmic bytes).  Dynamic hand-out also balances the ragged tile costs.
 // The leader CTA's producer warp fetches (one atomicAdd per unit, on demand: its latency hides behind the 6 stages
 // the producer runs ahead) and publishes the id to a 4-slot ring in both CTAs; every other role of the pair reads it.
+// A pair's FIRST unit is its own index in both schemes (no counter round trip in front of the first TMA: ~1 us of
+// every launch, which is a tenth of a lone light expert's kernel); the counter hands out units num_pairs, ...
 struct UnitCursor {
   int rnd = 0, idx = 0;
   uint32_t ph = 0;
+  bool first = true;
 };
 __device__ __forceinline__ int next_unit_fetch(SmemTail* tail, unsigned int* ctr, int total, int pair, int num_pairs,
                                                UnitCursor& c, int lane) {
@@ -266,11 +269,15 @@ __device__ __forceinline__ int next_unit_fetch(SmemTail* tail, unsigned int* ctr
     ++c.rnd;
     return u < total ? u : -1;
   }
+  if (c.first) {
+    c.first = false;
+    return pair < total ? pair : -1;
+  }
   const int slot = c.idx;
   ptx::mbar_wait(ptx::smem_u32(&tail->rempty[slot]), c.ph ^ 1u);
   int u = 0;
   if (lane == 0) {
-    u = (int)atomicAdd(ctr, 1u);
+    u = (int)atomicAdd(ctr, 1u) + num_pairs;
     if (u >= total) u = -1;
     const uint32_t ra = ptx::smem_u32(&tail->ring[slot]), fa = ptx::smem_u32(&tail->rfull[slot]);
     ptx::st_shared_cluster_u32(ptx::mapa_u32(ra, 0), (uint32_t)u);
@@ -288,6 +295,10 @@ __device__ __forceinline__ int next_unit_read(SmemTail* tail, bool dynamic, int 
     const int u = tile_of(c.rnd, pair, num_pairs);
     ++c.rnd;
     return u < total ? u : -1;
+  }
+  if (c.first) {
+    c.first = false;
+    return pair < total ? pair : -1;
   }
   const int slot = c.idx;
   ptx::mbar_wait_acq_cluster(ptx::smem_u32(&tail->rfull[slot]), c.ph);

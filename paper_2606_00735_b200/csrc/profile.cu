@@ -56,7 +56,10 @@ namespace {
 template <class Run>
 vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_points, int mode, int warmup, int iters,
                           float* latency_us, float* samples_us, int32_t* offsets, void* flush, cudaStream_t caller, Run run,
-                          int seg_align = 1) {
+                          int seg_align = 1, void* ffn_ws = nullptr) {
+  // ffn_ws: the FFN's split-K / scheduler counters are zeroed AHEAD of every execution, outside the timed region (as
+  // the layer entries do before the route kernel); the timed graph holds the two FFN kernels only
+  auto pre = [&](cudaStream_t ps) { return ffn_ws ? grouped_ffn_zero_counters(ffn_ws, ps) : VIBE_OK; };
   VIBE_CUDA(cudaStreamSynchronize(caller));
   cudaStream_t st = nullptr;
   VIBE_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
@@ -79,7 +82,11 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
       rc = VIBE_ERR_CUDA;
       break;
     }
-    for (int i = 0; i < std::max(warmup, 1) && rc == VIBE_OK; ++i) rc = run(st);
+    for (int i = 0; i < std::max(warmup, 1) && rc == VIBE_OK; ++i) {
+      rc = pre(st);
+      if (rc == VIBE_OK) rc = run(st);
+    }
+    if (rc == VIBE_OK) rc = pre(st);
     if (rc != VIBE_OK) break;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -93,6 +100,8 @@ vibe_status profile_sweep(int E_loc, const int32_t* tokens_per_expert, int n_poi
     }
     (void)cudaGetLastError();      // a failed capture leaves a sticky-free error behind; the fallback below still works
     for (int i = 0; i < iters && rc == VIBE_OK; ++i) {
+      rc = pre(st);
+      if (rc != VIBE_OK) break;
       l2_flush_kernel<<<num_sms() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(flush), kProfileFlushBytes / 16,
                                                      reinterpret_cast<uint32_t*>(flush));
       count_launch();
@@ -175,8 +184,9 @@ extern "C" vibe_status vibe_profile_expert_latency(int32_t E_loc, int32_t d, int
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st,
                        [&](cudaStream_t ps) {
                          return grouped_ffn_impl(Xp, offsets, E_loc, R_cap, d, f, W1, W3, W2, H, Y, ps, nullptr, nullptr, ffn_ws,
-                                                 grouped_ffn_ws_bytes(), false);
-                       });
+                                                 grouped_ffn_ws_bytes(), true);
+                       },
+                       1, ffn_ws);
 }
 
 extern "C" vibe_status vibe_profile_expert_latency_fp8(int32_t E_loc, int32_t d, int32_t f, const void* W1q,
@@ -279,9 +289,9 @@ extern "C" vibe_status vibe_profile_expert_latency_mxfp8(int32_t E_loc, int32_t 
   return profile_sweep(E_loc, tokens_per_expert, n_points, mode, warmup, iters, latency_us, samples_us, offsets, flush, st,
                        [&](cudaStream_t ps) {
                          return grouped_ffn_mxfp8_impl(Xq, xsf, offsets, E_loc, R_cap, d, f, W1q, W3q, sf13, W2q, sf2, Hq, hsf, Y, ps,
-                                                       ffn_ws, grouped_ffn_ws_bytes(), false);
+                                                       ffn_ws, grouped_ffn_ws_bytes(), true);
                        },
-                       kMxRowAlign);
+                       kMxRowAlign, ffn_ws);
 }
 
 // Measurement utility: evict the L2 (evict_last read sweep, see l2_flush_kernel) before a timed region.
