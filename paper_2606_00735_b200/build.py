@@ -38,7 +38,7 @@ def _digest() -> str:
     h = hashlib.sha256()
     files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + [os.path.join(INCLUDE, "vibe.h")]
     for f in files:
-        h.update(f.encode())
+        h.update(os.path.basename(f).encode())      # (not the absolute path: the stamp must survive a move of the tree)
         h.update(open(f, "rb").read())
     h.update(" ".join(NVCC_FLAGS).encode())
     return h.hexdigest()
