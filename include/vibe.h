@@ -120,6 +120,23 @@ VIBE_API vibe_status vibe_permute(const void* X, const int32_t* topk_ids, const 
                                   int32_t* row_to_assign, int32_t* assign_to_row, void* ws, size_t ws_bytes,
                                   void* stream);
 
+/* a3 without a workspace argument, for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the same operation, arguments, layouts and results as
+ * vibe_permute (readings P1-P4; /root/reference PAPER.md L28, L86: tokens are sent to their experts), with
+ * the scratch of the index kernel in a static device array of VIBE_PERMUTE_STATIC_BYTES inside the library (every GPU
+ * that loads the library holds it until the process exits).  The call allocates nothing (no cudaMalloc / cudaFree /
+ * allocating library routine).
+ * Limit: vibe_workspace_bytes(VIBE_WS_PERMUTE, ...) = roundup(4 * SMs * E_loc, 256) + 256 bytes must fit the array:
+ *   E_loc <= 512 on a 148-SM B200; beyond that VIBE_ERR_WORKSPACE (nothing is launched; use vibe_permute).
+ * ALL calls of a process on one GPU share the array: calls that may overlap on the GPU (different streams, graphs
+ * replayed side by side) race on it and must use vibe_permute with their own workspaces instead.  The array keeps
+ * the last call's contents; every call clears what it needs cleared.  Other errors: as vibe_permute. */
+#define VIBE_PERMUTE_STATIC_BYTES (304 * 1024)
+VIBE_API vibe_status vibe_permute_static(const void* X, const int32_t* topk_ids, const int32_t* counts,
+                                         const int32_t* expert_map, int32_t T, int32_t d, int32_t k, int32_t E,
+                                         int32_t E_loc, int32_t align, void* Xp, int32_t* offsets,
+                                         int32_t* row_to_assign, int32_t* assign_to_row, void* stream);
+
 /* ------------------------------------------------------------------------------------
  * a4.  Grouped SwiGLU expert FFN over the resident experts -- the kernel whose
  * latency-vs-token-load ViBE profiles and the dominant cost of MoE serving

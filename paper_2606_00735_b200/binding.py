@@ -34,8 +34,8 @@ MODEL_A, MODEL_B = 0, 1
 
 # every symbol include/vibe.h declares (tests check that the .so exports exactly these)
 EXPORTED_SYMBOLS = (
-    "vibe_route_topk", "vibe_permute", "vibe_grouped_ffn", "vibe_combine", "vibe_profile_expert_latency",
-    "vibe_moe_layer_forward", "vibe_moe_layer_forward_host", "vibe_workspace_bytes", "vibe_rows_cap",
+    "vibe_route_topk", "vibe_permute", "vibe_permute_static", "vibe_grouped_ffn", "vibe_combine",
+    "vibe_profile_expert_latency", "vibe_moe_layer_forward", "vibe_moe_layer_forward_host", "vibe_workspace_bytes", "vibe_rows_cap",
     "vibe_status_string", "vibe_last_error", "vibe_version", "vibe_launch_count",
     "vibe_placement_eval", "vibe_placement_greedy", "vibe_placement_token_balanced", "vibe_placement_contiguous",
     "vibe_grouped_ffn_scatter", "vibe_combine_scattered",
@@ -105,6 +105,8 @@ def load() -> C.CDLL:
     vp, i32, sz = C.c_void_p, C.c_int32, C.c_size_t
     lib.vibe_route_topk.argtypes = [C.POINTER(_RouteCfg), vp, i32, vp, vp, vp, vp]
     lib.vibe_permute.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    lib.vibe_permute_static.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.vibe_permute_static.restype = C.c_int
     lib.vibe_grouped_ffn.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.vibe_combine.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp]
     lib.vibe_grouped_ffn_scatter.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -274,6 +276,26 @@ def permute(X: torch.Tensor, topk_ids: torch.Tensor, counts: Optional[torch.Tens
                          expert_map.data_ptr() if expert_map is not None else None, T, d, k, E, E_loc, align,
                          Xp.data_ptr(), offsets.data_ptr(), r2a.data_ptr(), a2r.data_ptr(), ws.data_ptr(),
                          ws.numel(), _stream(stream)), "vibe_permute")
+    return Xp, offsets, r2a, a2r
+
+
+PERMUTE_STATIC_BYTES = 304 * 1024
+
+
+def permute_static(X: torch.Tensor, topk_ids: torch.Tensor, counts: Optional[torch.Tensor],
+                   expert_map: Optional[torch.Tensor], E: int, E_loc: int, align: int, out, stream=None):
+    """vibe_permute_static: permute() with the scratch in the library's static device array -- the call allocates
+    nothing, so every output is the caller's (`out` = (Xp, offsets, row_to_assign, assign_to_row), required)."""
+    lib = load()
+    _check(X, torch.bfloat16, "X")
+    _check(topk_ids, torch.int32, "topk_ids")
+    T, d = X.shape
+    k = topk_ids.shape[1]
+    Xp, offsets, r2a, a2r = out
+    _ok(lib.vibe_permute_static(X.data_ptr(), topk_ids.data_ptr(), counts.data_ptr() if counts is not None else None,
+                                expert_map.data_ptr() if expert_map is not None else None, T, d, k, E, E_loc, align,
+                                Xp.data_ptr(), offsets.data_ptr(), r2a.data_ptr(), a2r.data_ptr(), _stream(stream)),
+        "vibe_permute_static")
     return Xp, offsets, r2a, a2r
 
 

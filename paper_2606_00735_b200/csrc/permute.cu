@@ -27,6 +27,7 @@
 //                    so DRAM traffic equals the algorithmic 2*T_res*d + 2*R*d bytes.
 //                    (E_loc < E: the row-major variant perm_rows_by_row, work ~ R.)
 #include <atomic>
+#include <mutex>
 
 #include "common.cuh"
 #include "ptx.cuh"
@@ -437,4 +438,58 @@ extern "C" vibe_status vibe_permute(const void* X, const int32_t* topk_ids, cons
   }
   VIBE_LAUNCH_CHECK("perm_rows_kernel");
   return VIBE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// vibe_permute_static: vibe_permute for callers that cannot allocate device memory (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  The index kernel's scratch -- the [CTAs][E_loc] table of
+// slot totals and the grid-barrier counters -- lives in a file-scope device array of VIBE_PERMUTE_STATIC_BYTES
+// (304 KiB: E_loc <= 512 on the 148 SMs of a B200); every GPU that loads the library holds it until exit.
+// In HOST code the array's name is a host-side stand-in, not a device address: the device address is taken once per
+// device, with that device current, by cudaGetSymbolAddress, and that pointer is what the kernels get.
+// All calls share the array: calls that overlap on the GPU (two streams, graphs replayed side by side) race on it.
+// It keeps the last call's contents; what must start at zero -- the barrier counters of the cooperative path -- is
+// cleared by every call (vibe_permute does that for any workspace), the table is written before it is read.
+// No cudaMalloc / cudaFree / allocating library routine is called.
+// ------------------------------------------------------------------------------------------------------------
+namespace vibe {
+namespace {
+static __device__ __align__(256) unsigned char g_permute_static_scratch[VIBE_PERMUTE_STATIC_BYTES];
+
+vibe_status permute_static_scratch(void** out) {
+  static std::mutex mu;
+  static void* ptr[kMaxDevices] = {};
+  const int dev = current_device();
+  std::lock_guard<std::mutex> lk(mu);
+  if (ptr[dev] == nullptr) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_permute_static_scratch);
+    VIBE_REQUIRE(e == cudaSuccess && p != nullptr, VIBE_ERR_CUDA,
+                 "vibe_permute_static: cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+    ptr[dev] = p;
+  }
+  *out = ptr[dev];
+  return VIBE_OK;
+}
+}  // namespace
+}  // namespace vibe
+
+extern "C" vibe_status vibe_permute_static(const void* X, const int32_t* topk_ids, const int32_t* counts,
+                                           const int32_t* expert_map, int32_t T, int32_t d, int32_t k, int32_t E,
+                                           int32_t E_loc, int32_t align, void* Xp, int32_t* offsets,
+                                           int32_t* row_to_assign, int32_t* assign_to_row, void* stream) {
+  using namespace vibe;
+  clear_error();
+  VIBE_REQUIRE(T >= 0 && k >= 1 && E >= 1 && E_loc >= 1, VIBE_ERR_INVALID_ARG,
+               "vibe_permute_static: bad sizes T=%d k=%d E=%d E_loc=%d", T, k, E, E_loc);
+  const size_t need = permute_ws_bytes(T, k, E_loc);
+  VIBE_REQUIRE(need <= (size_t)VIBE_PERMUTE_STATIC_BYTES, VIBE_ERR_WORKSPACE,
+               "vibe_permute_static: E_loc=%d on %d SMs needs %zu bytes of scratch, the static array holds %d "
+               "(use vibe_permute with a caller-provided workspace)",
+               E_loc, num_sms(), need, (int)VIBE_PERMUTE_STATIC_BYTES);
+  void* scratch = nullptr;
+  const vibe_status s = permute_static_scratch(&scratch);
+  if (s != VIBE_OK) return s;
+  return vibe_permute(X, topk_ids, counts, expert_map, T, d, k, E, E_loc, align, Xp, offsets, row_to_assign,
+                      assign_to_row, scratch, (size_t)VIBE_PERMUTE_STATIC_BYTES, stream);
 }
