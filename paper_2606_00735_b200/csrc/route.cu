@@ -516,29 +516,13 @@ __global__ void __launch_bounds__(256, ROUTE8_MIN_BLOCKS) route_topk8_kernel(con
     b = lo_;                                 \
   }
 
-// (h0..h3) sorted descending <- the four largest of (h0..h3) sorted and (a, b, c, d) in any order
-__device__ __forceinline__ void merge_quad(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t a, uint32_t b,
-                                           uint32_t c, uint32_t d) {
-  VIBE_CSWAP(a, b);
-  VIBE_CSWAP(c, d);
-  VIBE_CSWAP(a, c);
-  VIBE_CSWAP(b, d);
-  VIBE_CSWAP(b, c);          // a >= b >= c >= d
-  h0 = max(h0, d);           // half-cleaner of the bitonic sequence h0 h1 h2 h3 d c b a: the four largest, bitonic
-  h1 = max(h1, c);
-  h2 = max(h2, b);
-  h3 = max(h3, a);
-  VIBE_CSWAP(h0, h2);
-  VIBE_CSWAP(h1, h3);
-  VIBE_CSWAP(h0, h1);
-  VIBE_CSWAP(h2, h3);
-}
-
 // One token by one warp on the EXACT keys (32 lanes x E/32 consecutive experts, k rounds of {lane best, redux max,
 // ballot, lowest lane wins}): the packed-key kernel calls it for the few tokens whose packed order is not provably the
 // exact one.  Writes the token's ids / weights and counts it in the block histogram.  No groups or 8 groups of 4 lanes; sigmoid, or
 // softmax with renormalisation (the configurations of the packed-key kernel).
-// merge_quad that also keeps r5, the fifth largest seen so far (the largest key the half-cleaner drops)
+// (h0..h3) sorted descending <- the four largest of (h0..h3) sorted and (a, b, c, d) in any order (sort the four, half-
+// cleaner of the bitonic sequence h0 h1 h2 h3 d c b a, bitonic sort of the four kept); r5 <- the largest key seen so
+// far that is not among them (the lane's fifth)
 __device__ __forceinline__ void merge_quad5(uint32_t& h0, uint32_t& h1, uint32_t& h2, uint32_t& h3, uint32_t& r5, uint32_t a,
                                             uint32_t b, uint32_t c, uint32_t d) {
   VIBE_CSWAP(a, b);

@@ -692,7 +692,7 @@ def write_markdown(r, path, command):
             o.append(f"| {s['config']} | {s['T']} | {s['E']} ({s['E_loc']}) | {s['k']} | {s['d']} | {s['real_rows']} | "
                      f"{s['route']['us']} | {s['route']['GB/s']} | {s['route']['frac_hbm']} | {s['route'].get('logit_read_stream_us', '')} | "
                      + " | ".join(f"{s[n]['us']} | {s[n]['GB/s']} | {s[n]['frac_hbm']}" for n in ('permute', 'combine')) + " |")
-        o.append("\nRoute: bound by the ALU pipe (packed-key kernel) or by the reproducible sigmoid (C3), not by HBM (`r2_route_ncu.md`); the column beside it is the floor of the OP on this box: a selection-free kernel that only streams the same logits once.  permute = 2 launches (cooperative index kernel + row kernel), combine = 1.\n")
+        o.append("\nRoute: bound by the ALU pipe at 64K tokens and by launch + latency at the C1-C3 batch sizes, not by HBM (`r2_route_ncu.md`); the column beside it is the floor of the OP on this box: a selection-free kernel that only streams the same logits once.  permute = 2 launches (cooperative index kernel + row kernel), combine = 1.\n")
     if "ffn_balanced" in r:
         o.append("## ffn_balanced: grouped FFN, every expert n rows (vibe_profile_expert_latency mode 0, largest n first, 2 s warm loop)\n")
         o.append("| shape | E_loc | d | f | tokens/expert | us/expert | TFLOP/s | of sustained | of burst | of per-expert roofline max(flops/sustained, bytes/HBM) |")
