@@ -52,6 +52,10 @@ def test_argument_errors_are_detected_before_any_launch(lib):
     assert lib.vibe_permute(16, 16, None, None, 4, 12, 2, 8, 8, 1, 16, 16, 16, 16, 16, 1 << 20, None) == 1
     assert lib.vibe_permute(16, 16, None, None, 4, 16, 2, 8, 4, 1, 16, 16, 16, 16, 16, 1 << 20, None) == 1
     assert lib.vibe_permute(16, 16, None, None, 4, 16, 2, 8, 8, 1, 16, 16, 16, 16, 16, 8, None) == 3
+    # permute without a workspace argument: bad sizes; more slots than the static scratch array holds (no launch either way)
+    assert lib.vibe_permute_static(16, 16, None, None, -1, 16, 2, 8, 8, 1, 16, 16, 16, 16, None) == 1
+    assert lib.vibe_permute_static(16, 16, None, None, 4, 16, 2, 2048, 1024, 1, 16, 16, 16, 16, None) == 3
+    assert b"static array" in lib.vibe_last_error()
     # ffn: shape limits, misalignment
     assert lib.vibe_grouped_ffn(16, 16, 8, 64, 100, 128, 16, 16, 16, 16, 16, None, 0, None) == 2
     assert lib.vibe_grouped_ffn(8, 16, 8, 64, 128, 128, 16, 16, 16, 16, 16, None, 0, None) == 1
