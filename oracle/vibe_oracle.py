@@ -105,6 +105,15 @@ def vsig_f32(x):
     return one / (one + e)
 
 
+def _argmax_untaken(v, taken):
+    """Per row: the lowest index among the largest entries of v that are not `taken` (R3).  The k picks (and the
+    topk_group kept groups) are k DISTINCT experts (groups) also when fewer than k entries are finite -- keys of
+    -inf, e.g. masked logits or a group limit that leaves fewer than k finite keys: marking a pick by overwriting
+    its key with -inf would then pick it again."""
+    m = np.where(taken, -np.inf, v).max(axis=1, keepdims=True)
+    return np.argmax((v == m) & ~taken, axis=1)              # first True = lowest index
+
+
 def route_topk(logits, num_experts, top_k, score_fn=SCORE_SOFTMAX, renormalize=1,
                routed_scale=1.0, n_group=0, topk_group=0, select_bias=None):
     """O1 steps 1-6.  logits f32 [T,E] -> (topk_ids i32 [T,k], topk_w f32 [T,k], counts i32 [E]).
@@ -146,20 +155,18 @@ def route_topk(logits, num_experts, top_k, score_fn=SCORE_SOFTMAX, renormalize=1
             gscore = srt[:, :, -1]
         assert gscore.dtype == _F
         keep = np.zeros((T, n_group), dtype=bool)
-        g = gscore.copy()
         for _ in range(topk_group):
-            best = np.argmax(g, axis=1)                      # first occurrence = lowest group index
+            best = _argmax_untaken(gscore, keep)             # lowest group index among the best not yet kept
             keep[np.arange(T), best] = True
-            g[np.arange(T), best] = -np.inf
         key = np.where(np.repeat(keep, gs, axis=1), key, _F(-np.inf)).astype(_F)
     # step 4
     ids = np.empty((T, k), dtype=np.int32)
-    kk = key.copy()
+    taken = np.zeros((T, E), dtype=bool)
     rows = np.arange(T)
     for j in range(k):
-        best = np.argmax(kk, axis=1)                         # first occurrence = lowest index
+        best = _argmax_untaken(key, taken)                   # lowest index among the largest keys not yet picked
         ids[:, j] = best
-        kk[rows, best] = -np.inf
+        taken[rows, best] = True
     # step 5
     xd = x.astype(np.float64)
     if score_fn == SCORE_SOFTMAX:

@@ -111,6 +111,38 @@ def test_group_limited_brute_force_sigmoid():
         assert all(e // gs in kept for e in ids[t])
 
 
+def test_fewer_than_k_finite_keys_still_gives_k_distinct_experts():
+    """R3 with keys of -inf (masked logits; a group limit that leaves fewer than k finite keys): the picks are the
+    first k of the order (key descending, index ascending) -- k DISTINCT experts -- and the kept groups are the first
+    topk_group of (score descending, group ascending).  Pinned against a pure-Python sort, with hand-worked rows."""
+    E, k = 16, 5
+    z = np.full((3, E), -np.inf, np.float32)
+    z[0, [9, 3]] = [1.0, 2.0]                     # two finite keys: 3, 9, then the lowest unpicked indices 0, 1, 2
+    z[1, :] = -np.inf                             # none finite: 0, 1, 2, 3, 4
+    z[2, [0, 1, 2, 15]] = [0.5, 0.5, -1.0, 7.0]   # 15, 0, 1, 2, then 3
+    with np.errstate(invalid="ignore"):          # the all -inf row has no defined weights (NaN): ids only
+        ids, _, counts = O.route_topk(z, E, k, renormalize=0)
+    assert ids.tolist() == [[3, 9, 0, 1, 2], [0, 1, 2, 3, 4], [15, 0, 1, 2, 3]]
+    assert counts.sum() == 3 * k and all(len(set(r)) == k for r in ids.tolist())
+    rng = np.random.default_rng(5)
+    zz = rng.standard_normal((200, 32)).astype(np.float32)
+    zz[rng.random(zz.shape) < 0.85] = -np.inf
+    assert np.array_equal(O.route_topk(zz, 32, 8, renormalize=0)[0], brute_topk(zz, 8))
+    # groups: 4 groups of 8; scores of -inf tie and go to the lower group index; all groups kept when topk_group = 4
+    ng, tg, gs = 4, 2, 8
+    for tg in (1, 2, 4):
+        ids, _, _ = O.route_topk(zz, 32, 8, renormalize=0, n_group=ng, topk_group=tg)
+        for t in range(zz.shape[0]):
+            scores = []
+            for g in range(ng):
+                vals = sorted((float(v) for v in zz[t, g * gs:(g + 1) * gs]), reverse=True)
+                scores.append(float(np.float32(vals[0]) + np.float32(vals[1])))
+            kept = sorted(range(ng), key=lambda g: (-scores[g], g))[:tg]
+            keyt = [float(zz[t, e]) if e // gs in kept else -np.inf for e in range(32)]
+            order = sorted(range(32), key=lambda e: (-keyt[e], e))[:8]
+            assert ids[t].tolist() == order, (tg, t)
+
+
 # ---------------------------------------------------------------- vsig (selection key)
 def test_vsig_accuracy_monotone_and_closed_forms():
     xs = np.concatenate([np.linspace(-30, 30, 200001), I._rng(0, 1).standard_normal(100000) * 3]).astype(np.float32)
