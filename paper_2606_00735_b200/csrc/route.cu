@@ -254,11 +254,14 @@ __global__ void __launch_bounds__(256) route_topk_kernel(const RouteParams p) {
         dry = (m1 == kTaken);
       }
     }
-    // the picked expert's logit: for softmax the key IS the logit (-0 arrives as +0, same exp);
-    // for sigmoid it is read back from the row (an L1/L2 hit, one load per pick)
+    // the picked expert's logit: for softmax without groups the key IS the logit (-0 arrives as +0, same exp);
+    // otherwise it is read back from the row (an L1/L2 hit, one load per pick): the sigmoid's key is not the logit,
+    // and under a group limit a pick can come from a masked group (key -inf) when the kept groups hold fewer than k
+    // experts that are not masked themselves (logits of -inf) -- its weight is that of its LOGIT (R1: weights from
+    // the scores, the mask is selection-only)
     float my_x = 0.0f;
     if (sub < k) {
-      if (SIGMOID) my_x = __ldg(row + my_id);
+      if (SIGMOID || p.n_group > 1) my_x = __ldg(row + my_id);
       else my_x = __uint_as_float((my_key & 0x80000000u) ? (my_key & 0x7fffffffu) : ~my_key);
     }
     // ---- gate weights in fp64 for the picked experts (R1, R4, R5) ----

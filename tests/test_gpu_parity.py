@@ -192,6 +192,34 @@ def test_route_packed_keys_ties_and_near_ties(E, k):
             check_route(near, kw, b)
 
 
+@pytest.mark.parametrize("E,k,ng,tg", [(256, 8, 0, 0), (256, 8, 8, 1), (128, 5, 8, 2), (64, 6, 4, 1), (384, 7, 8, 1),
+                                       (33, 5, 3, 1), (16, 3, 2, 1)])
+def test_route_masked_logits_fewer_finite_keys_than_k(E, k, ng, tg):
+    """Logits of -inf (masked experts), so many that a token -- or the groups it keeps -- has fewer than k finite keys:
+    the picks are still k distinct experts in (key descending, index ascending) order (R3), and a pick that comes from
+    a masked GROUP carries the weight of its logit (R1: the group mask is selection-only).  Every route kernel."""
+    rng = np.random.default_rng(E + k)
+    T = 517
+    for frac in (0.5, 0.9, 0.98):
+        x = (rng.standard_normal((T, E)) * 3).astype(np.float32)
+        x[rng.random((T, E)) < frac] = -np.inf
+        x[:, rng.integers(0, E)] = rng.standard_normal(T).astype(np.float32)       # one finite logit per token at least
+        for sf, renorm in ((0, 1), (0, 0), (1, 1), (1, 0)):
+            kw = dict(num_experts=E, top_k=k, score_fn=sf, renormalize=renorm, n_group=ng, topk_group=tg)
+            with np.errstate(invalid="ignore"):          # all picks masked + renormalisation: 0 / 0 on both sides
+                ids_o, w_o, c_o = O.route_topk(x, **kw)
+            ids, w, counts = B.route_topk(dev(x), B.RouteConfig(**kw))
+            torch.cuda.synchronize()
+            assert np.array_equal(ids.cpu().numpy(), ids_o), (frac, sf, renorm)
+            assert np.array_equal(counts.cpu().numpy(), c_o)
+            assert all(len(set(r)) == k for r in ids_o.tolist())
+            wg = w.cpu().numpy().astype(np.float64)
+            ok = w_o > 1e-30                                   # weights of masked picks are exactly 0 on both sides
+            assert np.array_equal(wg[~ok] == 0, w_o[~ok] == 0) or np.all(np.abs(wg[~ok]) <= 1e-30)
+            rel = np.abs(wg[ok] - w_o[ok]) / w_o[ok]
+            assert rel.size == 0 or rel.max() <= W_RTOL, (frac, sf, renorm, rel.max())
+
+
 def test_route_empty_batch():
     rc = B.RouteConfig(num_experts=16, top_k=2)
     logits = torch.empty((0, 16), dtype=torch.float32, device="cuda")
