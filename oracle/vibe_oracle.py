@@ -710,9 +710,12 @@ def fp8_quantize_static(v, scale):
     return e4m3_encode((np.asarray(v).astype(np.float32) / np.float32(scale)).astype(np.float64))
 
 
-def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q, s2, h_scale):
+def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q, s2, h_scale, Hq_given=None):
     """Per resident expert e and real row r:  g = sx[r] s1[e] (xq . w1q),  u = sx[r] s3[e] (xq . w3q),
-    h = silu(g) u,  hq = e4m3(h / sh[e]),  y = sh[e] s2[e] (hq . w2q).  Returns (Y f64 [R,d], Hq codes [R,f])."""
+    h = silu(g) u,  hq = e4m3(h / sh[e]),  y = sh[e] s2[e] (hq . w2q).  Returns (Y f64 [R,d], Hq codes [R,f]).
+    Hq_given (codes [R,f]): the down projection runs on THESE codes instead of the ones computed here (the returned
+    Hq is still the computed one) -- lets a parity test separate the two GEMMs: a code that the device decided one
+    e4m3 step away (its h is an fp32 sum in an order no oracle can know) moves y by up to 2^-3 |h| |w2|."""
     T8 = e4m3_decode_table()
     R = int(offsets[-1])
     f, d = W1q.shape[1], W1q.shape[2]
@@ -732,6 +735,8 @@ def grouped_ffn_fp8(Xq, row_scale, offsets, row_to_assign, W1q, s1, W3q, s3, W2q
         # in binary32 and rounded ONCE to e4m3
         hq = fp8_quantize_static(h, h_scale[e])
         Hq[rows] = hq
+        if Hq_given is not None:
+            hq = np.asarray(Hq_given)[rows]
         Y[rows] = (T8[hq] @ T8[W2q[e]].T) * np.float64(h_scale[e]) * np.float64(s2[e])
     return Y, Hq
 
@@ -799,10 +804,13 @@ def mx_quantize_rows(X_bits, block=32):
     return mx_quantize(bf16_bits_to_f64(X_bits), block)
 
 
-def grouped_ffn_mxfp8(Xq, Xsf, offsets, row_to_assign, W1q, W1sf, W3q, W3sf, W2q, W2sf):
+def grouped_ffn_mxfp8(Xq, Xsf, offsets, row_to_assign, W1q, W1sf, W3q, W3sf, W2q, W2sf, H_given=None):
     """Per resident expert e and real row r (Q8):  g = x . w1,  u = x . w3  on the dequantised values,
     h = silu(g) u,  (hq, hsf) = block-32 quantisation of binary32(h) along f (Q7),  y = deq(hq) . w2.
-    Returns (Y f64 [R,d], Hq codes [R,f], Hsf [R,f/32])."""
+    Returns (Y f64 [R,d], Hq codes [R,f], Hsf [R,f/32]).
+    H_given = (codes [R,f], scale bytes [R,f/32]): the down projection runs on THESE instead of the ones computed
+    here (the returned Hq / Hsf are still the computed ones) -- separates the two GEMMs in a parity test, as in
+    grouped_ffn_fp8."""
     R = int(offsets[-1])
     f, d = W1q.shape[1], W1q.shape[2]
     Y = np.zeros((R, d), dtype=np.float64)
@@ -819,6 +827,8 @@ def grouped_ffn_mxfp8(Xq, Xsf, offsets, row_to_assign, W1q, W1sf, W3q, W3sf, W2q
         h = g / (1.0 + np.exp(-g)) * u
         hq, hsf = mx_quantize(h.astype(np.float32).astype(np.float64), 32)
         Hq[rows], Hsf[rows] = hq, hsf
+        if H_given is not None:
+            hq, hsf = np.asarray(H_given[0])[rows], np.asarray(H_given[1])[rows]
         Y[rows] = mx_dequantize(hq, hsf) @ mx_dequantize(W2q[e], W2sf[e]).T
     return Y, Hq, Hsf
 

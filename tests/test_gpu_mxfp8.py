@@ -122,6 +122,11 @@ def run_ffn_case(off, r2a, Xp, W1, W3, W2, extra_rows=64):
     hs = read_sf(Hsf, B.MX_SF_TOKENS, R, f, R_cap=Rcap)[0]
     H_gpu = O.mx_dequantize(Hq.cpu().numpy()[:R][real], hs[real])
     H_ref = O.mx_dequantize(Hq_o[real], Hs_o[real])
+    # GEMM-2 in isolation: the device's Y against the oracle's down projection of the DEVICE's own H codes and scales
+    # (no code decision in between: fp32 accumulation order + the bf16 storage of Y, element by element)
+    Y_own = O.grouped_ffn_mxfp8(Xq, Xs, off, r2a, W1q, W1s, W3q, W3s, W2q, W2s, H_given=(Hq.cpu().numpy()[:R], hs))[0][real]
+    got = O.bf16_bits_to_f64(host_bits(Y)[:R][real])
+    assert np.all(np.abs(got - Y_own) <= 2.0 ** -8 * np.abs(Y_own) + 1e-3 * float(np.sqrt(np.mean(Y_own ** 2))))
     return Y_o, Y, H_ref, H_gpu, hs[real], Hs_o[real], real, R
 
 

@@ -619,6 +619,15 @@ def test_fp8_quantisers_bit_exact():
     assert np.array_equal(wq.cpu().numpy(), wq_o), "weight codes / [E,N,K] layout"
 
 
+def check_down_projection_on_own_codes(Y_gpu_bits, Y_on_gpu_codes):
+    """GEMM-2 in isolation: the device's Y against the oracle's down projection of the DEVICE's own H codes.  No code
+    decision lies between the two, so what is left is fp32 accumulation order and the bf16 storage of Y: element by
+    element 2^-8 |ref| + 1e-3 RMS."""
+    got = O.bf16_bits_to_f64(Y_gpu_bits)
+    rms = float(np.sqrt(np.mean(Y_on_gpu_codes ** 2)))
+    assert np.all(np.abs(got - Y_on_gpu_codes) <= 2.0 ** -8 * np.abs(Y_on_gpu_codes) + 1e-3 * rms)
+
+
 @pytest.mark.parametrize("T,E,k,d,f", [(64, 8, 2, 256, 512), (700, 4, 2, 384, 256), (300, 16, 4, 128, 128),
                                        (1500, 2, 1, 512, 640)])
 def test_ffn_fp8_against_oracle(T, E, k, d, f):
@@ -648,6 +657,9 @@ def test_ffn_fp8_against_oracle(T, E, k, d, f):
     assert np.all(np.abs(a - b) <= step * 1.0001)
     m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_o)
     assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
+    Y_own, _ = O.grouped_ffn_fp8(Xq, rs, off, r2a, W1q, s1, W3q, s3, W2q, s2, hs, Hq_given=hq)
+    real = np.nonzero(r2a[:R] >= 0)[0]
+    check_down_projection_on_own_codes(host_bits(Y)[:R][real], Y_own[real])
 
 
 @pytest.mark.parametrize("which", ["C2s", "C3s"])
@@ -721,6 +733,8 @@ def test_ffn_fp8_ragged_token_tiles(rows, d, f):
     assert (Hq.cpu().numpy()[:R] != Hq_o).mean() <= 0.02
     m = O.ffn_error_metrics(O.bf16_bits_to_f64(host_bits(Y)[:R]), Y_o)
     assert m["max_abs_err_over_rms"] <= FFN_MAX and m["mean_rel_err"] <= FFN_MEAN, m
+    Y_own, _ = O.grouped_ffn_fp8(Xq, rs, off, r2a, W1q, s1, W3q, s3, W2q, s2, hs, Hq_given=Hq.cpu().numpy()[:R])
+    check_down_projection_on_own_codes(host_bits(Y)[:R], Y_own)
 
 
 # ================================================================== f4: split-K for few active experts
