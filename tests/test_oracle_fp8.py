@@ -89,6 +89,19 @@ def test_fp8_ffn_reduces_to_the_plain_definition():
     assert np.allclose(Y2, 2 * Y, rtol=1e-12)
     Y3, _ = O.grouped_ffn_fp8(Xq, np.ones(E * n, np.float32), np.array([0, 0, 2 * n]), r2a, W1q, one, W3q, one, W2q, one, hs)
     assert Y3.shape == Y.shape
+    # Hq_given: the down projection on given codes.  The computed codes give the same Y bit for bit; ONE code moved to
+    # another e4m3 value changes exactly its row, by (new - old) * hs * w2[:, that feature] (hand formula, not the oracle's)
+    Yg, Hq2 = O.grouped_ffn_fp8(Xq, np.ones(E * n, np.float32), off, r2a, W1q, one, W3q, one, W2q, one, hs, Hq_given=Hq)
+    assert np.array_equal(Yg, Y) and np.array_equal(Hq2, Hq)
+    alt = Hq.copy()
+    r, c = n + 3, 5                                              # a row of expert 1
+    alt[r, c] = 0x38 if Hq[r, c] != 0x38 else 0x40               # 1.0 (or 2.0)
+    Ya, Hq3 = O.grouped_ffn_fp8(Xq, np.ones(E * n, np.float32), off, r2a, W1q, one, W3q, one, W2q, one, hs, Hq_given=alt)
+    assert np.array_equal(Hq3, Hq)                               # the returned codes are the computed ones
+    delta = (float(t[alt[r, c]]) - float(t[Hq[r, c]])) * float(hs[1]) * t[W2q[1]][:, c]
+    assert np.allclose(Ya[r] - Y[r], delta, rtol=1e-9, atol=1e-12)
+    others = np.ones(E * n, bool); others[r] = False
+    assert np.array_equal(Ya[others], Y[others])
 
 
 def test_fp8_pipeline_close_to_the_bf16_ffn():
@@ -306,6 +319,17 @@ def test_mx_ffn_reduces_to_the_plain_definition_and_tracks_the_bf16_ffn():
         assert np.allclose(Y[rows], y.numpy(), rtol=1e-12, atol=1e-300)
     Y2, _, _ = O.grouped_ffn_mxfp8(Xq, Xs, off, r2a, W1q, W1s, W3q, W3s, W2q, W2s + np.uint8(3))
     assert np.allclose(Y2, 8.0 * Y, rtol=1e-15)
+    # H_given: the down projection on given codes and scales -- the computed ones reproduce Y; one block's scale byte
+    # raised by 1 doubles that block's contribution to its row (torch-decoded hand formula) and nothing else
+    Yg, Hq2, Hs2 = O.grouped_ffn_mxfp8(Xq, Xs, off, r2a, W1q, W1s, W3q, W3s, W2q, W2s, H_given=(Hq, Hs))
+    assert np.array_equal(Yg, Y) and np.array_equal(Hq2, Hq) and np.array_equal(Hs2, Hs)
+    r = int(off[1]) + 2
+    Hs_alt = Hs.copy(); Hs_alt[r, 1] += 1
+    Ya = O.grouped_ffn_mxfp8(Xq, Xs, off, r2a, W1q, W1s, W3q, W3s, W2q, W2s, H_given=(Hq, Hs_alt))[0]
+    blk = deq(Hq[r:r + 1], Hs[r:r + 1])[:, 32:64] @ deq(W2q[1], W2s[1])[:, 32:64].T
+    assert np.allclose(Ya[r] - Y[r], blk.numpy()[0], rtol=1e-9, atol=1e-12)
+    others = np.ones(Y.shape[0], bool); others[r] = False
+    assert np.array_equal(Ya[others], Y[others])
     m = O.ffn_error_metrics(Y, Y_ref)
     W1p, s1 = O.fp8_pack_weights(L["W1"]); W3p, s3 = O.fp8_pack_weights(L["W3"]); W2p, s2 = O.fp8_pack_weights(L["W2"])
     Xr, rs = O.fp8_quantize_rows(Xp)
