@@ -742,9 +742,15 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     v += __shfl_xor_sync(FULL, v, 2);
     return v + __shfl_xor_sync(FULL, v, 1);
   };
-  const uint32_t e0 = (uint32_t)(sub * VPL);
+  // Which experts a lane holds.  GROUPED: VPL consecutive ones (a group is one lane's experts).  Otherwise the
+  // 16-byte chunks of the row are dealt round the 8 lanes -- chunk q * 8 + sub at step q, experts 32 q + 4 sub + c:
+  // the 8 lanes of a token read 128 contiguous bytes of the staged row (no bank conflict, no rotation), and the
+  // index byte of a key is a compile-time constant (255 - 32 q - c, inserted by one PRMT) less the lane's 4 sub,
+  // which comes off the five survivors of the network instead of off all VPL keys.
+  const uint32_t e0 = GROUPED ? (uint32_t)(sub * VPL) : (uint32_t)(4 * sub);
   const int k = p.k;
   const float* my_bias = s_bias + sub * (VPL + 1);
+  const float* il_bias = s_bias + (VPL == 32 ? 4 * sub : (sub >= 4 ? 4 * sub + 1 : 4 * sub));     // interleaved mapping: see below
   // f32 key -> order-preserving u32 with the low byte set (the caller subtracts the index): -0 -> +0 first
   auto packed_hi = [](float key) {
     const uint32_t b = __float_as_uint(__fadd_rn(key, 0.0f));
@@ -770,7 +776,8 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
   // in rotated order (chunk (q + rot) mod CH at step q), which spreads the 8 lanes over all 32 banks
   constexpr int CH = VPL / 4;
   const int rot = sub / (8 / CH);
-  const uint4* my_row4 = reinterpret_cast<const uint4*>(s_stage + (size_t)warp * TILE_BYTES) + (lane >> 3) * (E / 4) + sub * CH;
+  const uint4* my_row4 = reinterpret_cast<const uint4*>(s_stage + (size_t)warp * TILE_BYTES) + (lane >> 3) * (E / 4) +
+                         (GROUPED ? sub * CH : sub);
 
   uint32_t phase = 0;
   while (tile < n_tiles) {
@@ -785,15 +792,32 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     if (phase == 0 && tr1 == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr1));
 #endif
     phase ^= 1u;
+    if (GROUPED) {
 #pragma unroll
-    for (int q = 0; q < CH; ++q) {
-      const int ch = (q + rot) & (CH - 1);
-      const uint4 u = my_row4[ch];
-      const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+      for (int q = 0; q < CH; ++q) {
+        const int ch = (q + rot) & (CH - 1);
+        const uint4 u = my_row4[ch];
+        const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const float key = SIGMOID ? __fadd_rn(approx_sig(xv[c]), my_bias[4 * ch + c]) : xv[c];
-        pk[4 * q + c] = packed_hi(key) - (uint32_t)(4 * ch) - (uint32_t)c;
+        for (int c = 0; c < 4; ++c) {
+          const float key = SIGMOID ? __fadd_rn(approx_sig(xv[c]), my_bias[4 * ch + c]) : xv[c];
+          pk[4 * q + c] = packed_hi(key) - (uint32_t)(4 * ch) - (uint32_t)c;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < CH; ++q) {
+        const uint4 u = my_row4[q * 8];
+        const float xv[4] = {__uint_as_float(u.x), __uint_as_float(u.y), __uint_as_float(u.z), __uint_as_float(u.w)};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          // (the bias of expert e = 32 q + 4 sub + c in the padded [8][VPL + 1] layout)
+          const int eb = 32 * q + c;                                     // + 4 sub
+          const float key = SIGMOID ? __fadd_rn(approx_sig(xv[c]), il_bias[(eb / VPL) * (VPL + 1) + eb % VPL]) : xv[c];
+          const uint32_t bq = __float_as_uint(__fadd_rn(key, 0.0f));
+          const uint32_t tq = (uint32_t)((int32_t)bq >> 31) | 0x80000000u;
+          pk[4 * q + c] = __byte_perm(bq ^ tq, 255u - (uint32_t)(32 * q + c), 0x3214);
+        }
       }
     }
     // every lane has consumed its part of the buffer: the next tile's copy may overwrite it
@@ -880,7 +904,7 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
         bool hard = unsure || ran_out || (SIGMOID && collide);
         if (!SIGMOID) {
           uint32_t lo = 0;                       // OR of the raw bits of the lane's keys (reloaded: L2 hits)
-          const uint4* grow4 = reinterpret_cast<const uint4*>(row + e0);
+          const uint4* grow4 = reinterpret_cast<const uint4*>(row + sub * VPL);      // (any partition of the row does)
 #pragma unroll
           for (int q = 0; q < CH; ++q) {
             const uint4 u = __ldg(grow4 + q);
