@@ -153,7 +153,8 @@ perm_index_kernel(const int32_t* __restrict__ ids, const int32_t* __restrict__ e
   // NG row groups; group g takes rows g, g + NG, ... ----
   for (int s0 = 0; s0 < E_loc; s0 += kIdxThreads) {
     const int W = min(E_loc - s0, kIdxThreads);
-    const int NG = kIdxThreads / W;
+    // (row groups beyond G would have no row; the sums below run over NG: 128 -> 8 terms at 8 slots and 8 CTAs, 0.8 us)
+    const int NG = min(kIdxThreads / W, G);
     const int g = tid / W, c = tid - g * W;
     int pre = 0, total = 0;
     if (g < NG) {
