@@ -840,10 +840,11 @@ def main():
         json.dump(rep, fh, indent=1)
     if "profile" in rep:
         with open(args.out.replace(".json", "") + ".profile.csv", "w") as fh:
-            fh.write("shape,mode,tokens_per_expert,latency_us,p10_us,p90_us\n")
+            fh.write("shape,mode,tokens_per_expert,latency_us,p10_us,p90_us,fp8_latency_us,mxfp8_latency_us\n")
             for name, p in rep["profile"].items():
                 for r in p["rows"]:
-                    fh.write(f"{name},{r['mode']},{r['tokens_per_expert']},{r['latency_us']},{r['p10_us']},{r['p90_us']}\n")
+                    fh.write(f"{name},{r['mode']},{r['tokens_per_expert']},{r['latency_us']},{r['p10_us']},{r['p90_us']},"
+                             f"{r.get('fp8_latency_us', '')},{r.get('mxfp8_latency_us', '')}\n")
     if args.md:
         write_markdown(rep, args.md, "python -m paper_2606_00735_b200.report " + " ".join(sys.argv[1:]))
     print("wrote", args.out)
