@@ -715,10 +715,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     *s_redo_n = 0;
   }
   int tile = warp * gridDim.x + blockIdx.x;
-#ifdef ROUTE_TRACE
-  unsigned long long tr0, tr1 = 0, tr2;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr0));
-#endif
   if (lane == 0) {
     ptx::mbar_init(my_bar, 1);
     ptx::fence_barrier_init();
@@ -788,9 +784,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     const float* row = p.logits + (size_t)t * E;
     uint32_t pk[VPL];                          // packed keys with the IN-LANE index (low byte 255 - v)
     ptx::mbar_wait(my_bar, phase);
-#ifdef ROUTE_TRACE
-    if (phase == 0 && tr1 == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr1));
-#endif
     phase ^= 1u;
     if (GROUPED) {
 #pragma unroll
@@ -959,9 +952,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
       atomicAdd(&s_hist[my_id], 1);
     }
   }
-#ifdef ROUTE_TRACE
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr2));
-#endif
   __syncthreads();
   {
     const int n_redo = min(*s_redo_n, ROUTE8P_REDO_CAP);
@@ -974,16 +964,6 @@ __global__ void __launch_bounds__(ROUTE8P_WARPS * 32, 1) route_topk8p_kernel(con
     const int c = s_hist[i];
     if (c) atomicAdd(&p.counts[i], c);
   }
-#ifdef ROUTE_TRACE
-  if (lane == 0) {          // debug build only: the trace overwrites the first gate weights
-    unsigned long long tr3;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tr3));
-    unsigned long long* o = reinterpret_cast<unsigned long long*>(p.w) + (size_t)(blockIdx.x * NW + warp) * 5;
-    unsigned smid;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-    o[0] = tr0; o[1] = tr1; o[2] = tr2; o[3] = tr3; o[4] = smid;
-  }
-#endif
 }
 
 template <int VPL>
