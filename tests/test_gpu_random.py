@@ -141,3 +141,21 @@ def test_layer_random_configs(seed):
         none = np.nonzero(~(slot >= 0).any(axis=1))[0]
         if len(none):
             assert torch.count_nonzero(out[torch.from_numpy(none[:256]).cuda()].view(torch.int16)).item() == 0, tag
+
+
+@pytest.mark.parametrize("seed", range(2))
+def test_fp8_ffn_random_ragged_segments(seed):
+    """Both FP8 kinds on random ragged segment lists around the tile boundaries (the bodies of the fixed ragged tests:
+    H codes within one step, GEMM-2 on the device's own codes element by element, Y at the stated bars)."""
+    from test_gpu_mxfp8 import test_ffn_mxfp8_ragged_token_tiles
+    from test_gpu_parity import test_ffn_fp8_ragged_token_tiles
+    rng = np.random.default_rng(4000 + seed)
+    pool = [0, 1, 15, 16, 17, 31, 33, 63, 64, 65, 127, 128, 129, 191, 192, 193, 255, 256, 257, 383, 385, 511, 513, 769]
+    for case in range(4):
+        E = int(rng.choice([2, 3, 5, 8]))
+        rows = [int(x) for x in rng.choice(pool, E)]
+        if sum(rows) == 0:
+            rows[0] = 40
+        d, f = int(rng.choice([128, 256, 384])), int(rng.choice([128, 256, 640]))
+        test_ffn_fp8_ragged_token_tiles(rows, d, f)
+        test_ffn_mxfp8_ragged_token_tiles(rows, d, f)
